@@ -1,0 +1,644 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, obviously-correct CPU implementation of the hot path of arXiv 1606.03743
+// (Glueck & Hilk): potential and field of constant-sigma BEM triangles / rectangles by
+// Gaussian cubature (Eq. 4.1), the distance-ratio rule choice of Sec. 4 (L159), an analytic
+// near-field formula, and the collocation-matrix entries that follow from them.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+// may build, load or call this file.  It shares NO code with the CUDA library
+// (paper_1606_03743_b200/csrc): no headers, no tables, no helpers.  The product path never
+// routes through it.
+//
+// Every function cites the passage of /root/reference/PAPER.md it follows.  Arithmetic is
+// long double (x87 80-bit) in the parity instantiation; a double instantiation of the very
+// same template is what bench.py times as the CPU baseline.  No blocking, fusion or
+// reordering beyond the paper's statement: per field point, elements in index order, the
+// rule's points in table order.
+//
+// Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`):
+//   tables      : sum w = 1, exact monomial integrals up to the stated degree, failure at d+1
+//   mapping     : sum q_i = sigma*A, first moment about the centroid vanishes
+//   Eq. 4.1 sum : far-field point-charge limit; closed-form on-axis rectangle potential/field
+//                 (also for two triangles tiling the rectangle); uniformly charged sphere;
+//                 E = -grad Phi by central differences
+//   analytic    : closed forms (square centre, equilateral centroid, on-axis rectangle),
+//                 GL2 16 vs 32, long-double adaptive quadrature on tiny inputs
+//   KATRIN Table 1 numbers: parity unpinned (meshes not available).
+//
+// Build: g++ -O2 -std=c++17 -fopenmp -shared -fPIC bem_oracle.cpp -o liboracle.so
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+#include "rule_tables.hpp"
+
+namespace orc {
+
+// CODATA-2018 vacuum permittivity (paper gives no value; DESIGN.md §3 reading 10).
+static const long double EPS0 = 8.8541878128e-12L;
+static const long double PI_L = 3.14159265358979323846264338327950288L;
+inline long double coulomb_k() { return 1.0L / (4.0L * PI_L * EPS0); }
+
+enum { TRI = 0, RECT = 1 };
+enum { ERR_OK = 0, ERR_INVALID = -1, ERR_DEGENERATE = -2, ERR_NOT_RECT = -3, ERR_BAD_RULE = -4 };
+
+template <class T> inline T tsqrt(T x);
+template <> inline long double tsqrt(long double x) { return sqrtl(x); }
+template <> inline double tsqrt(double x) { return sqrt(x); }
+template <class T> inline T tlog(T x);
+template <> inline long double tlog(long double x) { return logl(x); }
+template <> inline double tlog(double x) { return log(x); }
+template <class T> inline T tatan(T x);
+template <> inline long double tatan(long double x) { return atanl(x); }
+template <> inline double tatan(double x) { return atan(x); }
+template <class T> inline T tabs(T x) { return x < 0 ? -x : x; }
+
+template <class T> struct V3 { T x, y, z; };
+template <class T> inline V3<T> sub(const V3<T>& a, const V3<T>& b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+template <class T> inline T dot(const V3<T>& a, const V3<T>& b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+template <class T> inline V3<T> cross(const V3<T>& a, const V3<T>& b) {
+    return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+template <class T> inline T norm(const V3<T>& a) { return tsqrt<T>(dot(a, a)); }
+
+// ---------------------------------------------------------------------------------------
+// Geometry of one element.  Triangle: vertices A,B,C (Eq. 3.3).  Rectangle: corner
+// P0, P1 = P0 + a u_x, P3 = P0 + b u_y; centre, side lengths and side unit vectors as in
+// Eq. 3.2 (L101-105).  L = average side length (L66): (a+b+c)/3 for the triangle, (a+b)/2
+// for the rectangle (DESIGN.md §3 reading 6).
+template <class T> struct Geom {
+    int type;
+    V3<T> v[4];     // polygon vertices in order (3 or 4)
+    int nv;
+    V3<T> cen;      // Q_cen
+    T area;         // script-A
+    T L;            // average side length
+    V3<T> hx, hy;   // rectangle: (a/2) u_x, (b/2) u_y
+};
+
+template <class T>
+int make_geom(int type, const double* vv, Geom<T>& g) {
+    V3<T> p0{(T)vv[0], (T)vv[1], (T)vv[2]}, p1{(T)vv[3], (T)vv[4], (T)vv[5]}, p2{(T)vv[6], (T)vv[7], (T)vv[8]};
+    g.type = type;
+    if (type == TRI) {
+        g.nv = 3;
+        g.v[0] = p0; g.v[1] = p1; g.v[2] = p2;
+        V3<T> e1 = sub(p1, p0), e2 = sub(p2, p0);
+        g.area = (T)0.5 * norm(cross(e1, e2));
+        g.cen = {(p0.x + p1.x + p2.x) / (T)3, (p0.y + p1.y + p2.y) / (T)3, (p0.z + p1.z + p2.z) / (T)3};
+        g.L = (norm(sub(p1, p0)) + norm(sub(p2, p1)) + norm(sub(p0, p2))) / (T)3;
+        g.hx = g.hy = {0, 0, 0};
+        if (!(g.area > 0)) return ERR_DEGENERATE;
+    } else if (type == RECT) {
+        g.nv = 4;
+        V3<T> e1 = sub(p1, p0), e2 = sub(p2, p0);
+        T a = norm(e1), b = norm(e2);
+        if (!(a > 0) || !(b > 0)) return ERR_DEGENERATE;
+        if (tabs(dot(e1, e2)) > (T)1e-12 * a * b) return ERR_NOT_RECT;
+        g.v[0] = p0; g.v[1] = p1;
+        g.v[2] = {p1.x + e2.x, p1.y + e2.y, p1.z + e2.z};
+        g.v[3] = p2;
+        g.area = a * b;
+        g.cen = {p0.x + (T)0.5 * e1.x + (T)0.5 * e2.x, p0.y + (T)0.5 * e1.y + (T)0.5 * e2.y,
+                 p0.z + (T)0.5 * e1.z + (T)0.5 * e2.z};
+        g.L = (a + b) / (T)2;
+        // (a/2) u_x = e1/2, (b/2) u_y = e2/2
+        g.hx = {(T)0.5 * e1.x, (T)0.5 * e1.y, (T)0.5 * e1.z};
+        g.hy = {(T)0.5 * e2.x, (T)0.5 * e2.y, (T)0.5 * e2.z};
+    } else {
+        return ERR_INVALID;
+    }
+    return ERR_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// Gaussian points Q_i and relative weights w_i of one element for one rule level.
+// Triangle: Q = lA*A + lB*B + lC*C (Eq. 3.3).  Rectangle: Q = Q_cen + (a/2) x u_x +
+// (b/2) y u_y (Eq. 3.2).
+template <class T> struct Pt { T x, y, z, w; };
+
+template <class T>
+void element_points(const Geom<T>& g, int level, std::vector<Pt<T>>& out) {
+    out.clear();
+    if (g.type == TRI) {
+        for (const TriNode& nd : tri_rule(level)) {
+            T la = (T)nd.la, lb = (T)nd.lb, lc = (T)nd.lc;
+            out.push_back({la * g.v[0].x + lb * g.v[1].x + lc * g.v[2].x,
+                           la * g.v[0].y + lb * g.v[1].y + lc * g.v[2].y,
+                           la * g.v[0].z + lb * g.v[1].z + lc * g.v[2].z, (T)nd.w});
+        }
+    } else {
+        for (const RectNode& nd : rect_rule(level)) {
+            T x = (T)nd.x, y = (T)nd.y;
+            out.push_back({g.cen.x + x * g.hx.x + y * g.hy.x, g.cen.y + x * g.hx.y + y * g.hy.y,
+                           g.cen.z + x * g.hx.z + y * g.hy.z, (T)nd.w});
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// Analytic near-field integrals of a flat polygon (the paper cites but does not print its
+// analytic formulas, L68/L78; DESIGN.md §3 reading 9 takes this exact closed form of
+// Eq. 2.1, a line-integral form of the same family as Ref. [27]):
+//   I_phi = Int dS / R,  I_E = Int dS (P-Q)/R^3     (unit sigma, no 1/(4 pi eps0))
+// With n the unit normal, h = n.(P - V0), and per edge V- -> V+:
+//   l = unit edge vector, u = l x n (outward in-plane normal), s+- = (V+- - P).l,
+//   t0 = (V- - P).u, R+- = |P - V+-|, R0^2 = t0^2 + h^2,
+//   f  = ln[(R+ + s+)/(R- + s-)] written in the cancellation-free equivalent form for the
+//        sign pattern of s+-,
+//   beta = atan(t0 s+ /(R0^2 + |h| R+)) - atan(t0 s- /(R0^2 + |h| R-)),
+//   I_phi = sum_i (t0 f - |h| beta),  I_E = sgn(h) n sum_i beta + sum_i u f.
+// An edge whose line contains P (R0 = 0) contributes 0 to I_phi; its f is finite unless P
+// lies on the edge segment itself (then the in-plane field is log-singular: inf).
+template <class T>
+void analytic_integrals(const Geom<T>& g, const V3<T>& P, T& Iphi, V3<T>& IE) {
+    V3<T> nrm = cross(sub(g.v[1], g.v[0]), sub(g.v[g.nv - 1], g.v[0]));
+    T nn = norm(nrm);
+    nrm = {nrm.x / nn, nrm.y / nn, nrm.z / nn};
+    T h = dot(nrm, sub(P, g.v[0]));
+    T ah = tabs(h);
+    T sg = (h > 0) ? (T)1 : ((h < 0) ? (T)-1 : (T)0);
+    Iphi = 0;
+    T sumbeta = 0;
+    IE = {0, 0, 0};
+    for (int i = 0; i < g.nv; ++i) {
+        const V3<T>& Vm = g.v[i];
+        const V3<T>& Vp = g.v[(i + 1) % g.nv];
+        V3<T> l = sub(Vp, Vm);
+        T len = norm(l);
+        l = {l.x / len, l.y / len, l.z / len};
+        V3<T> u = cross(l, nrm);
+        V3<T> dm = sub(Vm, P), dp = sub(Vp, P);
+        T sp = dot(dp, l), sm = dot(dm, l), t0 = dot(dm, u);
+        T Rp = norm(dp), Rm = norm(dm);
+        T R02 = t0 * t0 + h * h;
+        T f, beta = 0;
+        if (sp < 0 && sm < 0)        f = tlog<T>((Rm - sm) / (Rp - sp));
+        else if (sm < 0) {           // s- < 0 <= s+ : R- + s- = R0^2 / (R- - s-)
+            if (R02 > 0) f = tlog<T>((Rp + sp) * (Rm - sm) / R02);
+            else         f = (T)INFINITY;                 // P on the edge segment
+        } else                       f = tlog<T>((Rp + sp) / (Rm + sm));
+        if (R02 > 0) {
+            beta = tatan<T>(t0 * sp / (R02 + ah * Rp)) - tatan<T>(t0 * sm / (R02 + ah * Rm));
+            Iphi += t0 * f - ah * beta;
+        }
+        sumbeta += beta;
+        IE.x += u.x * f; IE.y += u.y * f; IE.z += u.z * f;
+    }
+    IE.x += sg * nrm.x * sumbeta; IE.y += sg * nrm.y * sumbeta; IE.z += sg * nrm.z * sumbeta;
+}
+
+// ---------------------------------------------------------------------------------------
+// Gauss-Legendre nodes on [-1,1] by Newton iteration on P_n (used by GL2 and by the adaptive
+// reference).  Textbook; pinned in the tests by exact polynomial integration.
+static void gauss_legendre(int n, std::vector<long double>& x, std::vector<long double>& w) {
+    x.resize(n); w.resize(n);
+    for (int i = 0; i < n; ++i) {
+        long double z = cosl(PI_L * (i + 0.75L) / (n + 0.5L));
+        long double pp = 1;
+        for (int it = 0; it < 100; ++it) {
+            long double p1 = 1, p2 = 0;
+            for (int j = 1; j <= n; ++j) {
+                long double p3 = p2; p2 = p1;
+                p1 = ((2 * j - 1) * z * p2 - (j - 1) * p3) / j;
+            }
+            pp = n * (z * p1 - p2) / (z * z - 1);
+            long double dz = p1 / pp;
+            z -= dz;
+            if (fabsl(dz) < 1e-21L) break;
+        }
+        // recompute derivative at converged z
+        long double p1 = 1, p2 = 0;
+        for (int j = 1; j <= n; ++j) { long double p3 = p2; p2 = p1; p1 = ((2 * j - 1) * z * p2 - (j - 1) * p3) / j; }
+        pp = n * (z * p1 - p2) / (z * z - 1);
+        x[i] = z;
+        w[i] = 2 / ((1 - z * z) * pp * pp);
+    }
+}
+
+struct F4 { long double v[4]; };
+
+// integrand of Eq. 2.1 (L64) at surface point Q, times the area Jacobian jac
+static inline void coulomb_integrand(const V3<long double>& P, const V3<long double>& Q, long double jac, F4& acc) {
+    V3<long double> d = sub(P, Q);
+    long double r2 = dot(d, d), r = sqrtl(r2), i3 = jac / (r2 * r);
+    acc.v[0] += jac / r; acc.v[1] += d.x * i3; acc.v[2] += d.y * i3; acc.v[3] += d.z * i3;
+}
+
+// surface point and Jacobian for parameters (s,t) in [0,1]^2.
+// Rectangle: x = 2s-1, y = 2t-1 in Eq. 3.2, dS = area ds dt.
+// Triangle: collapsed map Q = A + s(B-A) + t(1-s)(C-A), dS = 2*area*(1-s) ds dt.
+static inline void surface_point(const Geom<long double>& g, long double s, long double t,
+                                 V3<long double>& Q, long double& jac) {
+    if (g.type == RECT) {
+        long double x = 2 * s - 1, y = 2 * t - 1;
+        Q = {g.cen.x + x * g.hx.x + y * g.hy.x, g.cen.y + x * g.hx.y + y * g.hy.y, g.cen.z + x * g.hx.z + y * g.hy.z};
+        jac = g.area;
+    } else {
+        V3<long double> e1 = sub(g.v[1], g.v[0]), e2 = sub(g.v[2], g.v[0]);
+        long double c = t * (1 - s);
+        Q = {g.v[0].x + s * e1.x + c * e2.x, g.v[0].y + s * e1.y + c * e2.y, g.v[0].z + s * e1.z + c * e2.z};
+        jac = 2 * g.area * (1 - s);
+    }
+}
+
+// GL2: two successive one-dimensional Gauss-Legendre quadratures with n nodes each (L40, L78).
+static void gl2_integrals(const Geom<long double>& g, const V3<long double>& P, int n, F4& out) {
+    std::vector<long double> x, w;
+    gauss_legendre(n, x, w);
+    out = F4{{0, 0, 0, 0}};
+    for (int i = 0; i < n; ++i) {
+        F4 inner{{0, 0, 0, 0}};
+        long double s = 0.5L * (x[i] + 1);
+        for (int j = 0; j < n; ++j) {
+            long double t = 0.5L * (x[j] + 1), jac;
+            V3<long double> Q;
+            surface_point(g, s, t, Q, jac);
+            coulomb_integrand(P, Q, jac * 0.25L * w[j], inner);
+        }
+        for (int k = 0; k < 4; ++k) out.v[k] += w[i] * inner.v[k];
+    }
+}
+
+// Adaptive reference: nested 1-D adaptive bisection, each panel integrated with GL-12 and
+// accepted when it agrees with the sum of its two half panels (brute force for tiny inputs).
+struct Adaptive {
+    const Geom<long double>& g;
+    V3<long double> P;
+    std::vector<long double> x, w;
+    long double scale[4];
+    long double tol;
+    long double err;
+    Adaptive(const Geom<long double>& g_, const V3<long double>& P_, long double tol_) : g(g_), P(P_), tol(tol_), err(0) {
+        gauss_legendre(12, x, w);
+    }
+    F4 inner_panel(long double s, long double a, long double b) const {
+        F4 r{{0, 0, 0, 0}};
+        for (size_t j = 0; j < x.size(); ++j) {
+            long double t = 0.5L * ((b - a) * x[j] + (a + b)), jac;
+            V3<long double> Q;
+            surface_point(g, s, t, Q, jac);
+            coulomb_integrand(P, Q, jac * 0.5L * (b - a) * w[j], r);
+        }
+        return r;
+    }
+    bool close(const F4& a, const F4& b, long double frac, long double t) const {
+        for (int k = 0; k < 4; ++k)
+            if (fabsl(a.v[k] - b.v[k]) > t * frac * scale[k]) return false;
+        return true;
+    }
+    F4 inner_rec(long double s, long double a, long double b, const F4& whole, int depth) const {
+        long double m = 0.5L * (a + b);
+        F4 l = inner_panel(s, a, m), r = inner_panel(s, m, b), sum;
+        for (int k = 0; k < 4; ++k) sum.v[k] = l.v[k] + r.v[k];
+        if (depth > 48 || close(whole, sum, b - a, tol * 0.1L)) return sum;
+        F4 L2 = inner_rec(s, a, m, l, depth + 1), R2 = inner_rec(s, m, b, r, depth + 1);
+        for (int k = 0; k < 4; ++k) sum.v[k] = L2.v[k] + R2.v[k];
+        return sum;
+    }
+    F4 inner(long double s) const { return inner_rec(s, 0, 1, inner_panel(s, 0, 1), 0); }
+    F4 outer_panel(long double a, long double b) const {
+        F4 r{{0, 0, 0, 0}};
+        for (size_t i = 0; i < x.size(); ++i) {
+            long double s = 0.5L * ((b - a) * x[i] + (a + b));
+            F4 in = inner(s);
+            for (int k = 0; k < 4; ++k) r.v[k] += 0.5L * (b - a) * w[i] * in.v[k];
+        }
+        return r;
+    }
+    F4 outer_rec(long double a, long double b, const F4& whole, int depth) {
+        long double m = 0.5L * (a + b);
+        F4 l = outer_panel(a, m), r = outer_panel(m, b), sum;
+        for (int k = 0; k < 4; ++k) sum.v[k] = l.v[k] + r.v[k];
+        if (depth > 48 || close(whole, sum, b - a, tol)) {
+            for (int k = 0; k < 4; ++k) err = std::max(err, fabsl(whole.v[k] - sum.v[k]) / scale[k]);
+            return sum;
+        }
+        F4 L2 = outer_rec(a, m, l, depth + 1), R2 = outer_rec(m, b, r, depth + 1);
+        for (int k = 0; k < 4; ++k) sum.v[k] = L2.v[k] + R2.v[k];
+        return sum;
+    }
+    F4 run() {
+        F4 est;
+        gl2_integrals(g, P, 16, est);
+        scale[0] = fabsl(est.v[0]);
+        long double e = sqrtl(est.v[1] * est.v[1] + est.v[2] * est.v[2] + est.v[3] * est.v[3]);
+        // field scale: never smaller than potential/distance so that symmetric zeros do not stall
+        long double D = norm(sub(P, g.cen));
+        scale[1] = scale[2] = scale[3] = std::max(e, scale[0] / std::max(D, g.L));
+        return outer_rec(0, 1, outer_panel(0, 1), 0);
+    }
+};
+
+// ---------------------------------------------------------------------------------------
+// Distance-ratio rule choice (L66, L159).  dr[type][0..4] = upper DR limits of
+// {analytic, N=33, N=19|17, N=12, N=7}; N=4 above dr[type][4].  Bands are lower-inclusive
+// (DESIGN.md §3 reading 8).  The decision is taken in double precision by comparing D^2 with
+// (limit*L)^2.  Returns 0..4 = rule level (N = 4,7,12,19|17,33), 5 = analytic.
+// levels_mask: bit k enables level k, bit 5 enables the analytic branch; a disabled choice
+// moves to the next more accurate enabled one (and, if none, to the most accurate enabled).
+static int choose_level(double D2, double L, const double* dr5, int levels_mask) {
+    int want = 0;                                 // band -> level: band 0 = analytic (5), 1 -> 4, 2 -> 3, 3 -> 2, 4 -> 1
+    for (int b = 0; b < 5; ++b) {
+        double thr = dr5[b] * L;
+        if (D2 < thr * thr) { want = (b == 0) ? 5 : 5 - b; break; }
+    }
+    for (int lv = want; lv <= 5; ++lv)
+        if (levels_mask & (1 << lv)) return lv;
+    for (int lv = want - 1; lv >= 0; --lv)
+        if (levels_mask & (1 << lv)) return lv;
+    return -1;
+}
+
+// ---------------------------------------------------------------------------------------
+// Eq. 4.1 (L139-143): Phi(P) = k sum q_i / |P-Q_i|,  E(P) = k sum q_i (P-Q_i)/|P-Q_i|^3,
+// q_i = w_i sigma A; summed over all elements for each field point (L34, L202).
+template <class T>
+int eval_impl(int64_t n, const uint8_t* etype, const double* verts, const double* sigma, int level,
+              const double* dr, int levels_mask, int64_t m, const double* pts, double* phi, double* E,
+              double* Sphi, double* SE, int64_t* npi, int nthreads) {
+    if (n < 0 || m < 0) return ERR_INVALID;
+    if (level < -1 || level > 4) return ERR_BAD_RULE;
+    if (level == -1 && (!dr || (levels_mask & 63) == 0)) return ERR_INVALID;
+    // validate geometry once
+    for (int64_t e = 0; e < n; ++e) {
+        Geom<T> g;
+        int rc = make_geom<T>(etype[e], verts + 9 * e, g);
+        if (rc) return rc;
+    }
+    const int64_t BS = 32;
+    const int64_t nblocks = (m + BS - 1) / BS;
+    const T k = (T)coulomb_k();
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t b = 0; b < nblocks; ++b) {
+        const int64_t j0 = b * BS, j1 = std::min(m, j0 + BS);
+        T aphi[BS], aex[BS], aey[BS], aez[BS], asphi[BS], ase[BS];
+        int64_t cnt[BS];
+        for (int64_t j = 0; j < BS; ++j) { aphi[j] = aex[j] = aey[j] = aez[j] = asphi[j] = ase[j] = 0; cnt[j] = 0; }
+        std::vector<Pt<T>> cache[5];
+        for (int64_t e = 0; e < n; ++e) {
+            Geom<T> g;
+            make_geom<T>(etype[e], verts + 9 * e, g);
+            bool have[5] = {false, false, false, false, false};
+            const T q = (T)sigma[e] * g.area;               // q = sigma * A (L143)
+            const double cx = (double)g.cen.x, cy = (double)g.cen.y, cz = (double)g.cen.z, Ld = (double)g.L;
+            for (int64_t j = j0; j < j1; ++j) {
+                const V3<T> P{(T)pts[3 * j], (T)pts[3 * j + 1], (T)pts[3 * j + 2]};
+                int lv = level;
+                if (level == -1) {
+                    double dx = pts[3 * j] - cx, dy = pts[3 * j + 1] - cy, dz = pts[3 * j + 2] - cz;
+                    lv = choose_level(dx * dx + dy * dy + dz * dz, Ld, dr + 5 * g.type, levels_mask);
+                }
+                const int jj = (int)(j - j0);
+                if (lv == 5) {
+                    T Ip; V3<T> Ie;
+                    analytic_integrals<T>(g, P, Ip, Ie);
+                    const T s = (T)sigma[e];
+                    aphi[jj] += s * Ip; aex[jj] += s * Ie.x; aey[jj] += s * Ie.y; aez[jj] += s * Ie.z;
+                    asphi[jj] += tabs(s * Ip);
+                    ase[jj] += tabs(s) * norm(Ie);
+                    continue;
+                }
+                if (!have[lv]) { element_points<T>(g, lv, cache[lv]); have[lv] = true; }
+                for (const Pt<T>& p : cache[lv]) {
+                    const T qi = p.w * q;                    // q_i = w_i q (L143)
+                    const T dx = P.x - p.x, dy = P.y - p.y, dz = P.z - p.z;
+                    const T r2 = dx * dx + dy * dy + dz * dz;
+                    const T inv = (T)1 / tsqrt<T>(r2);       // one square root, one division (L46)
+                    const T inv3 = inv * inv * inv;
+                    aphi[jj] += qi * inv;
+                    aex[jj] += qi * dx * inv3; aey[jj] += qi * dy * inv3; aez[jj] += qi * dz * inv3;
+                    asphi[jj] += tabs(qi) * inv;
+                    ase[jj] += tabs(qi) * inv * inv;
+                }
+                cnt[jj] += (int64_t)cache[lv].size();
+            }
+        }
+        for (int64_t j = j0; j < j1; ++j) {
+            const int jj = (int)(j - j0);
+            if (phi) phi[j] = (double)(k * aphi[jj]);
+            if (E) { E[3 * j] = (double)(k * aex[jj]); E[3 * j + 1] = (double)(k * aey[jj]); E[3 * j + 2] = (double)(k * aez[jj]); }
+            if (Sphi) Sphi[j] = (double)(k * asphi[jj]);
+            if (SE) SE[j] = (double)(k * ase[jj]);
+            if (npi) npi[j] = cnt[jj];
+        }
+    }
+    return ERR_OK;
+}
+
+}  // namespace orc
+
+using namespace orc;
+
+extern "C" {
+
+double orc_coulomb_k() { return (double)coulomb_k(); }
+
+int orc_rule_info(int etype, int level, int* npts, int* degree) {
+    if (level < 0 || level > 4 || (etype != TRI && etype != RECT)) return ERR_BAD_RULE;
+    if (etype == TRI) { if (npts) *npts = (int)tri_rule(level).size(); if (degree) *degree = tri_degree(level); }
+    else              { if (npts) *npts = (int)rect_rule(level).size(); if (degree) *degree = rect_degree(level); }
+    return ERR_OK;
+}
+
+// coords: triangle [N][3] barycentric, rectangle [N][2] natural; w: [N]
+int orc_rule_nodes(int etype, int level, double* coords, double* w) {
+    if (level < 0 || level > 4 || (etype != TRI && etype != RECT)) return ERR_BAD_RULE;
+    if (etype == TRI) {
+        auto r = tri_rule(level);
+        for (size_t i = 0; i < r.size(); ++i) { coords[3 * i] = (double)r[i].la; coords[3 * i + 1] = (double)r[i].lb; coords[3 * i + 2] = (double)r[i].lc; w[i] = (double)r[i].w; }
+    } else {
+        auto r = rect_rule(level);
+        for (size_t i = 0; i < r.size(); ++i) { coords[2 * i] = (double)r[i].x; coords[2 * i + 1] = (double)r[i].y; w[i] = (double)r[i].w; }
+    }
+    return ERR_OK;
+}
+
+// The residual |sum_i w_i m(Q_i) - exact| of monomial integration, evaluated in long double
+// (reference triangle (0,0),(1,0),(0,1): x^a y^b, exact a! b! 2/(a+b+2)! ; square [-1,1]^2:
+// x^a y^b, exact 1/((a+1)(b+1)) for even a,b else 0 — all relative to the area).  L113.
+double orc_rule_monomial_residual(int etype, int level, int a, int b) {
+    long double s = 0, exact;
+    if (etype == TRI) {
+        for (const TriNode& nd : tri_rule(level)) s += nd.w * powl(nd.lb, a) * powl(nd.lc, b);
+        long double num = 2;
+        for (int i = 2; i <= a; ++i) num *= i;
+        for (int i = 2; i <= b; ++i) num *= i;
+        long double den = 1;
+        for (int i = 2; i <= a + b + 2; ++i) den *= i;
+        exact = num / den;
+    } else {
+        for (const RectNode& nd : rect_rule(level)) s += nd.w * powl(nd.x, a) * powl(nd.y, b);
+        exact = (a % 2 == 0 && b % 2 == 0) ? 1.0L / ((a + 1) * (b + 1)) : 0.0L;
+    }
+    return (double)(s - exact);
+}
+
+int orc_geometry(int64_t n, const uint8_t* etype, const double* verts, double* cen, double* area, double* L) {
+    for (int64_t e = 0; e < n; ++e) {
+        Geom<long double> g;
+        int rc = make_geom<long double>(etype[e], verts + 9 * e, g);
+        if (rc) return rc;
+        if (cen) { cen[3 * e] = (double)g.cen.x; cen[3 * e + 1] = (double)g.cen.y; cen[3 * e + 2] = (double)g.cen.z; }
+        if (area) area[e] = (double)g.area;
+        if (L) L[e] = (double)g.L;
+    }
+    return ERR_OK;
+}
+
+// Expanded point charges of all elements for one rule level: xyzq[sumN][4] = (Q_i, q_i = w_i sigma A).
+// Returns the number of points written (or a negative error).
+int64_t orc_points(int64_t n, const uint8_t* etype, const double* verts, const double* sigma, int level, double* xyzq) {
+    if (level < 0 || level > 4) return ERR_BAD_RULE;
+    int64_t c = 0;
+    std::vector<Pt<long double>> p;
+    for (int64_t e = 0; e < n; ++e) {
+        Geom<long double> g;
+        int rc = make_geom<long double>(etype[e], verts + 9 * e, g);
+        if (rc) return rc;
+        element_points<long double>(g, level, p);
+        for (auto& q : p) {
+            if (xyzq) { xyzq[4 * c] = (double)q.x; xyzq[4 * c + 1] = (double)q.y; xyzq[4 * c + 2] = (double)q.z; xyzq[4 * c + 3] = (double)(q.w * (long double)sigma[e] * g.area); }
+            ++c;
+        }
+    }
+    return c;
+}
+
+// Default DR limits dr[2][5] ([0] = triangle, [1] = rectangle; entries = upper limits of
+// {analytic, N=33, N=19|17, N=12, N=7}).  want_field = 0: the printed triangle-potential
+// limits 3/8/20/80/1500 (L159), used for both element types (rectangle limits are not
+// printed); want_field = 1: limits for Phi and E together ("slightly higher", L159; values
+// re-derived with the paper's protocol, DESIGN.md §3 reading 7).
+int orc_default_policy(double* dr, int want_field) {
+    static const double pot[5] = {3, 8, 20, 80, 1500};
+    static const double ftri[5] = {4, 10, 25, 100, 2000};
+    static const double frect[5] = {6, 15, 40, 150, 3000};
+    for (int b = 0; b < 5; ++b) {
+        dr[b] = want_field ? ftri[b] : pot[b];
+        dr[5 + b] = want_field ? frect[b] : pot[b];
+    }
+    return ERR_OK;
+}
+
+int orc_choose_level(double D2, double L, const double* dr5, int levels_mask) { return choose_level(D2, L, dr5, levels_mask); }
+
+// precision: 0 = long double (parity), 1 = double (timed CPU baseline).  level -1 = adaptive.
+int orc_eval(int64_t n, const uint8_t* etype, const double* verts, const double* sigma, int level,
+             const double* dr, int levels_mask, int64_t m, const double* pts, double* phi, double* E,
+             double* Sphi, double* SE, int64_t* npi, int precision, int nthreads) {
+    if (precision == 0)
+        return eval_impl<long double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
+    return eval_impl<double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
+}
+
+// Unit-sigma integrals of Eq. 2.1 without the 1/(4 pi eps0) prefactor, three ways.
+int orc_analytic(int etype, const double* verts9, const double* P, double* Iphi, double* IE, int precision) {
+    if (precision == 0) {
+        Geom<long double> g;
+        int rc = make_geom<long double>(etype, verts9, g);
+        if (rc) return rc;
+        long double ip; V3<long double> ie;
+        analytic_integrals<long double>(g, {(long double)P[0], (long double)P[1], (long double)P[2]}, ip, ie);
+        *Iphi = (double)ip; IE[0] = (double)ie.x; IE[1] = (double)ie.y; IE[2] = (double)ie.z;
+    } else {
+        Geom<double> g;
+        int rc = make_geom<double>(etype, verts9, g);
+        if (rc) return rc;
+        double ip; V3<double> ie;
+        analytic_integrals<double>(g, {P[0], P[1], P[2]}, ip, ie);
+        *Iphi = ip; IE[0] = ie.x; IE[1] = ie.y; IE[2] = ie.z;
+    }
+    return ERR_OK;
+}
+
+int orc_gl2(int etype, const double* verts9, const double* P, int ngl, double* Iphi, double* IE) {
+    Geom<long double> g;
+    int rc = make_geom<long double>(etype, verts9, g);
+    if (rc) return rc;
+    F4 r;
+    gl2_integrals(g, {(long double)P[0], (long double)P[1], (long double)P[2]}, ngl, r);
+    *Iphi = (double)r.v[0]; IE[0] = (double)r.v[1]; IE[1] = (double)r.v[2]; IE[2] = (double)r.v[3];
+    return ERR_OK;
+}
+
+int orc_adaptive(int etype, const double* verts9, const double* P, double reltol, double* Iphi, double* IE, double* errest) {
+    Geom<long double> g;
+    int rc = make_geom<long double>(etype, verts9, g);
+    if (rc) return rc;
+    Adaptive a(g, {(long double)P[0], (long double)P[1], (long double)P[2]}, (long double)reltol);
+    F4 r = a.run();
+    *Iphi = (double)r.v[0]; IE[0] = (double)r.v[1]; IE[1] = (double)r.v[2]; IE[2] = (double)r.v[3];
+    if (errest) *errest = (double)a.err;
+    return ERR_OK;
+}
+
+int orc_gauss_legendre(int n, double* x, double* w) {
+    std::vector<long double> xx, ww;
+    gauss_legendre(n, xx, ww);
+    for (int i = 0; i < n; ++i) { x[i] = (double)xx[i]; w[i] = (double)ww[i]; }
+    return ERR_OK;
+}
+
+// Collocation-matrix rows (L34): A_ij = k * Int_{elem j} dS / |c_i - Q| with unit sigma,
+// c_i = centroid of element i; per pair the rule by DR(i,j) (L159), analytic below the first
+// limit (self term included: D = 0).  code[r][j] = level used (0..4) or 5 = analytic.
+int orc_assemble_rows(int64_t n, const uint8_t* etype, const double* verts, const double* dr, int levels_mask,
+                      int64_t nrows, const int64_t* rows, double* out, uint8_t* code, int precision, int nthreads) {
+    typedef long double T;
+    (void)precision;
+    std::vector<Geom<T>> G(n);
+    for (int64_t e = 0; e < n; ++e) {
+        int rc = make_geom<T>(etype[e], verts + 9 * e, G[e]);
+        if (rc) return rc;
+    }
+    const T k = coulomb_k();
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t r = 0; r < nrows; ++r) {
+        const int64_t i = rows[r];
+        const V3<T> P = G[i].cen;
+        const double px = (double)P.x, py = (double)P.y, pz = (double)P.z;
+        std::vector<Pt<T>> p;
+        for (int64_t j = 0; j < n; ++j) {
+            const Geom<T>& g = G[j];
+            double dx = px - (double)g.cen.x, dy = py - (double)g.cen.y, dz = pz - (double)g.cen.z;
+            int lv = choose_level(dx * dx + dy * dy + dz * dz, (double)g.L, dr + 5 * g.type, levels_mask);
+            T val = 0;
+            if (lv == 5) {
+                T ip; V3<T> ie;
+                analytic_integrals<T>(g, P, ip, ie);
+                val = ip;
+            } else {
+                element_points<T>(g, lv, p);
+                for (const Pt<T>& q : p) {
+                    const T ddx = P.x - q.x, ddy = P.y - q.y, ddz = P.z - q.z;
+                    val += q.w * g.area / sqrtl(ddx * ddx + ddy * ddy + ddz * ddz);
+                }
+            }
+            out[r * n + j] = (double)(k * val);
+            if (code) code[r * n + j] = (uint8_t)lv;
+        }
+    }
+    return ERR_OK;
+}
+
+int orc_num_threads() {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+}  // extern "C"
