@@ -1,0 +1,171 @@
+/*
+ * bemcub — C ABI of the B200 (sm_100a) library for the hot path of arXiv 1606.03743
+ * (Glueck & Hilk, "Electric potential and field calculation of charged BEM triangles and
+ * rectangles by Gaussian cubature").  Citations are to /root/reference/PAPER.md line numbers.
+ *
+ * What the library computes
+ *   Every constant-sigma triangle / rectangle is replaced by the N weighted point charges of one
+ *   of the paper's ten tabulated cubature rules (App. A/B, L283-386), q_i = w_i sigma A (L143),
+ *   placed at Q_i by Eq. 3.3 (triangle, L109) or Eq. 3.2 (rectangle, L103).  Potential and field
+ *   at a field point P are the direct sums of Eq. 4.1 (L139-143)
+ *       Phi(P) = k sum_i q_i / |P-Q_i|,   E(P) = k sum_i q_i (P-Q_i) / |P-Q_i|^3,   k = 1/(4 pi eps0)
+ *   over all points of all elements (L34, L202).  In distance-ratio-adaptive mode the rule of each
+ *   (element, field point) pair is picked from DR = |P - Q_cen| / L (L66) by the limits of Sec. 4
+ *   (L159), and pairs below the first limit use an exact closed-form integral of Eq. 2.1 (L62-64)
+ *   instead.  The dense BEM collocation matrix (L34) is the same computation with unit sigma and
+ *   the element centroids as field points, one entry per (row = field point, column = element).
+ *
+ * General conventions
+ *   - Unless a parameter is marked HOST, every pointer is a DEVICE pointer owned by the caller
+ *     (e.g. a PyTorch allocation) on the device given to bemcub_create.  The library never frees
+ *     or keeps caller buffers; bemcub_set_elements copies what it needs into ctx-owned memory.
+ *   - All work is enqueued on the CUDA stream given to bemcub_create (NULL = legacy default
+ *     stream).  bemcub_eval / bemcub_assemble* are asynchronous: results are valid once the caller
+ *     has synchronised that stream.  bemcub_set_elements, the *_host calls and bemcub_fp64_peak
+ *     synchronise internally.  (A call that has to grow ctx-owned scratch calls cudaMalloc.)
+ *   - Every function returns BEMCUB_OK (0) or a negative error code; nothing throws or longjmps
+ *     across the ABI.  There is no CPU fallback: without a usable CUDA device bemcub_create fails.
+ *   - SI units: lengths m, sigma C/m^2, Phi V, E V/m.  eps0 = 8.8541878128e-12 F/m (CODATA 2018;
+ *     the paper prints no value), applied once after the summation.
+ *   - A ctx is not thread-safe; use one ctx per host thread / stream.
+ *
+ * Element layout
+ *   type[n]        uint8   BEMCUB_TRI or BEMCUB_RECT
+ *   verts[n][3][3] double  triangle: vertices A, B, C (Eq. 3.3);
+ *                          rectangle: corner P0, P1 = P0 + a u_x, P3 = P0 + b u_y (Eq. 3.2); the
+ *                          fourth corner P0 + a u_x + b u_y is implied, Q_cen = P0 + (P1-P0)/2 + (P3-P0)/2
+ *   sigma[n]       double  constant charge density of each element (L36, L62)
+ *   L (L66) = (|AB|+|BC|+|CA|)/3 for a triangle, (a+b)/2 for a rectangle.
+ */
+#ifndef BEMCUB_H
+#define BEMCUB_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bemcub_ctx bemcub_ctx; /* opaque; owns device scratch and the expanded points */
+
+enum { BEMCUB_TRI = 0, BEMCUB_RECT = 1 };
+
+/* rule levels: the triangle and rectangle rule of the same level are paired by degree (L125) */
+enum {
+  BEMCUB_RULE_ADAPTIVE = -1, /* per-pair choice by distance ratio (L159)                  */
+  BEMCUB_RULE_L0 = 0,        /* Table A1 / B1: N = 4,        degree 3                      */
+  BEMCUB_RULE_L1 = 1,        /* Table A2 / B2: N = 7,        degree 5                      */
+  BEMCUB_RULE_L2 = 2,        /* Table A3 / B3: N = 12,       degree 7                      */
+  BEMCUB_RULE_L3 = 3,        /* Table A4 / B4: N = 19 | 17,  degree 9                      */
+  BEMCUB_RULE_L4 = 4,        /* Table A5 / B5: N = 33,       degree 12 | 13                */
+  BEMCUB_LEVEL_ANALYTIC = 5  /* bit index of the analytic branch in use_levels_mask        */
+};
+
+enum { BEMCUB_F64 = 0, BEMCUB_F32 = 1 };
+
+enum {
+  BEMCUB_OK = 0,
+  BEMCUB_ERR_INVALID_ARG = -1,
+  BEMCUB_ERR_DEGENERATE_ELEMENT = -2, /* an element with zero area / zero side            */
+  BEMCUB_ERR_NOT_RECTANGLE = -3,      /* |e1.e2| > 1e-12 |e1||e2| for a BEMCUB_RECT        */
+  BEMCUB_ERR_BAD_RULE = -4,
+  BEMCUB_ERR_CUDA = -5,
+  BEMCUB_ERR_NOMEM = -6,
+  BEMCUB_ERR_NO_ELEMENTS = -7         /* eval/assemble before a successful set_elements    */
+};
+
+/* Distance-ratio policy (Sec. 4).  dr[t][b], t = element type, are the UPPER distance-ratio
+ * limits of the bands {analytic, N=33, N=19|17, N=12, N=7}; N=4 is used above dr[t][4].  A band
+ * contains its lower limit (DR == limit belongs to the band above it): the decision is
+ * "D^2 < (dr*L)^2" in double precision.  use_levels_mask: bit k (k = 0..4) enables rule level k,
+ * bit 5 the analytic branch; a disabled choice moves to the next MORE accurate enabled one, or, if
+ * there is none, to the most accurate enabled one (the paper's GPU integrator used N = 7/12/33 +
+ * analytic only, L239).  allow_upgrade = 1 lets the library evaluate an (element, field-point
+ * tile) with the most accurate rule any pair of the tile asks for, instead of choosing per pair;
+ * results then differ from the per-pair policy only by the (smaller) truncation error of the
+ * better rule.  allow_upgrade = 0 reproduces the per-pair choice exactly. */
+typedef struct {
+  double dr[2][5];
+  int32_t allow_upgrade;
+  int32_t use_levels_mask;
+} bemcub_policy;
+
+/* Counters of the work enqueued by this ctx since creation / the last reset (host side). */
+typedef struct {
+  int64_t kernel_launches;     /* CUDA kernels of this library launched                    */
+  int64_t point_interactions;  /* point-charge interactions of the last eval (fixed rule:   */
+                               /* m * sum N; adaptive: counted on the device, valid after   */
+                               /* the stream is synchronised and bemcub_get_stats is called)*/
+  int64_t analytic_pairs;      /* (element, point) pairs sent to the analytic branch, ditto */
+  int64_t last_eval_launches;  /* kernels launched by the most recent eval/assemble call    */
+} bemcub_stats;
+
+/* device: CUDA device ordinal.  cuda_stream: a cudaStream_t cast to void* (NULL = default).    */
+int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream);
+int bemcub_destroy(bemcub_ctx* ctx);
+
+/* HOST struct.  want_field = 0: the printed triangle-potential limits 3/8/20/80/1500 (L159) for
+ * both element types; want_field = 1: limits for Phi and E together ("slightly higher", L159):
+ * triangles 4/10/25/100/2000, rectangles 6/15/40/150/3000 (reading 7).
+ * allow_upgrade = 1, use_levels_mask = 63. */
+int bemcub_default_policy(bemcub_policy* host_policy, int want_field);
+
+/* Copies the mesh into the ctx and computes centroid, area and L of every element (Eq. 3.2/3.3,
+ * L66).  Synchronises.  Errors: DEGENERATE_ELEMENT, NOT_RECTANGLE (the ctx then holds no mesh),
+ * INVALID_ARG (n < 0, null pointers with n > 0, a type other than 0/1). */
+int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const double* verts);
+
+/* Eq. 4.1 summed over all elements at m field points.
+ *   sigma[n]; rule_id = BEMCUB_RULE_L0..L4 (fixed rule for every pair; no near-field switching: a
+ *   field point that coincides with a Gaussian point gives IEEE inf/nan) or BEMCUB_RULE_ADAPTIVE
+ *   (policy must be non-NULL; HOST pointer); field_pts[m][3]; out_phi[m]; out_E[m][3] or NULL.
+ *   precision = BEMCUB_F64, or BEMCUB_F32: points, field points and the interaction arithmetic
+ *   are FP32, sums of at most 128 terms are FP32 and those block sums are accumulated in FP64
+ *   (the analytic branch stays FP64); buffers keep their double type.
+ * m = 0 is a no-op.  Asynchronous. */
+int bemcub_eval(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
+                int64_t m, const double* field_pts, double* out_phi, double* out_E, int precision);
+
+/* Dense collocation matrix (L34): out_matrix[i*ld + j] = k * Int_{element j} dS / |c_i - Q| (unit
+ * sigma), c_i = centroid of element i, rule per pair by the policy (DR(i,j) uses L of element j;
+ * the self term has D = 0 and is analytic).  Units V m^2 / C.  ld >= n.  The policy's
+ * allow_upgrade is honoured per 32-row tile.  Asynchronous.
+ * bemcub_assemble_rows fills rows [row0, row0+nrows) only, into out_rows[(i-row0)*ld + j]
+ * (row sharding across GPUs; sampling). */
+int bemcub_assemble(bemcub_ctx* ctx, const bemcub_policy* host_policy, double* out_matrix, int64_t ld);
+int bemcub_assemble_rows(bemcub_ctx* ctx, const bemcub_policy* host_policy, int64_t row0, int64_t nrows,
+                         double* out_rows, int64_t ld);
+
+/* Same as bemcub_set_elements / bemcub_eval with HOST buffers: copies the inputs to ctx-owned
+ * device memory, runs, copies phi / E back and synchronises (the end-to-end path bench.py times). */
+int bemcub_set_elements_host(bemcub_ctx* ctx, int64_t n, const uint8_t* host_type, const double* host_verts);
+int bemcub_eval_host(bemcub_ctx* ctx, const double* host_sigma, int rule_id, const bemcub_policy* host_policy,
+                     int64_t m, const double* host_field_pts, double* host_phi, double* host_E, int precision);
+
+/* The tabulated rules (HOST outputs).  coords: triangle [N][3] barycentric (lambda_A, lambda_B,
+ * lambda_C), rectangle [N][2] natural (x, y) in [-1,1]^2; w[N], sum w = 1 (Eq. 3.1). */
+int bemcub_rule_info(int elem_type, int rule_id, int* npts, int* degree);
+int bemcub_rule_points(int elem_type, int rule_id, double* host_coords, double* host_w);
+
+/* Expanded point charges of the current mesh for one level, as the evaluation kernel reads them:
+ * out_xyzq[n*stride][4] = (Q_i, q_i); stride = max N over the element types present; an element
+ * with fewer points is padded with zero charges at its centroid.  sigma may be NULL (unit sigma).
+ * Returns the stride in *out_stride.  Asynchronous. */
+int bemcub_expand_points(bemcub_ctx* ctx, const double* sigma, int rule_id, double* out_xyzq, int* out_stride);
+
+/* Centroid [n][3], area [n], L [n] of the current mesh (any pointer may be NULL).  Asynchronous. */
+int bemcub_get_geometry(bemcub_ctx* ctx, double* out_cen, double* out_area, double* out_L);
+
+/* Roofline denominator: runs a dependent-chain-free DFMA kernel on all SMs for about `seconds`
+ * and returns the sustained rate in FP64 FMA/s (flop/s = 2x).  Synchronises. */
+int bemcub_fp64_peak(bemcub_ctx* ctx, double seconds, double* host_dfma_per_s);
+
+int bemcub_get_stats(bemcub_ctx* ctx, bemcub_stats* host_stats);  /* synchronises the stream */
+int bemcub_reset_stats(bemcub_ctx* ctx);
+
+const char* bemcub_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BEMCUB_H */

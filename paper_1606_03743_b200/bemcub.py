@@ -1,0 +1,252 @@
+"""Thin ctypes binding of the bemcub C ABI (include/bemcub.h): argument marshalling only.
+
+Every function below has the name and the argument order of its C counterpart; device buffers
+are passed as torch CUDA tensors (or raw integer addresses) and only their `data_ptr()` crosses
+the boundary.  All arithmetic of the hot path runs in the CUDA kernels of libbemcub.so.  There is
+no CPU fallback: if the library cannot be loaded the import of this module fails loudly.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from . import build as _build
+
+TRI, RECT = 0, 1
+RULE_ADAPTIVE = -1
+LEVEL_ANALYTIC = 5
+F64, F32 = 0, 1
+ALL_LEVELS = 63
+
+OK = 0
+ERR_INVALID_ARG, ERR_DEGENERATE_ELEMENT, ERR_NOT_RECTANGLE = -1, -2, -3
+ERR_BAD_RULE, ERR_CUDA, ERR_NOMEM, ERR_NO_ELEMENTS = -4, -5, -6, -7
+
+
+class bemcub_policy(C.Structure):
+    _fields_ = [("dr", (C.c_double * 5) * 2), ("allow_upgrade", C.c_int32), ("use_levels_mask", C.c_int32)]
+
+
+class bemcub_stats(C.Structure):
+    _fields_ = [("kernel_launches", C.c_int64), ("point_interactions", C.c_int64),
+                ("analytic_pairs", C.c_int64), ("last_eval_launches", C.c_int64)]
+
+
+class BemcubError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} (code {code})")
+
+
+def _load() -> C.CDLL:
+    path = _build.LIB
+    if _build.is_stale():
+        try:
+            _build.build()
+        except Exception as exc:  # no nvcc on this box and no prebuilt library
+            if not Path(path).exists():
+                raise ImportError(f"libbemcub.so is missing and could not be built: {exc}") from exc
+    lib = C.CDLL(str(path))
+    vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
+    PP = C.POINTER(bemcub_policy)
+    sig = {
+        "bemcub_create": [C.POINTER(vp), C.c_int, vp],
+        "bemcub_destroy": [vp],
+        "bemcub_default_policy": [PP, C.c_int],
+        "bemcub_set_elements": [vp, i64, vp, vp],
+        "bemcub_eval": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
+        "bemcub_assemble": [vp, PP, vp, i64],
+        "bemcub_assemble_rows": [vp, PP, i64, i64, vp, i64],
+        "bemcub_set_elements_host": [vp, i64, vp, vp],
+        "bemcub_eval_host": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
+        "bemcub_rule_info": [C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)],
+        "bemcub_rule_points": [C.c_int, C.c_int, vp, vp],
+        "bemcub_expand_points": [vp, vp, C.c_int, vp, C.POINTER(C.c_int)],
+        "bemcub_get_geometry": [vp, vp, vp, vp],
+        "bemcub_fp64_peak": [vp, dbl, C.POINTER(dbl)],
+        "bemcub_get_stats": [vp, C.POINTER(bemcub_stats)],
+        "bemcub_reset_stats": [vp],
+    }
+    for name, args in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes = args
+        fn.restype = C.c_int
+    lib.bemcub_strerror.argtypes = [C.c_int]
+    lib.bemcub_strerror.restype = C.c_char_p
+    return lib
+
+
+_lib = _load()
+EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval",
+            "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
+            "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
+            "bemcub_fp64_peak", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_strerror"]
+
+
+def library_path() -> str:
+    return str(_build.LIB)
+
+
+def strerror(code: int) -> str:
+    return _lib.bemcub_strerror(code).decode()
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != OK:
+        raise BemcubError(rc, where)
+
+
+def _dptr(t):
+    """Device address of a torch CUDA tensor (must be contiguous), an int address, or None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return C.c_void_p(t)
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("device buffers must be contiguous CUDA tensors")
+    return C.c_void_p(t.data_ptr())
+
+
+def _hptr(a):
+    """Host address of a contiguous numpy array / CPU torch tensor, or None."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        if not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("host buffers must be C-contiguous")
+        return C.c_void_p(a.ctypes.data)
+    if a.is_cuda or not a.is_contiguous():
+        raise ValueError("host buffers must be contiguous CPU tensors")
+    return C.c_void_p(a.data_ptr())
+
+
+def _policy_ptr(policy):
+    return None if policy is None else C.byref(policy)
+
+
+# ---- one Python function per C entry point ---------------------------------------------------
+
+def bemcub_create(device: int = 0, cuda_stream: int = 0) -> C.c_void_p:
+    ctx = C.c_void_p()
+    _check(_lib.bemcub_create(C.byref(ctx), device, C.c_void_p(cuda_stream)), "bemcub_create")
+    return ctx
+
+
+def bemcub_destroy(ctx) -> None:
+    _check(_lib.bemcub_destroy(ctx), "bemcub_destroy")
+
+
+def bemcub_default_policy(want_field: bool) -> bemcub_policy:
+    p = bemcub_policy()
+    _check(_lib.bemcub_default_policy(C.byref(p), int(want_field)), "bemcub_default_policy")
+    return p
+
+
+def make_policy(dr, allow_upgrade: bool = True, use_levels_mask: int = ALL_LEVELS) -> bemcub_policy:
+    """bemcub_policy from dr[2][5] (marshalling helper, no arithmetic)."""
+    p = bemcub_policy()
+    for t in range(2):
+        for b in range(5):
+            p.dr[t][b] = float(dr[t][b])
+    p.allow_upgrade = int(allow_upgrade)
+    p.use_levels_mask = int(use_levels_mask)
+    return p
+
+
+def bemcub_set_elements(ctx, n: int, etype, verts) -> None:
+    _check(_lib.bemcub_set_elements(ctx, n, _dptr(etype), _dptr(verts)), "bemcub_set_elements")
+
+
+def bemcub_eval(ctx, sigma, rule_id: int, policy, m: int, field_pts, out_phi, out_E, precision: int = F64) -> None:
+    _check(_lib.bemcub_eval(ctx, _dptr(sigma), rule_id, _policy_ptr(policy), m, _dptr(field_pts), _dptr(out_phi),
+                            _dptr(out_E), precision), "bemcub_eval")
+
+
+def bemcub_assemble(ctx, policy, out_matrix, ld: int) -> None:
+    _check(_lib.bemcub_assemble(ctx, _policy_ptr(policy), _dptr(out_matrix), ld), "bemcub_assemble")
+
+
+def bemcub_assemble_rows(ctx, policy, row0: int, nrows: int, out_rows, ld: int) -> None:
+    _check(_lib.bemcub_assemble_rows(ctx, _policy_ptr(policy), row0, nrows, _dptr(out_rows), ld),
+           "bemcub_assemble_rows")
+
+
+def bemcub_set_elements_host(ctx, n: int, host_type, host_verts) -> None:
+    _check(_lib.bemcub_set_elements_host(ctx, n, _hptr(host_type), _hptr(host_verts)), "bemcub_set_elements_host")
+
+
+def bemcub_eval_host(ctx, host_sigma, rule_id: int, policy, m: int, host_field_pts, host_phi, host_E,
+                     precision: int = F64) -> None:
+    _check(_lib.bemcub_eval_host(ctx, _hptr(host_sigma), rule_id, _policy_ptr(policy), m, _hptr(host_field_pts),
+                                 _hptr(host_phi), _hptr(host_E), precision), "bemcub_eval_host")
+
+
+def bemcub_rule_info(elem_type: int, rule_id: int):
+    n, d = C.c_int(), C.c_int()
+    _check(_lib.bemcub_rule_info(elem_type, rule_id, C.byref(n), C.byref(d)), "bemcub_rule_info")
+    return n.value, d.value
+
+
+def bemcub_rule_points(elem_type: int, rule_id: int):
+    n, _ = bemcub_rule_info(elem_type, rule_id)
+    coords = np.zeros((n, 3 if elem_type == TRI else 2))
+    w = np.zeros(n)
+    _check(_lib.bemcub_rule_points(elem_type, rule_id, _hptr(coords), _hptr(w)), "bemcub_rule_points")
+    return coords, w
+
+
+def bemcub_expand_points(ctx, sigma, rule_id: int, out_xyzq) -> int:
+    stride = C.c_int()
+    _check(_lib.bemcub_expand_points(ctx, _dptr(sigma), rule_id, _dptr(out_xyzq), C.byref(stride)),
+           "bemcub_expand_points")
+    return stride.value
+
+
+def bemcub_get_geometry(ctx, out_cen, out_area, out_L) -> None:
+    _check(_lib.bemcub_get_geometry(ctx, _dptr(out_cen), _dptr(out_area), _dptr(out_L)), "bemcub_get_geometry")
+
+
+def bemcub_fp64_peak(ctx, seconds: float) -> float:
+    v = C.c_double()
+    _check(_lib.bemcub_fp64_peak(ctx, seconds, C.byref(v)), "bemcub_fp64_peak")
+    return v.value
+
+
+def bemcub_get_stats(ctx) -> dict:
+    s = bemcub_stats()
+    _check(_lib.bemcub_get_stats(ctx, C.byref(s)), "bemcub_get_stats")
+    return {k: getattr(s, k) for k, _ in bemcub_stats._fields_}
+
+
+def bemcub_reset_stats(ctx) -> None:
+    _check(_lib.bemcub_reset_stats(ctx), "bemcub_reset_stats")
+
+
+class Context:
+    """RAII wrapper: owns one bemcub_ctx bound to a device and to torch's current stream."""
+
+    def __init__(self, device: int = 0, stream: int | None = None):
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream(device).cuda_stream
+        self.device = device
+        self.handle = bemcub_create(device, stream)
+
+    def close(self):
+        if self.handle is not None:
+            bemcub_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,656 @@
+// Host side of the bemcub C ABI (include/bemcub.h): context, scratch management, launch
+// configuration.  All arithmetic of the hot path lives in the kernels included below; this file
+// only validates arguments, sizes grids and enqueues kernels on the ctx stream.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include <cuda_runtime.h>
+
+#include "../../include/bemcub.h"
+#include "kernels_assemble.cuh"
+#include "kernels_eval.cuh"
+#include "kernels_pre.cuh"
+#include "rules.h"
+
+using namespace bemcub;
+
+namespace {
+
+// CODATA-2018 vacuum permittivity; the paper prints no value (reading 10).
+const double kEps0 = 8.8541878128e-12;
+const double kPi = 3.14159265358979323846;
+inline double coulomb_k() { return 1.0 / (4.0 * kPi * kEps0); }
+
+struct DevBuf {
+  void* ptr = nullptr;
+  size_t bytes = 0;
+};
+
+}  // namespace
+
+struct bemcub_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int num_sms = 148;
+  // mesh
+  int64_t n = 0;
+  bool has_mesh = false;
+  bool has_tri = false, has_rect = false;
+  int64_t n_tri = 0, n_rect = 0;
+  DevBuf type, verts, cenL, area;
+  GeomStatus* d_status = nullptr;
+  // expanded points per level (FP64 / FP32) and the stride they were built with
+  DevBuf pts64[5], pts32[5];
+  int stride[5] = {4, 7, 12, 19, 33};
+  // scratch
+  DevBuf partial;
+  DevBuf host_stage[5];  // device copies of host inputs/outputs for the *_host entry points
+  unsigned long long* d_counters = nullptr;
+  bemcub_stats stats{};
+  bool counters_pending = false;
+};
+
+namespace {
+
+#define CUDA_TRY(expr)                         \
+  do {                                         \
+    cudaError_t _e = (expr);                   \
+    if (_e != cudaSuccess) {                   \
+      cudaGetLastError();                      \
+      return _e == cudaErrorMemoryAllocation ? BEMCUB_ERR_NOMEM : BEMCUB_ERR_CUDA; \
+    }                                          \
+  } while (0)
+
+int ensure(DevBuf& b, size_t bytes) {
+  if (bytes <= b.bytes) return BEMCUB_OK;
+  if (b.ptr) {
+    cudaFree(b.ptr);
+    b.ptr = nullptr;
+    b.bytes = 0;
+  }
+  // grow with some headroom so that repeated slightly larger calls do not reallocate each time
+  size_t want = bytes + bytes / 8 + 256;
+  cudaError_t e = cudaMalloc(&b.ptr, want);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    want = bytes;
+    e = cudaMalloc(&b.ptr, want);
+  }
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    b.ptr = nullptr;
+    return BEMCUB_ERR_NOMEM;
+  }
+  b.bytes = want;
+  return BEMCUB_OK;
+}
+
+void release(DevBuf& b) {
+  if (b.ptr) cudaFree(b.ptr);
+  b.ptr = nullptr;
+  b.bytes = 0;
+}
+
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != dev) ok = (cudaSetDevice(dev) == cudaSuccess);
+  }
+  ~DeviceGuard() {
+    int cur = -1;
+    if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+  }
+};
+
+inline int rule_n(int type, int level) { return type == 0 ? bemcub_rules::kTriN[level] : bemcub_rules::kRectN[level]; }
+
+void count_launch(bemcub_ctx* c, int k = 1) {
+  c->stats.kernel_launches += k;
+  c->stats.last_eval_launches += k;
+}
+
+int upload_tables() {
+  double tri[75 * 4], rect[73 * 4];
+  int toff[6], roff[6];
+  int nt = 0, nr = 0;
+  for (int l = 0; l < 5; ++l) {
+    bemcub_rules::TriPoint tp[bemcub_rules::kMaxN];
+    bemcub_rules::RectPoint rp[bemcub_rules::kMaxN];
+    toff[l] = nt;
+    roff[l] = nr;
+    const int a = bemcub_rules::tri_points(l, tp), b = bemcub_rules::rect_points(l, rp);
+    if (a != bemcub_rules::kTriN[l] || b != bemcub_rules::kRectN[l]) return BEMCUB_ERR_BAD_RULE;
+    for (int i = 0; i < a; ++i, ++nt) {
+      tri[4 * nt] = tp[i].la; tri[4 * nt + 1] = tp[i].lb; tri[4 * nt + 2] = tp[i].lc; tri[4 * nt + 3] = tp[i].w;
+    }
+    for (int i = 0; i < b; ++i, ++nr) {
+      rect[4 * nr] = rp[i].x; rect[4 * nr + 1] = rp[i].y; rect[4 * nr + 2] = rp[i].w; rect[4 * nr + 3] = 0.0;
+    }
+  }
+  toff[5] = nt;
+  roff[5] = nr;
+  CUDA_TRY(cudaMemcpyToSymbol(c_tri_tab, tri, sizeof(tri)));
+  CUDA_TRY(cudaMemcpyToSymbol(c_rect_tab, rect, sizeof(rect)));
+  CUDA_TRY(cudaMemcpyToSymbol(c_tri_off, toff, sizeof(toff)));
+  CUDA_TRY(cudaMemcpyToSymbol(c_rect_off, roff, sizeof(roff)));
+  return BEMCUB_OK;
+}
+
+// use_levels_mask -> level actually used for each wanted level (bemcub.h: next more accurate
+// enabled one, else the most accurate enabled one below).
+int build_policy(const bemcub_policy* hp, PolicyDev* out) {
+  if (!hp) return BEMCUB_ERR_INVALID_ARG;
+  const int mask = hp->use_levels_mask & 63;
+  if (mask == 0) return BEMCUB_ERR_INVALID_ARG;
+  for (int t = 0; t < 2; ++t)
+    for (int b = 0; b < 5; ++b) {
+      const double v = hp->dr[t][b];
+      if (!(v >= 0.0) || !std::isfinite(v)) return BEMCUB_ERR_INVALID_ARG;
+      if (b > 0 && v < hp->dr[t][b - 1]) return BEMCUB_ERR_INVALID_ARG;  // limits must not decrease
+      out->dr[t][b] = v;
+    }
+  for (int want = 0; want <= 5; ++want) {
+    int use = -1;
+    for (int lv = want; lv <= 5 && use < 0; ++lv)
+      if (mask & (1 << lv)) use = lv;
+    for (int lv = want - 1; lv >= 0 && use < 0; --lv)
+      if (mask & (1 << lv)) use = lv;
+    out->map[want] = use;
+  }
+  out->allow_upgrade = hp->allow_upgrade ? 1 : 0;
+  return BEMCUB_OK;
+}
+
+// Expanded points of one level, FP64 or FP32, into ctx-owned memory.
+template <typename T>
+int expand_level(bemcub_ctx* c, int level, const double* sigma, DevBuf& dst) {
+  typedef typename Point4<T>::type P4;
+  const int64_t total = c->n * c->stride[level];
+  int rc = ensure(dst, (size_t)std::max<int64_t>(total, 1) * sizeof(P4));
+  if (rc) return rc;
+  if (total == 0) return BEMCUB_OK;
+  const int threads = 256;
+  const int64_t blocks = (total + threads - 1) / threads;
+  expand_kernel<T><<<(unsigned)blocks, threads, 0, c->stream>>>(
+      c->n, level, c->stride[level], (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr,
+      (const double4*)c->cenL.ptr, (const double*)c->area.ptr, sigma, (P4*)dst.ptr);
+  count_launch(c);
+  CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
+
+struct SplitPlan {
+  int R;
+  int64_t ntiles, ctas_x;
+  int nsplit;
+  int64_t elems_per_split;
+};
+
+// Work decomposition: warp item = (tile of 32R field points) x (split of the elements).  Enough
+// CTAs for ~50 waves on all SMs at 2 CTAs/SM so the tail is small; splits are multiples of 32
+// elements (the adaptive kernel's batch) and at least 256 elements long.
+SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, bool allow_r2) {
+  SplitPlan s;
+  const int64_t slots = (int64_t)c->num_sms * 2;
+  s.R = (allow_r2 && m >= slots * kWarpsPerCta * 64) ? 2 : 1;
+  s.ntiles = (m + 32 * s.R - 1) / (32 * s.R);
+  s.ctas_x = (s.ntiles + kWarpsPerCta - 1) / kWarpsPerCta;
+  const int64_t target = slots * 50;
+  int64_t ns = (target + s.ctas_x - 1) / s.ctas_x;
+  const int64_t max_by_len = std::max<int64_t>(1, c->n / 256);
+  const int64_t max_by_mem = std::max<int64_t>(1, (int64_t)(1ull << 31) / std::max<int64_t>(32 * m, 1));
+  ns = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(ns, max_by_len), std::min<int64_t>(max_by_mem, 4096)));
+  int64_t eps = (c->n + ns - 1) / ns;
+  eps = (eps + 31) / 32 * 32;
+  if (eps < 32) eps = 32;
+  s.elems_per_split = eps;
+  s.nsplit = (int)std::max<int64_t>(1, (c->n + eps - 1) / eps);
+  return s;
+}
+
+template <typename T, int R>
+int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
+  const size_t smem = eval_smem_bytes<T>();
+  CUDA_TRY(cudaFuncSetAttribute(eval_fixed_kernel<T, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  dim3 grid((unsigned)sp.ctas_x, (unsigned)sp.nsplit);
+  eval_fixed_kernel<T, R><<<grid, kThreads, smem, c->stream>>>(fp);
+  count_launch(c);
+  CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
+
+template <int R>
+int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp) {
+  const size_t smem = eval_smem_bytes<double>();
+  CUDA_TRY(cudaFuncSetAttribute(eval_adaptive_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  dim3 grid((unsigned)sp.ctas_x, (unsigned)sp.nsplit);
+  eval_adaptive_kernel<R><<<grid, kThreads, smem, c->stream>>>(ap);
+  count_launch(c);
+  CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
+
+void refresh_counters(bemcub_ctx* c) {
+  if (!c->counters_pending) return;
+  unsigned long long h[2] = {0, 0};
+  cudaStreamSynchronize(c->stream);
+  if (cudaMemcpy(h, c->d_counters, sizeof(h), cudaMemcpyDeviceToHost) == cudaSuccess) {
+    c->stats.point_interactions = (int64_t)h[0];
+    c->stats.analytic_pairs = (int64_t)h[1];
+  }
+  c->counters_pending = false;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bemcub_strerror(int code) {
+  switch (code) {
+    case BEMCUB_OK: return "ok";
+    case BEMCUB_ERR_INVALID_ARG: return "invalid argument";
+    case BEMCUB_ERR_DEGENERATE_ELEMENT: return "degenerate element (zero area or zero side)";
+    case BEMCUB_ERR_NOT_RECTANGLE: return "rectangle sides are not orthogonal";
+    case BEMCUB_ERR_BAD_RULE: return "unknown rule id / element type";
+    case BEMCUB_ERR_CUDA: return "CUDA error";
+    case BEMCUB_ERR_NOMEM: return "out of device memory";
+    case BEMCUB_ERR_NO_ELEMENTS: return "no mesh: call bemcub_set_elements first";
+  }
+  return "unknown error code";
+}
+
+int bemcub_rule_info(int elem_type, int rule_id, int* npts, int* degree) {
+  if ((elem_type != BEMCUB_TRI && elem_type != BEMCUB_RECT) || rule_id < 0 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
+  if (npts) *npts = rule_n(elem_type, rule_id);
+  if (degree) *degree = elem_type == 0 ? bemcub_rules::kTriDegree[rule_id] : bemcub_rules::kRectDegree[rule_id];
+  return BEMCUB_OK;
+}
+
+int bemcub_rule_points(int elem_type, int rule_id, double* host_coords, double* host_w) {
+  if ((elem_type != BEMCUB_TRI && elem_type != BEMCUB_RECT) || rule_id < 0 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
+  if (!host_coords || !host_w) return BEMCUB_ERR_INVALID_ARG;
+  if (elem_type == BEMCUB_TRI) {
+    bemcub_rules::TriPoint tp[bemcub_rules::kMaxN];
+    const int n = bemcub_rules::tri_points(rule_id, tp);
+    for (int i = 0; i < n; ++i) {
+      host_coords[3 * i] = tp[i].la; host_coords[3 * i + 1] = tp[i].lb; host_coords[3 * i + 2] = tp[i].lc;
+      host_w[i] = tp[i].w;
+    }
+  } else {
+    bemcub_rules::RectPoint rp[bemcub_rules::kMaxN];
+    const int n = bemcub_rules::rect_points(rule_id, rp);
+    for (int i = 0; i < n; ++i) {
+      host_coords[2 * i] = rp[i].x; host_coords[2 * i + 1] = rp[i].y;
+      host_w[i] = rp[i].w;
+    }
+  }
+  return BEMCUB_OK;
+}
+
+int bemcub_default_policy(bemcub_policy* hp, int want_field) {
+  if (!hp) return BEMCUB_ERR_INVALID_ARG;
+  // L159: printed triangle-potential limits; Phi+E limits per DESIGN.md reading 7
+  static const double pot[5] = {3, 8, 20, 80, 1500};
+  static const double ftri[5] = {4, 10, 25, 100, 2000};
+  static const double frect[5] = {6, 15, 40, 150, 3000};
+  for (int b = 0; b < 5; ++b) {
+    hp->dr[0][b] = want_field ? ftri[b] : pot[b];
+    hp->dr[1][b] = want_field ? frect[b] : pot[b];
+  }
+  hp->allow_upgrade = 1;
+  hp->use_levels_mask = 63;
+  return BEMCUB_OK;
+}
+
+int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream) {
+  if (!out_ctx) return BEMCUB_ERR_INVALID_ARG;
+  *out_ctx = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+    cudaGetLastError();
+    return BEMCUB_ERR_CUDA;  // no CPU fallback: the library is useless without a GPU
+  }
+  DeviceGuard g(device);
+  if (!g.ok) return BEMCUB_ERR_CUDA;
+  bemcub_ctx* c = new (std::nothrow) bemcub_ctx();
+  if (!c) return BEMCUB_ERR_NOMEM;
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+    delete c;
+    return BEMCUB_ERR_CUDA;
+  }
+  c->num_sms = prop.multiProcessorCount;
+  int rc = upload_tables();
+  if (rc == BEMCUB_OK && cudaMalloc(&c->d_status, sizeof(GeomStatus)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
+  if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, 2 * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
+  if (rc != BEMCUB_OK) {
+    bemcub_destroy(c);
+    return rc;
+  }
+  *out_ctx = c;
+  return BEMCUB_OK;
+}
+
+int bemcub_destroy(bemcub_ctx* c) {
+  if (!c) return BEMCUB_OK;
+  DeviceGuard g(c->device);
+  cudaStreamSynchronize(c->stream);
+  release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial);
+  for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); }
+  if (c->d_status) cudaFree(c->d_status);
+  if (c->d_counters) cudaFree(c->d_counters);
+  delete c;
+  return BEMCUB_OK;
+}
+
+int bemcub_set_elements(bemcub_ctx* c, int64_t n, const uint8_t* type, const double* verts) {
+  if (!c || n < 0 || (n > 0 && (!type || !verts))) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  c->has_mesh = false;
+  c->n = 0;
+  int rc;
+  const size_t nn = (size_t)std::max<int64_t>(n, 1);
+  if ((rc = ensure(c->type, nn)) || (rc = ensure(c->verts, nn * 72)) || (rc = ensure(c->cenL, nn * sizeof(double4))) ||
+      (rc = ensure(c->area, nn * 8)))
+    return rc;
+  GeomStatus st = {0, 0, 0, 0};
+  if (n > 0) {
+    CUDA_TRY(cudaMemcpyAsync(c->type.ptr, type, (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->verts.ptr, verts, (size_t)n * 72, cudaMemcpyDeviceToDevice, c->stream));
+    CUDA_TRY(cudaMemsetAsync(c->d_status, 0, sizeof(GeomStatus), c->stream));
+    const int threads = 256;
+    geometry_kernel<<<(unsigned)((n + threads - 1) / threads), threads, 0, c->stream>>>(
+        n, (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr, (double4*)c->cenL.ptr, (double*)c->area.ptr,
+        c->d_status);
+    c->stats.kernel_launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(&st, c->d_status, sizeof(st), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (st.code != 0) return st.code;  // -1 invalid type, -2 degenerate, -3 not a rectangle
+  }
+  c->n = n;
+  c->n_tri = (int64_t)st.n_tri;
+  c->n_rect = (int64_t)st.n_rect;
+  c->has_tri = st.n_tri != 0;
+  c->has_rect = st.n_rect != 0;
+  for (int l = 0; l < 5; ++l)
+    c->stride[l] = std::max(c->has_tri ? bemcub_rules::kTriN[l] : 0, c->has_rect ? bemcub_rules::kRectN[l] : 0);
+  if (n == 0)
+    for (int l = 0; l < 5; ++l) c->stride[l] = bemcub_rules::kTriN[l];
+  c->has_mesh = true;
+  return BEMCUB_OK;
+}
+
+int bemcub_get_geometry(bemcub_ctx* c, double* out_cen, double* out_area, double* out_L) {
+  if (!c) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  DeviceGuard g(c->device);
+  if (c->n == 0) return BEMCUB_OK;
+  if (out_cen)
+    CUDA_TRY(cudaMemcpy2DAsync(out_cen, 24, c->cenL.ptr, 32, 24, (size_t)c->n, cudaMemcpyDeviceToDevice, c->stream));
+  if (out_L)
+    CUDA_TRY(cudaMemcpy2DAsync(out_L, 8, (const char*)c->cenL.ptr + 24, 32, 8, (size_t)c->n, cudaMemcpyDeviceToDevice,
+                               c->stream));
+  if (out_area) CUDA_TRY(cudaMemcpyAsync(out_area, c->area.ptr, (size_t)c->n * 8, cudaMemcpyDeviceToDevice, c->stream));
+  return BEMCUB_OK;
+}
+
+int bemcub_expand_points(bemcub_ctx* c, const double* sigma, int rule_id, double* out_xyzq, int* out_stride) {
+  if (!c || !out_xyzq) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  if (rule_id < 0 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
+  DeviceGuard g(c->device);
+  if (out_stride) *out_stride = c->stride[rule_id];
+  int rc = expand_level<double>(c, rule_id, sigma, c->pts64[rule_id]);
+  if (rc) return rc;
+  if (c->n > 0)
+    CUDA_TRY(cudaMemcpyAsync(out_xyzq, c->pts64[rule_id].ptr, (size_t)c->n * c->stride[rule_id] * 32,
+                             cudaMemcpyDeviceToDevice, c->stream));
+  return BEMCUB_OK;
+}
+
+int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
+                const double* field_pts, double* out_phi, double* out_E, int precision) {
+  if (!c || m < 0) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  if (rule_id < -1 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
+  if (precision != BEMCUB_F64 && precision != BEMCUB_F32) return BEMCUB_ERR_INVALID_ARG;
+  if (m == 0) return BEMCUB_OK;
+  if (!field_pts || (!out_phi && !out_E) || (c->n > 0 && !sigma)) return BEMCUB_ERR_INVALID_ARG;
+  const bool adaptive = rule_id == BEMCUB_RULE_ADAPTIVE;
+  PolicyDev pol;
+  if (adaptive) {
+    if (precision != BEMCUB_F64) return BEMCUB_ERR_INVALID_ARG;  // the adaptive path is FP64 only
+    int rc = build_policy(host_policy, &pol);
+    if (rc) return rc;
+  }
+  DeviceGuard g(c->device);
+  c->stats.last_eval_launches = 0;
+  int rc;
+
+  if (c->n == 0) {  // empty mesh: zero potential and field
+    if (out_phi) CUDA_TRY(cudaMemsetAsync(out_phi, 0, (size_t)m * 8, c->stream));
+    if (out_E) CUDA_TRY(cudaMemsetAsync(out_E, 0, (size_t)m * 24, c->stream));
+    c->stats.point_interactions = 0;
+    c->stats.analytic_pairs = 0;
+    return BEMCUB_OK;
+  }
+
+  // a1: expand the levels this call needs, sigma folded in
+  if (adaptive) {
+    for (int l = 0; l < 5; ++l) {
+      bool used = false;
+      for (int w = 0; w <= 5; ++w) used |= (pol.map[w] == l);
+      if (used && (rc = expand_level<double>(c, l, sigma, c->pts64[l]))) return rc;
+    }
+  } else if (precision == BEMCUB_F64) {
+    if ((rc = expand_level<double>(c, rule_id, sigma, c->pts64[rule_id]))) return rc;
+  } else {
+    if ((rc = expand_level<float>(c, rule_id, sigma, c->pts32[rule_id]))) return rc;
+  }
+
+  const SplitPlan sp = plan_splits(c, m, true);
+  if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
+
+  if (!adaptive) {
+    FixedParams fp;
+    fp.pts = precision == BEMCUB_F64 ? c->pts64[rule_id].ptr : c->pts32[rule_id].ptr;
+    fp.npts = c->n * c->stride[rule_id];
+    fp.pts_per_split = sp.elems_per_split * c->stride[rule_id];
+    fp.field = field_pts;
+    fp.m = m;
+    fp.partial = (double4*)c->partial.ptr;
+    fp.split_stride = m;
+    fp.ntiles = sp.ntiles;
+    if (precision == BEMCUB_F64) rc = sp.R == 2 ? launch_fixed<double, 2>(c, fp, sp) : launch_fixed<double, 1>(c, fp, sp);
+    else rc = sp.R == 2 ? launch_fixed<float, 2>(c, fp, sp) : launch_fixed<float, 1>(c, fp, sp);
+    if (rc) return rc;
+    // point-charge interactions of a fixed rule: every element's own N at every field point
+    c->stats.point_interactions =
+        (c->n_tri * bemcub_rules::kTriN[rule_id] + c->n_rect * bemcub_rules::kRectN[rule_id]) * m;
+    c->stats.analytic_pairs = 0;
+    c->counters_pending = false;
+  } else {
+    AdaptiveParams ap;
+    for (int l = 0; l < 5; ++l) {
+      ap.lvl_pts[l] = (const double4*)c->pts64[l].ptr;
+      ap.stride[l] = c->stride[l];
+    }
+    ap.cenL = (const double4*)c->cenL.ptr;
+    ap.type = (const uint8_t*)c->type.ptr;
+    ap.verts = (const double*)c->verts.ptr;
+    ap.sigma = sigma;
+    ap.n = c->n;
+    ap.elems_per_split = sp.elems_per_split;
+    ap.pol = pol;
+    ap.field = field_pts;
+    ap.m = m;
+    ap.partial = (double4*)c->partial.ptr;
+    ap.split_stride = m;
+    ap.ntiles = sp.ntiles;
+    ap.counters = c->d_counters;
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 2 * sizeof(unsigned long long), c->stream));
+    rc = sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
+    if (rc) return rc;
+    c->counters_pending = true;
+  }
+
+  // a6: cross-split reduction and the 1/(4 pi eps0) prefactor
+  const int threads = 256;
+  reduce_scale_kernel<<<(unsigned)((m + threads - 1) / threads), threads, 0, c->stream>>>(
+      m, sp.nsplit, m, (const double4*)c->partial.ptr, coulomb_k(), out_phi, out_E);
+  count_launch(c);
+  CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
+
+int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_t row0, int64_t nrows, double* out_rows,
+                         int64_t ld) {
+  if (!c) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  if (row0 < 0 || nrows < 0 || row0 + nrows > c->n || ld < c->n) return BEMCUB_ERR_INVALID_ARG;
+  PolicyDev pol;
+  int rc = build_policy(host_policy, &pol);
+  if (rc) return rc;
+  if (nrows == 0 || c->n == 0) return BEMCUB_OK;
+  if (!out_rows) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  c->stats.last_eval_launches = 0;
+  AssembleParams ap;
+  for (int l = 0; l < 5; ++l) {
+    bool used = false;
+    for (int w = 0; w <= 5; ++w) used |= (pol.map[w] == l);
+    if (used && (rc = expand_level<double>(c, l, nullptr, c->pts64[l]))) return rc;  // unit sigma
+    ap.lvl_pts[l] = (const double4*)c->pts64[l].ptr;
+    ap.stride[l] = c->stride[l];
+  }
+  ap.cenL = (const double4*)c->cenL.ptr;
+  ap.type = (const uint8_t*)c->type.ptr;
+  ap.verts = (const double*)c->verts.ptr;
+  ap.n = c->n;
+  ap.pol = pol;
+  ap.row0 = row0;
+  ap.nrows = nrows;
+  ap.out = out_rows;
+  ap.ld = ld;
+  ap.k = coulomb_k();
+  ap.counters = c->d_counters;
+  CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 2 * sizeof(unsigned long long), c->stream));
+  CUDA_TRY(cudaFuncSetAttribute(assemble_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)assemble_smem_bytes()));
+  const int64_t coltiles = (c->n + 31) / 32, rowtiles = (nrows + 31) / 32;
+  // rows on grid.x would exceed no limit either way; y is limited to 65535 tiles = 2.1 M rows per call
+  if (rowtiles > 65535) return BEMCUB_ERR_INVALID_ARG;
+  dim3 grid((unsigned)((coltiles + kWarpsPerCta - 1) / kWarpsPerCta), (unsigned)rowtiles);
+  assemble_kernel<<<grid, kThreads, assemble_smem_bytes(), c->stream>>>(ap);
+  count_launch(c);
+  CUDA_TRY(cudaGetLastError());
+  c->counters_pending = true;
+  return BEMCUB_OK;
+}
+
+int bemcub_assemble(bemcub_ctx* c, const bemcub_policy* host_policy, double* out_matrix, int64_t ld) {
+  if (!c) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  return bemcub_assemble_rows(c, host_policy, 0, c->n, out_matrix, ld);
+}
+
+int bemcub_set_elements_host(bemcub_ctx* c, int64_t n, const uint8_t* host_type, const double* host_verts) {
+  if (!c || n < 0 || (n > 0 && (!host_type || !host_verts))) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  int rc;
+  const size_t nn = (size_t)std::max<int64_t>(n, 1);
+  if ((rc = ensure(c->host_stage[0], nn)) || (rc = ensure(c->host_stage[1], nn * 72))) return rc;
+  if (n > 0) {
+    CUDA_TRY(cudaMemcpyAsync(c->host_stage[0].ptr, host_type, (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->host_stage[1].ptr, host_verts, (size_t)n * 72, cudaMemcpyHostToDevice, c->stream));
+  }
+  return bemcub_set_elements(c, n, (const uint8_t*)c->host_stage[0].ptr, (const double*)c->host_stage[1].ptr);
+}
+
+int bemcub_eval_host(bemcub_ctx* c, const double* host_sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
+                     const double* host_field_pts, double* host_phi, double* host_E, int precision) {
+  if (!c || m < 0) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  if (m == 0) return BEMCUB_OK;
+  if (!host_field_pts || (!host_phi && !host_E) || (c->n > 0 && !host_sigma)) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  int rc;
+  const size_t nn = (size_t)std::max<int64_t>(c->n, 1);
+  if ((rc = ensure(c->host_stage[2], nn * 8)) || (rc = ensure(c->host_stage[3], (size_t)m * 24)) ||
+      (rc = ensure(c->host_stage[4], (size_t)m * 32)))
+    return rc;
+  double* d_sigma = (double*)c->host_stage[2].ptr;
+  double* d_pts = (double*)c->host_stage[3].ptr;
+  double* d_phi = (double*)c->host_stage[4].ptr;
+  double* d_E = d_phi + m;
+  if (c->n > 0) CUDA_TRY(cudaMemcpyAsync(d_sigma, host_sigma, (size_t)c->n * 8, cudaMemcpyHostToDevice, c->stream));
+  CUDA_TRY(cudaMemcpyAsync(d_pts, host_field_pts, (size_t)m * 24, cudaMemcpyHostToDevice, c->stream));
+  rc = bemcub_eval(c, d_sigma, rule_id, host_policy, m, d_pts, host_phi ? d_phi : nullptr, host_E ? d_E : nullptr, precision);
+  if (rc) return rc;
+  if (host_phi) CUDA_TRY(cudaMemcpyAsync(host_phi, d_phi, (size_t)m * 8, cudaMemcpyDeviceToHost, c->stream));
+  if (host_E) CUDA_TRY(cudaMemcpyAsync(host_E, d_E, (size_t)m * 24, cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(cudaStreamSynchronize(c->stream));
+  return BEMCUB_OK;
+}
+
+int bemcub_fp64_peak(bemcub_ctx* c, double seconds, double* host_dfma_per_s) {
+  if (!c || !host_dfma_per_s || !(seconds > 0.0) || seconds > 30.0) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  const int threads = 256, blocks = c->num_sms * 8;
+  int rc = ensure(c->partial, (size_t)threads * blocks * 8);
+  if (rc) return rc;
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  auto run = [&](int iters, float* ms) -> int {
+    CUDA_TRY(cudaEventRecord(e0, c->stream));
+    dfma_peak_kernel<<<blocks, threads, 0, c->stream>>>((double*)c->partial.ptr, iters, 0.999999, 1e-9);
+    c->stats.kernel_launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaEventRecord(e1, c->stream));
+    CUDA_TRY(cudaEventSynchronize(e1));
+    CUDA_TRY(cudaEventElapsedTime(ms, e0, e1));
+    return BEMCUB_OK;
+  };
+  float ms = 0.f;
+  const double per_iter = 64.0 * threads * blocks;  // DFMAs per loop iteration of the whole grid
+  if ((rc = run(2000, &ms))) return rc;             // warm-up + calibration
+  if ((rc = run(20000, &ms))) return rc;
+  const double rate0 = per_iter * 20000 / (ms * 1e-3);
+  // timed: launches of ~0.25 s each until `seconds` have elapsed; report total work / total time
+  const int iters = (int)std::min(2.0e9, std::max(1000.0, 0.25 * rate0 / per_iter));
+  double total_ms = 0.0, total_fma = 0.0;
+  while (total_ms < seconds * 1e3) {
+    if ((rc = run(iters, &ms))) return rc;
+    total_ms += ms;
+    total_fma += per_iter * iters;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *host_dfma_per_s = total_fma / (total_ms * 1e-3);
+  return BEMCUB_OK;
+}
+
+int bemcub_get_stats(bemcub_ctx* c, bemcub_stats* host_stats) {
+  if (!c || !host_stats) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  refresh_counters(c);
+  *host_stats = c->stats;
+  return BEMCUB_OK;
+}
+
+int bemcub_reset_stats(bemcub_ctx* c) {
+  if (!c) return BEMCUB_ERR_INVALID_ARG;
+  c->stats = bemcub_stats{};
+  c->counters_pending = false;
+  return BEMCUB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,488 @@
+// Steps a2 + a3 + a4 of the hot path: the point-charge sum of Eq. 4.1
+// at many field points, with either one fixed rule or the distance-ratio
+// choice of Sec. 4 (L159).
+//
+// Execution model (both kernels): every WARP is an autonomous worker.  It owns 32*R field points
+// in registers (lane l holds points tile*32R + r*32 + l, r < R), walks one contiguous range of
+// elements ("split") and streams the packed (x,y,z,q) point records of those elements through its
+// private double-buffered shared-memory window, filled by 1-D bulk TMA copies
+// (cp.async.bulk -> UBLKCP) that complete on a per-warp mbarrier.  There is no __syncthreads in
+// the loop.  The inner loop reads one point with two broadcast LDS.128 and applies it to the R
+// field points of each lane: 18 FP64-pipe instructions per point-charge interaction
+// (4 DADD + 6 DMUL + 8 DFMA = 26 flop) plus one MUFU.RSQ64H.
+//
+// Adaptive kernel: per batch of 32 elements each lane classifies ONE element against the bounding
+// sphere of the warp's field points (conservative in both directions), so the rule of an element
+// is warp-uniform: elements whose whole tile falls in one distance-ratio band are streamed at that
+// level (consecutive elements merge into one bulk copy); an element whose tile straddles a band
+// limit is either evaluated with the more accurate rule (allow_upgrade) or pair by pair with the
+// exact per-pair choice; elements below the analytic limit go through analytic_integrals().
+#pragma once
+#include <math_constants.h>
+#include "analytic.cuh"
+#include "device_utils.cuh"
+#include "kernels_pre.cuh"
+
+namespace bemcub {
+
+constexpr int kWarpsPerCta = 8;
+constexpr int kThreads = kWarpsPerCta * 32;
+constexpr int kBuf = 128;  // points per stage of a warp's window
+constexpr int kStages = 2;
+
+template <typename T>
+constexpr size_t eval_smem_bytes() {
+  return (size_t)kWarpsPerCta * kStages * kBuf * sizeof(typename Point4<T>::type) + (size_t)kWarpsPerCta * kStages * 8;
+}
+
+template <typename T, int R>
+struct Accum {
+  T phi[R], ex[R], ey[R], ez[R];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int r = 0; r < R; ++r) phi[r] = ex[r] = ey[r] = ez[r] = (T)0;
+  }
+};
+
+// One point charge (sx,sy,sz,q) seen from one field point: Eq. 4.1 term.
+__device__ __forceinline__ void interact_one(double sx, double sy, double sz, double q, double px, double py, double pz,
+                                             double& phi, double& ex, double& ey, double& ez) {
+  const double dx = __dsub_rn(px, sx), dy = __dsub_rn(py, sy), dz = __dsub_rn(pz, sz);
+  const double r2 = __fma_rn(dx, dx, __fma_rn(dy, dy, __dmul_rn(dz, dz)));
+  const double y = rsqrt_f64(r2);  // 1/|P-Q_i|: "one square root and one division" (L46)
+  const double qy = __dmul_rn(q, y);
+  phi = __dadd_rn(phi, qy);
+  const double y2 = __dmul_rn(y, y);
+  const double g = __dmul_rn(qy, y2);  // q / r^3
+  ex = __fma_rn(dx, g, ex);
+  ey = __fma_rn(dy, g, ey);
+  ez = __fma_rn(dz, g, ez);
+}
+__device__ __forceinline__ void interact_one(float sx, float sy, float sz, float q, float px, float py, float pz,
+                                             float& phi, float& ex, float& ey, float& ez) {
+  const float dx = px - sx, dy = py - sy, dz = pz - sz;
+  const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+  const float y = rsqrt_f32(r2);
+  const float qy = q * y;
+  phi += qy;
+  const float g = qy * (y * y);
+  ex = fmaf(dx, g, ex);
+  ey = fmaf(dy, g, ey);
+  ez = fmaf(dz, g, ez);
+}
+
+template <typename T, int R, typename P4>
+__device__ __forceinline__ void interact(const P4 s, const T (&px)[R], const T (&py)[R], const T (&pz)[R],
+                                         Accum<T, R>& a) {
+#pragma unroll
+  for (int r = 0; r < R; ++r) interact_one(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], a.ex[r], a.ey[r], a.ez[r]);
+}
+
+// All `cnt` points of a filled window applied to the warp's field points.
+template <typename T, int R, typename P4>
+__device__ __forceinline__ void consume(const P4* __restrict__ buf, int cnt, const T (&px)[R], const T (&py)[R],
+                                        const T (&pz)[R], Accum<T, R>& a) {
+  int i = 0;
+#pragma unroll 1
+  for (; i + 2 <= cnt; i += 2) {
+    const P4 s0 = buf[i];
+    const P4 s1 = buf[i + 1];
+    interact<T, R>(s0, px, py, pz, a);
+    interact<T, R>(s1, px, py, pz, a);
+  }
+  if (i < cnt) interact<T, R>(buf[i], px, py, pz, a);
+}
+
+// FP64: the window's sum goes straight into the running totals.  FP32: the window (<= kBuf
+// terms) is summed in FP32 and the block sum is added to FP64 totals (reading 11).
+template <int R>
+__device__ __forceinline__ void consume_into(const double4* buf, int cnt, const double (&px)[R], const double (&py)[R],
+                                             const double (&pz)[R], Accum<double, R>& tot) {
+  consume<double, R>(buf, cnt, px, py, pz, tot);
+}
+template <int R>
+__device__ __forceinline__ void consume_into(const float4* buf, int cnt, const float (&px)[R], const float (&py)[R],
+                                             const float (&pz)[R], Accum<double, R>& tot) {
+  Accum<float, R> a;
+  a.zero();
+  consume<float, R>(buf, cnt, px, py, pz, a);
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    tot.phi[r] += (double)a.phi[r];
+    tot.ex[r] += (double)a.ex[r];
+    tot.ey[r] += (double)a.ey[r];
+    tot.ez[r] += (double)a.ez[r];
+  }
+}
+
+template <typename T, int R>
+__device__ __forceinline__ void load_field_points(const double* __restrict__ field, int64_t m, int64_t tile, int lane,
+                                                  T (&px)[R], T (&py)[R], T (&pz)[R]) {
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    int64_t j = tile * (32 * R) + r * 32 + lane;
+    if (j >= m) j = m - 1;  // clamped duplicates compute harmlessly and are never stored
+    px[r] = (T)field[3 * j];
+    py[r] = (T)field[3 * j + 1];
+    pz[r] = (T)field[3 * j + 2];
+  }
+}
+
+template <int R>
+__device__ __forceinline__ void store_partial(double4* __restrict__ partial, int64_t m, int64_t tile, int lane,
+                                              const Accum<double, R>& tot) {
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    const int64_t j = tile * (32 * R) + r * 32 + lane;
+    if (j < m) partial[j] = make_double4(tot.phi[r], tot.ex[r], tot.ey[r], tot.ez[r]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+struct FixedParams {
+  const void* pts;          // Point4<T>[npts], one rule level
+  int64_t npts;             // n * stride
+  int64_t pts_per_split;    // elements per split * stride
+  const double* field;      // [m][3]
+  int64_t m;
+  double4* partial;         // [nsplit][split_stride]
+  int64_t split_stride;
+  int64_t ntiles;           // ceil(m / (32 R))
+};
+
+template <typename T, int R>
+__global__ void __launch_bounds__(kThreads, 2) eval_fixed_kernel(const __grid_constant__ FixedParams p) {
+  typedef typename Point4<T>::type P4;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + warp;
+  if (tile >= p.ntiles) return;  // whole warp; no block-level barrier is ever used
+
+  P4* win = reinterpret_cast<P4*>(smem_raw) + (size_t)warp * kStages * kBuf;
+  uint64_t* bars =
+      reinterpret_cast<uint64_t*>(smem_raw + (size_t)kWarpsPerCta * kStages * kBuf * sizeof(P4)) + warp * kStages;
+  const uint32_t bar0 = smem_u32(bars), win0 = smem_u32(win);
+  if (lane == 0) {
+    mbar_init(bar0, 1);
+    mbar_init(bar0 + 8, 1);
+    mbar_fence_init();
+  }
+  __syncwarp();
+
+  T px[R], py[R], pz[R];
+  load_field_points<T, R>(p.field, p.m, tile, lane, px, py, pz);
+
+  const int64_t q0 = (int64_t)blockIdx.y * p.pts_per_split;
+  const int64_t q1 = min(p.npts, q0 + p.pts_per_split);
+  const P4* src = reinterpret_cast<const P4*>(p.pts);
+  const int64_t nchunks = (q1 - q0 + kBuf - 1) / kBuf;
+
+  Accum<double, R> tot;
+  tot.zero();
+  auto fill = [&](int64_t c, int stage) {
+    if (lane == 0) {
+      const int64_t a = q0 + c * kBuf;
+      const uint32_t bytes = (uint32_t)(min((int64_t)kBuf, q1 - a) * sizeof(P4));
+      mbar_arrive_expect_tx(bar0 + 8 * stage, bytes);
+      tma_load_1d(win0 + stage * (uint32_t)(kBuf * sizeof(P4)), src + a, bytes, bar0 + 8 * stage);
+    }
+  };
+  if (nchunks > 0) fill(0, 0);
+  uint32_t phases = 0;
+  for (int64_t c = 0; c < nchunks; ++c) {
+    const int stage = (int)(c & 1);
+    if (c + 1 < nchunks) fill(c + 1, stage ^ 1);
+    mbar_wait(bar0 + 8 * stage, (phases >> stage) & 1u);
+    phases ^= 1u << stage;
+    const int cnt = (int)min((int64_t)kBuf, q1 - (q0 + c * kBuf));
+    consume_into<R>(win + stage * kBuf, cnt, px, py, pz, tot);
+    __syncwarp();  // every lane is done with this stage before it is refilled
+  }
+  store_partial<R>(p.partial + (int64_t)blockIdx.y * p.split_stride, p.m, tile, lane, tot);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Distance-ratio policy on the device.  map[want] = level actually used for a wanted level
+// (use_levels_mask applied on the host).
+struct PolicyDev {
+  double dr[2][5];
+  int map[6];
+  int allow_upgrade;
+};
+
+// Band of a squared distance: the smallest b with D^2 < (dr[b] L)^2 gives level 5-b (b = 0 is the
+// analytic branch); none gives level 0 (N = 4).  Lower-inclusive bands (reading 8).
+__device__ __forceinline__ int want_level(double D2, double L, const double* dr5) {
+  int want = 0;
+#pragma unroll
+  for (int b = 4; b >= 0; --b) {
+    const double thr = __dmul_rn(dr5[b], L);
+    if (D2 < __dmul_rn(thr, thr)) want = 5 - b;
+  }
+  return want;
+}
+
+__device__ __forceinline__ int rule_npts(int type, int level) {
+  return type == 0 ? (c_tri_off[level + 1] - c_tri_off[level]) : (c_rect_off[level + 1] - c_rect_off[level]);
+}
+
+struct AdaptiveParams {
+  const double4* lvl_pts[5];  // expanded points per level (FP64), may be null for disabled levels
+  int stride[5];
+  const double4* cenL;
+  const uint8_t* type;
+  const double* verts;
+  const double* sigma;
+  int64_t n;
+  int64_t elems_per_split;
+  PolicyDev pol;
+  const double* field;
+  int64_t m;
+  double4* partial;
+  int64_t split_stride;
+  int64_t ntiles;
+  unsigned long long* counters;  // [0] point-charge interactions, [1] analytic pairs
+};
+
+template <int R>
+struct WarpTile {
+  double px[R], py[R], pz[R];
+  bool ok[R];  // field point exists (not a clamped duplicate)
+  double cx, cy, cz, rho, mag;  // bounding sphere of the tile, coordinate magnitude
+  int nvalid;                   // field points of this tile that exist
+};
+
+// Element `e` evaluated analytically at every field point of the tile (a4).
+template <int R>
+__device__ __forceinline__ void analytic_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, const bool (&take)[R],
+                                              Accum<double, R>& tot) {
+  Vec3 V[4];
+  const int nv = load_polygon(p.type, p.verts, e, V);
+  const double sg = __ldg(p.sigma + e);
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    if (!take[r]) continue;
+    double ip;
+    Vec3 ie;
+    analytic_integrals<true>(V, nv, Vec3{w.px[r], w.py[r], w.pz[r]}, ip, ie);
+    tot.phi[r] += sg * ip;
+    tot.ex[r] += sg * ie.x;
+    tot.ey[r] += sg * ie.y;
+    tot.ez[r] += sg * ie.z;
+  }
+}
+
+// Element `e` with the exact per-pair rule choice (tile straddles a band limit, allow_upgrade = 0).
+template <int R>
+__device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, Accum<double, R>& tot,
+                                           unsigned long long& n_inter, unsigned long long& n_ana) {
+  const double4 c = ldg4(p.cenL + e);
+  const int t = __ldg(p.type + e);
+  int lev[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    const double dx = __dsub_rn(w.px[r], c.x), dy = __dsub_rn(w.py[r], c.y), dz = __dsub_rn(w.pz[r], c.z);
+    const double D2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    lev[r] = p.pol.map[want_level(D2, c.w, p.pol.dr[t])];
+  }
+  for (int l = 0; l <= 5; ++l) {
+    bool take[R];
+    bool any = false;
+    int mine = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      take[r] = (lev[r] == l);
+      any |= take[r];
+      mine += (take[r] && w.ok[r]) ? 1 : 0;
+    }
+    if (!__any_sync(kFullMask, any)) continue;
+    if (l == 5) {
+      analytic_element<R>(p, e, w, take, tot);
+      n_ana += mine;
+    } else {
+      const int N = rule_npts(t, l);
+      const double4* src = p.lvl_pts[l] + e * p.stride[l];
+      for (int i = 0; i < N; ++i) {
+        const double4 s = ldg4(src + i);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+          interact_one(s.x, s.y, s.z, take[r] ? s.w : 0.0, w.px[r], w.py[r], w.pz[r], tot.phi[r], tot.ex[r], tot.ey[r],
+                       tot.ez[r]);
+      }
+      n_inter += (unsigned long long)mine * N;
+    }
+  }
+}
+
+template <int R>
+__global__ void __launch_bounds__(kThreads, 2) eval_adaptive_kernel(const __grid_constant__ AdaptiveParams p) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + warp;
+  if (tile >= p.ntiles) return;
+
+  double4* win = reinterpret_cast<double4*>(smem_raw) + (size_t)warp * kStages * kBuf;
+  uint64_t* bars =
+      reinterpret_cast<uint64_t*>(smem_raw + (size_t)kWarpsPerCta * kStages * kBuf * sizeof(double4)) + warp * kStages;
+  const uint32_t bar0 = smem_u32(bars), win0 = smem_u32(win);
+  if (lane == 0) {
+    mbar_init(bar0, 1);
+    mbar_init(bar0 + 8, 1);
+    mbar_fence_init();
+  }
+  __syncwarp();
+
+  WarpTile<R> w;
+  load_field_points<double, R>(p.field, p.m, tile, lane, w.px, w.py, w.pz);
+  {
+    double lox = w.px[0], hix = w.px[0], loy = w.py[0], hiy = w.py[0], loz = w.pz[0], hiz = w.pz[0];
+    int cntok = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      w.ok[r] = (tile * (32 * R) + r * 32 + lane) < p.m;
+      cntok += w.ok[r] ? 1 : 0;
+      lox = fmin(lox, w.px[r]); hix = fmax(hix, w.px[r]);
+      loy = fmin(loy, w.py[r]); hiy = fmax(hiy, w.py[r]);
+      loz = fmin(loz, w.pz[r]); hiz = fmax(hiz, w.pz[r]);
+    }
+    lox = warp_min(lox); hix = warp_max(hix);
+    loy = warp_min(loy); hiy = warp_max(hiy);
+    loz = warp_min(loz); hiz = warp_max(hiz);
+    w.cx = 0.5 * (lox + hix);
+    w.cy = 0.5 * (loy + hiy);
+    w.cz = 0.5 * (loz + hiz);
+    double d2 = 0.0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const double dx = w.px[r] - w.cx, dy = w.py[r] - w.cy, dz = w.pz[r] - w.cz;
+      d2 = fmax(d2, dx * dx + dy * dy + dz * dz);
+    }
+    w.rho = sqrt(warp_max(d2));
+    w.mag = fmax(fmax(fabs(w.cx), fabs(w.cy)), fabs(w.cz)) + w.rho;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cntok += __shfl_xor_sync(kFullMask, cntok, o);
+    w.nvalid = cntok;
+  }
+
+  const int64_t e_begin = (int64_t)blockIdx.y * p.elems_per_split;
+  const int64_t e_end = min(p.n, e_begin + p.elems_per_split);
+
+  Accum<double, R> tot;
+  tot.zero();
+  unsigned long long n_inter = 0, n_ana = 0;  // per-lane tallies, summed at the end
+
+  // state of the current 32-element batch: lane l holds element batch0 + l
+  int64_t batch_next = e_begin;
+  int cnt = 0, pre = 0, total = 0, lvl = 0, cursor = 32;
+  const double4* src = nullptr;
+
+  // Fills `stage` with the next round of whole elements; returns the number of points (0 = done).
+  auto produce = [&](int stage) -> int {
+    for (;;) {
+      if (cursor < 32) {
+        const int base = __shfl_sync(kFullMask, pre, cursor);
+        const bool after = lane >= cursor;
+        const unsigned nofit = __ballot_sync(kFullMask, after && (pre + cnt - base > kBuf));
+        const int next = nofit ? (__ffs(nofit) - 1) : 32;
+        const int pre_next = __shfl_sync(kFullMask, pre, next & 31);
+        const int endp = (next < 32) ? pre_next : total;
+        const int nstage = endp - base;
+        const bool inc = after && lane < next && cnt > 0;
+        const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
+        const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
+        // a lane continues its predecessor's copy if that one ends exactly where this one starts
+        const bool cont = inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == p.stride[lvl];
+        const unsigned heads = __ballot_sync(kFullMask, inc && !cont);
+        const unsigned higher = heads & ~((2u << lane) - 1u);
+        const int h2 = higher ? (__ffs(higher) - 1) : 32;
+        const int pre_h2 = __shfl_sync(kFullMask, pre, h2 & 31);
+        const int run_end = (h2 < 32) ? pre_h2 : endp;
+        cursor = next;
+        if (nstage == 0) continue;
+        if (lane == 0) mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
+        __syncwarp();
+        if (inc && !cont)
+          tma_load_1d(win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
+                      (uint32_t)((run_end - pre) * sizeof(double4)), bar0 + 8 * stage);
+        if (lane == 0) n_inter += (unsigned long long)nstage * w.nvalid;
+        return nstage;
+      }
+      if (batch_next >= e_end) return 0;
+      // ---- a2: classify 32 elements, one per lane, against the tile's bounding sphere
+      const int64_t batch0 = batch_next;
+      const int64_t e = batch0 + lane;
+      batch_next += 32;
+      cnt = 0;
+      lvl = -1;
+      bool is_ana = false, is_mixed = false;
+      if (e < e_end) {
+        const double4 c = p.cenL[e];
+        const int t = p.type[e];
+        const double dx = w.cx - c.x, dy = w.cy - c.y, dz = w.cz - c.z;
+        const double Dc = sqrt(dx * dx + dy * dy + dz * dz);
+        const double slack =
+            1e-9 * (Dc + w.rho) + 1e-12 * (w.mag + fmax(fmax(fabs(c.x), fabs(c.y)), fabs(c.z)));
+        const double Dhi = Dc + w.rho + slack;
+        const double Dlo = fmax(Dc - w.rho - slack, 0.0);
+        const int lfar = p.pol.map[want_level(Dhi * Dhi, c.w, p.pol.dr[t])];
+        const int lnear = p.pol.map[want_level(Dlo * Dlo, c.w, p.pol.dr[t])];
+        if (lnear != lfar && !p.pol.allow_upgrade) {
+          is_mixed = true;
+        } else {
+          lvl = lnear;  // the more accurate end of the tile's range
+          if (lvl == 5) {
+            is_ana = true;
+          } else {
+            cnt = rule_npts(t, lvl);
+            src = p.lvl_pts[lvl] + e * p.stride[lvl];
+          }
+        }
+      }
+      pre = warp_excl_scan(cnt, lane, &total);
+      cursor = 0;
+      unsigned amask = __ballot_sync(kFullMask, is_ana), xmask = __ballot_sync(kFullMask, is_mixed);
+      while (amask) {
+        const int l = __ffs(amask) - 1;
+        amask &= amask - 1;
+        analytic_element<R>(p, batch0 + l, w, w.ok, tot);
+        if (lane == 0) n_ana += w.nvalid;
+      }
+      while (xmask) {
+        const int l = __ffs(xmask) - 1;
+        xmask &= xmask - 1;
+        mixed_element<R>(p, batch0 + l, w, tot, n_inter, n_ana);
+      }
+    }
+  };
+
+  // software pipeline with a single produce() call site: fill stage s^1, then consume stage s
+  int cur = 0, stage = 1;
+  uint32_t phases = 0;
+  for (;;) {
+    const int nxt = produce(stage ^ 1);
+    if (cur > 0) {
+      mbar_wait(bar0 + 8 * stage, (phases >> stage) & 1u);
+      phases ^= 1u << stage;
+      consume_into<R>(win + stage * kBuf, cur, w.px, w.py, w.pz, tot);
+      __syncwarp();
+    }
+    if (nxt == 0) break;
+    stage ^= 1;
+    cur = nxt;
+  }
+  store_partial<R>(p.partial + (int64_t)blockIdx.y * p.split_stride, p.m, tile, lane, tot);
+
+  if (p.counters) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      n_inter += __shfl_xor_sync(kFullMask, n_inter, o);
+      n_ana += __shfl_xor_sync(kFullMask, n_ana, o);
+    }
+    if (lane == 0) {
+      atomicAdd(p.counters, n_inter);
+      if (n_ana) atomicAdd(p.counters + 1, n_ana);
+    }
+  }
+}
+
+}  // namespace bemcub

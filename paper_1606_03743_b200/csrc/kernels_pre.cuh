@@ -1,0 +1,170 @@
+// Step a1 of the hot path: element preprocessing.
+//   geometry_kernel : per element centroid Q_cen, area A, mean side L, validity
+//   expand_kernel   : per (element, rule point) the Gaussian point Q_i by Eq. 3.3 (triangle, L109)
+//                     or Eq. 3.2 (rectangle, L103) and its charge q_i = w_i sigma A (L143),
+//                     stored as one packed (x,y,z,q) record per point, one array per rule level.
+#pragma once
+#include "device_utils.cuh"
+
+namespace bemcub {
+
+// Rule tables in constant memory, filled by bemcub_create from rules.h.
+// Triangle: (lambda_A, lambda_B, lambda_C, w) per point; rectangle: (x, y, w, 0).
+__constant__ double c_tri_tab[75 * 4];
+__constant__ double c_rect_tab[73 * 4];
+__constant__ int c_tri_off[6];
+__constant__ int c_rect_off[6];
+
+struct GeomStatus {
+  int code;  // min over elements of the (negative) error code, 0 = fine
+  int pad;
+  unsigned long long n_tri, n_rect;
+};
+
+// cenL[e] = (Q_cen.x, Q_cen.y, Q_cen.z, L); area[e] = A.
+__global__ void geometry_kernel(int64_t n, const uint8_t* __restrict__ type, const double* __restrict__ verts,
+                                double4* __restrict__ cenL, double* __restrict__ area, GeomStatus* status) {
+  const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  const double* v = verts + 9 * e;
+  const double ax = v[0], ay = v[1], az = v[2];
+  const double e1x = v[3] - ax, e1y = v[4] - ay, e1z = v[5] - az;
+  const double e2x = v[6] - ax, e2y = v[7] - ay, e2z = v[8] - az;
+  const int t = type[e];
+  double4 c;
+  double A;
+  int code = 0;
+  if (t == 0) {
+    // triangle A,B,C: area = |AB x AC|/2, centroid = (A+B+C)/3, L = (|AB|+|BC|+|CA|)/3
+    const double nx = e1y * e2z - e1z * e2y, ny = e1z * e2x - e1x * e2z, nz = e1x * e2y - e1y * e2x;
+    A = 0.5 * sqrt(nx * nx + ny * ny + nz * nz);
+    c.x = (ax + v[3] + v[6]) / 3.0;
+    c.y = (ay + v[4] + v[7]) / 3.0;
+    c.z = (az + v[5] + v[8]) / 3.0;
+    const double bx = v[6] - v[3], by = v[7] - v[4], bz = v[8] - v[5];
+    c.w = (sqrt(e1x * e1x + e1y * e1y + e1z * e1z) + sqrt(bx * bx + by * by + bz * bz) +
+           sqrt(e2x * e2x + e2y * e2y + e2z * e2z)) / 3.0;
+    if (!(A > 0.0)) code = -2;
+  } else if (t == 1) {
+    // rectangle P0, P1 = P0 + a u_x, P3 = P0 + b u_y: A = ab, centre = P0 + e1/2 + e2/2, L = (a+b)/2
+    const double a = sqrt(e1x * e1x + e1y * e1y + e1z * e1z), b = sqrt(e2x * e2x + e2y * e2y + e2z * e2z);
+    A = a * b;
+    c.x = ax + 0.5 * e1x + 0.5 * e2x;
+    c.y = ay + 0.5 * e1y + 0.5 * e2y;
+    c.z = az + 0.5 * e1z + 0.5 * e2z;
+    c.w = 0.5 * (a + b);
+    if (!(a > 0.0) || !(b > 0.0)) code = -2;
+    else if (fabs(e1x * e2x + e1y * e2y + e1z * e2z) > 1e-12 * a * b) code = -3;
+  } else {
+    A = 0.0;
+    c = make_double4(0, 0, 0, 0);
+    code = -1;
+  }
+  cenL[e] = c;
+  area[e] = A;
+  if (code) atomicMin(&status->code, code);
+  // element-type census, one atomic per warp
+  const unsigned act = __activemask();
+  const unsigned tris = __ballot_sync(act, t == 0), rects = __ballot_sync(act, t == 1);
+  if ((threadIdx.x & 31) == __ffs(act) - 1) {
+    if (tris) atomicAdd(&status->n_tri, (unsigned long long)__popc(tris));
+    if (rects) atomicAdd(&status->n_rect, (unsigned long long)__popc(rects));
+  }
+}
+
+template <typename T> struct Point4;
+template <> struct Point4<double> { typedef double4 type; };
+template <> struct Point4<float> { typedef float4 type; };
+
+__device__ __forceinline__ void store_point(double4* dst, double x, double y, double z, double q) {
+  *dst = make_double4(x, y, z, q);
+}
+__device__ __forceinline__ void store_point(float4* dst, double x, double y, double z, double q) {
+  *dst = make_float4((float)x, (float)y, (float)z, (float)q);
+}
+
+// One thread per (element, slot); slot < stride.  Slots beyond the element's own N are padding:
+// zero charge at the centroid.  sigma == nullptr means unit sigma (matrix assembly, L34).
+template <typename T>
+__global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* __restrict__ type,
+                              const double* __restrict__ verts, const double4* __restrict__ cenL,
+                              const double* __restrict__ area, const double* __restrict__ sigma,
+                              typename Point4<T>::type* __restrict__ out) {
+  const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (idx >= n * stride) return;
+  const int64_t e = idx / stride;
+  const int i = (int)(idx - e * stride);
+  const int t = type[e];
+  const double* v = verts + 9 * e;
+  const double q = (sigma ? sigma[e] : 1.0) * area[e];  // q = sigma A (L143)
+  if (t == 0) {
+    const int N = c_tri_off[level + 1] - c_tri_off[level];
+    if (i < N) {
+      const double* r = c_tri_tab + 4 * (c_tri_off[level] + i);
+      const double la = r[0], lb = r[1], lc = r[2];
+      // Eq. 3.3: Q = lambda_A A + lambda_B B + lambda_C C
+      const double x = fma(lc, v[6], fma(lb, v[3], la * v[0]));
+      const double y = fma(lc, v[7], fma(lb, v[4], la * v[1]));
+      const double z = fma(lc, v[8], fma(lb, v[5], la * v[2]));
+      store_point(out + idx, x, y, z, r[3] * q);
+      return;
+    }
+  } else {
+    const int N = c_rect_off[level + 1] - c_rect_off[level];
+    if (i < N) {
+      const double* r = c_rect_tab + 4 * (c_rect_off[level] + i);
+      const double4 c = cenL[e];
+      const double xs = 0.5 * r[0], ys = 0.5 * r[1];
+      // Eq. 3.2: Q = Q_cen + (a/2) x u_x + (b/2) y u_y, with a u_x = P1 - P0 and b u_y = P3 - P0
+      const double x = fma(ys, v[6] - v[0], fma(xs, v[3] - v[0], c.x));
+      const double y = fma(ys, v[7] - v[1], fma(xs, v[4] - v[1], c.y));
+      const double z = fma(ys, v[8] - v[2], fma(xs, v[5] - v[2], c.z));
+      store_point(out + idx, x, y, z, r[2] * q);
+      return;
+    }
+  }
+  const double4 c = cenL[e];
+  store_point(out + idx, c.x, c.y, c.z, 0.0);
+}
+
+// Step a6: sum the per-split partial results in split order and apply k = 1/(4 pi eps0) once
+// (Eq. 4.1 prefactor, L141).
+__global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride, const double4* __restrict__ partial,
+                                    double k, double* __restrict__ phi, double* __restrict__ E) {
+  const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (j >= m) return;
+  double4 s = partial[j];
+  for (int sp = 1; sp < nsplit; ++sp) {
+    const double4 p = partial[sp * split_stride + j];
+    s.x += p.x;
+    s.y += p.y;
+    s.z += p.z;
+    s.w += p.w;
+  }
+  if (phi) phi[j] = k * s.x;
+  if (E) {
+    E[3 * j] = k * s.y;
+    E[3 * j + 1] = k * s.z;
+    E[3 * j + 2] = k * s.w;
+  }
+}
+
+// Roofline denominator: 16 independent DFMA chains per thread, nothing else in the loop.
+__global__ void dfma_peak_kernel(double* out, int iters, double a, double b) {
+  double x[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) x[k] = (double)(threadIdx.x + k) * 1e-3;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+#pragma unroll
+      for (int k = 0; k < 16; ++k) x[k] = __fma_rn(x[k], a, b);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += x[k];
+  out[blockIdx.x * (int64_t)blockDim.x + threadIdx.x] = s;
+}
+
+}  // namespace bemcub
