@@ -83,7 +83,9 @@ enum {
  * analytic only, L239).  allow_upgrade = 1 lets the library evaluate an (element, field-point
  * tile) with the most accurate rule any pair of the tile asks for, instead of choosing per pair;
  * results then differ from the per-pair policy only by the (smaller) truncation error of the
- * better rule.  allow_upgrade = 0 reproduces the per-pair choice exactly. */
+ * better rule.  Only cubature rules are upgraded to better cubature rules; the analytic branch
+ * is always chosen pair by pair (its rounding error grows with the distance ratio, L44, so it
+ * is no upgrade far away).  allow_upgrade = 0 reproduces the per-pair choice exactly. */
 typedef struct {
   double dr[2][5];
   int32_t allow_upgrade;
@@ -159,6 +161,14 @@ int bemcub_get_geometry(bemcub_ctx* ctx, double* out_cen, double* out_area, doub
 /* Roofline denominator: runs a dependent-chain-free DFMA kernel on all SMs for about `seconds`
  * and returns the sustained rate in FP64 FMA/s (flop/s = 2x).  Synchronises. */
 int bemcub_fp64_peak(bemcub_ctx* ctx, double seconds, double* host_dfma_per_s);
+
+/* Device timing of the dominant kernel.  bemcub_set_timing(ctx, 1) makes every following
+ * bemcub_eval / bemcub_assemble* call record CUDA events on the ctx stream: around the whole call
+ * and around its dominant kernel (the evaluation kernel of a3, the fill kernel of a5).
+ * bemcub_get_timing waits for the most recent such call to finish and returns both durations in
+ * milliseconds (HOST outputs, either may be NULL); INVALID_ARG if no timed call has been made. */
+int bemcub_set_timing(bemcub_ctx* ctx, int enable);
+int bemcub_get_timing(bemcub_ctx* ctx, double* host_ms_total, double* host_ms_kernel);
 
 int bemcub_get_stats(bemcub_ctx* ctx, bemcub_stats* host_stats);  /* synchronises the stream */
 int bemcub_reset_stats(bemcub_ctx* ctx);

@@ -68,6 +68,8 @@ def _load() -> C.CDLL:
         "bemcub_fp64_peak": [vp, dbl, C.POINTER(dbl)],
         "bemcub_get_stats": [vp, C.POINTER(bemcub_stats)],
         "bemcub_reset_stats": [vp],
+        "bemcub_set_timing": [vp, C.c_int],
+        "bemcub_get_timing": [vp, C.POINTER(dbl), C.POINTER(dbl)],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -82,15 +84,19 @@ _lib = _load()
 EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval",
             "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
             "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
-            "bemcub_fp64_peak", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_strerror"]
+            "bemcub_fp64_peak", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
+            "bemcub_get_timing", "bemcub_strerror"]
 
 
 def library_path() -> str:
     return str(_build.LIB)
 
 
-def strerror(code: int) -> str:
+def bemcub_strerror(code: int) -> str:
     return _lib.bemcub_strerror(code).decode()
+
+
+strerror = bemcub_strerror
 
 
 def _check(rc: int, where: str) -> None:
@@ -218,6 +224,17 @@ def bemcub_get_stats(ctx) -> dict:
     s = bemcub_stats()
     _check(_lib.bemcub_get_stats(ctx, C.byref(s)), "bemcub_get_stats")
     return {k: getattr(s, k) for k, _ in bemcub_stats._fields_}
+
+
+def bemcub_set_timing(ctx, enable: bool) -> None:
+    _check(_lib.bemcub_set_timing(ctx, int(enable)), "bemcub_set_timing")
+
+
+def bemcub_get_timing(ctx):
+    """(ms of the whole call, ms of its dominant kernel) of the most recent timed call."""
+    a, b = C.c_double(), C.c_double()
+    _check(_lib.bemcub_get_timing(ctx, C.byref(a), C.byref(b)), "bemcub_get_timing")
+    return a.value, b.value
 
 
 def bemcub_reset_stats(ctx) -> None:

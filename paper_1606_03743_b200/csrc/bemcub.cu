@@ -51,6 +51,10 @@ struct bemcub_ctx {
   unsigned long long* d_counters = nullptr;
   bemcub_stats stats{};
   bool counters_pending = false;
+  // optional per-call timing of the dominant kernel (bemcub_set_timing)
+  bool timing = false;
+  bool timing_valid = false;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 namespace {
@@ -235,6 +239,11 @@ int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp
   return BEMCUB_OK;
 }
 
+// ev[0] call start, ev[1] before the dominant kernel, ev[2] after it, ev[3] call end
+void mark(bemcub_ctx* c, int i) {
+  if (c->timing) cudaEventRecord(c->ev[i], c->stream);
+}
+
 void refresh_counters(bemcub_ctx* c) {
   if (!c->counters_pending) return;
   unsigned long long h[2] = {0, 0};
@@ -346,6 +355,8 @@ int bemcub_destroy(bemcub_ctx* c) {
   for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); }
   if (c->d_status) cudaFree(c->d_status);
   if (c->d_counters) cudaFree(c->d_counters);
+  for (int i = 0; i < 4; ++i)
+    if (c->ev[i]) cudaEventDestroy(c->ev[i]);
   delete c;
   return BEMCUB_OK;
 }
@@ -443,6 +454,8 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     return BEMCUB_OK;
   }
 
+  c->timing_valid = false;
+  mark(c, 0);
   // a1: expand the levels this call needs, sigma folded in
   if (adaptive) {
     for (int l = 0; l < 5; ++l) {
@@ -458,6 +471,7 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
 
   const SplitPlan sp = plan_splits(c, m, true);
   if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
+  mark(c, 1);
 
   if (!adaptive) {
     FixedParams fp;
@@ -502,12 +516,15 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     c->counters_pending = true;
   }
 
+  mark(c, 2);
   // a6: cross-split reduction and the 1/(4 pi eps0) prefactor
   const int threads = 256;
   reduce_scale_kernel<<<(unsigned)((m + threads - 1) / threads), threads, 0, c->stream>>>(
       m, sp.nsplit, m, (const double4*)c->partial.ptr, coulomb_k(), out_phi, out_E);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
+  mark(c, 3);
+  c->timing_valid = c->timing;
   return BEMCUB_OK;
 }
 
@@ -523,6 +540,8 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   if (!out_rows) return BEMCUB_ERR_INVALID_ARG;
   DeviceGuard g(c->device);
   c->stats.last_eval_launches = 0;
+  c->timing_valid = false;
+  mark(c, 0);
   AssembleParams ap;
   for (int l = 0; l < 5; ++l) {
     bool used = false;
@@ -548,9 +567,13 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   // rows on grid.x would exceed no limit either way; y is limited to 65535 tiles = 2.1 M rows per call
   if (rowtiles > 65535) return BEMCUB_ERR_INVALID_ARG;
   dim3 grid((unsigned)((coltiles + kWarpsPerCta - 1) / kWarpsPerCta), (unsigned)rowtiles);
+  mark(c, 1);
   assemble_kernel<<<grid, kThreads, assemble_smem_bytes(), c->stream>>>(ap);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
+  mark(c, 2);
+  mark(c, 3);
+  c->timing_valid = c->timing;
   c->counters_pending = true;
   return BEMCUB_OK;
 }
@@ -643,6 +666,30 @@ int bemcub_get_stats(bemcub_ctx* c, bemcub_stats* host_stats) {
   DeviceGuard g(c->device);
   refresh_counters(c);
   *host_stats = c->stats;
+  return BEMCUB_OK;
+}
+
+int bemcub_set_timing(bemcub_ctx* c, int enable) {
+  if (!c) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  if (enable)
+    for (int i = 0; i < 4; ++i)
+      if (!c->ev[i]) CUDA_TRY(cudaEventCreate(&c->ev[i]));
+  c->timing = enable != 0;
+  c->timing_valid = false;
+  return BEMCUB_OK;
+}
+
+int bemcub_get_timing(bemcub_ctx* c, double* host_ms_total, double* host_ms_kernel) {
+  if (!c) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->timing_valid) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  CUDA_TRY(cudaEventSynchronize(c->ev[3]));
+  float a = 0.f, b = 0.f;
+  CUDA_TRY(cudaEventElapsedTime(&a, c->ev[0], c->ev[3]));
+  CUDA_TRY(cudaEventElapsedTime(&b, c->ev[1], c->ev[2]));
+  if (host_ms_total) *host_ms_total = a;
+  if (host_ms_kernel) *host_ms_kernel = b;
   return BEMCUB_OK;
 }
 

@@ -71,7 +71,9 @@ __global__ void __launch_bounds__(kThreads, 2) assemble_kernel(const __grid_cons
     const double Dhi = Dc + rho + slack, Dlo = fmax(Dc - rho - slack, 0.0);
     lfar = p.pol.map[want_level(Dhi * Dhi, cj.w, p.pol.dr[tcol])];
     lnear = p.pol.map[want_level(Dlo * Dlo, cj.w, p.pol.dr[tcol])];
-    if (p.pol.allow_upgrade) lfar = lnear;
+    // the analytic formula is never an "upgrade" (see eval_adaptive_kernel): a tile straddling
+    // the analytic limit keeps the exact per-pair choice
+    if (p.pol.allow_upgrade && lnear != 5) lfar = lnear;
   }
 
   unsigned long long n_inter = 0, n_ana = 0;

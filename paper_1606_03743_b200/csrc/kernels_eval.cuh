@@ -426,7 +426,11 @@ __global__ void __launch_bounds__(kThreads, 2) eval_adaptive_kernel(const __grid
         const double Dlo = fmax(Dc - w.rho - slack, 0.0);
         const int lfar = p.pol.map[want_level(Dhi * Dhi, c.w, p.pol.dr[t])];
         const int lnear = p.pol.map[want_level(Dlo * Dlo, c.w, p.pol.dr[t])];
-        if (lnear != lfar && !p.pol.allow_upgrade) {
+        // A tile that straddles a band limit: per-pair choice, or (allow_upgrade) the more accurate
+        // cubature rule for the whole tile.  The analytic formula is never an "upgrade": its
+        // rounding error grows with the distance ratio (Figs. 2-4), so a tile that
+        // straddles the analytic limit is always resolved pair by pair.
+        if (lnear != lfar && (!p.pol.allow_upgrade || lnear == 5)) {
           is_mixed = true;
         } else {
           lvl = lnear;  // the more accurate end of the tile's range

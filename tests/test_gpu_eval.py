@@ -1,0 +1,251 @@
+"""-m gpu parity tests of bemcub_eval (steps a1, a2, a3, a4, a6 of DESIGN.md §2) against the CPU
+oracle, element by element on the same seeded inputs, through the C ABI."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1606_03743_b200 import synth
+
+from gpu_common import Gpu, TOL_F32, TOL_F64, assert_parity, parity_errors
+
+pytestmark = pytest.mark.gpu
+
+
+def _mixed_mesh(n_tri, n_rect, seed):
+    tt, tv = synth.random_elements(synth.TRI, n_tri, seed)
+    rt, rv = synth.random_elements(synth.RECT, n_rect, seed + 1)
+    etype = np.concatenate([tt, rt])
+    verts = np.concatenate([tv, rv], axis=0)
+    perm = np.random.default_rng(seed + 2).permutation(len(etype))
+    return np.ascontiguousarray(etype[perm]), np.ascontiguousarray(verts[perm])
+
+
+def _far_points(m, seed, lo=3.0, hi=8.0):
+    rng = np.random.default_rng(seed)
+    d = synth.isotropic_directions(rng, m)
+    return np.ascontiguousarray(0.5 + d * rng.uniform(lo, hi, m)[:, None])
+
+
+# ------------------------------------------------------------------ a1: preprocessing
+@pytest.mark.parametrize("n_tri,n_rect", [(50, 0), (0, 50), (37, 41)])
+def test_geometry_and_expanded_points(n_tri, n_rect):
+    etype, verts = _mixed_mesh(n_tri, n_rect, 11)
+    n = len(etype)
+    sigma = np.random.default_rng(5).uniform(-1, 1, n)
+    g = Gpu(etype, verts)
+    torch, b = g.torch, g.b
+    cen = torch.empty((n, 3), dtype=torch.float64, device="cuda")
+    area = torch.empty(n, dtype=torch.float64, device="cuda")
+    L = torch.empty(n, dtype=torch.float64, device="cuda")
+    b.bemcub_get_geometry(g.ctx.handle, cen, area, L)
+    torch.cuda.synchronize()
+    ocen, oarea, oL = oracle.geometry(etype, verts)
+    np.testing.assert_allclose(cen.cpu().numpy(), ocen, rtol=0, atol=4e-16)
+    np.testing.assert_allclose(area.cpu().numpy(), oarea, rtol=4e-16)
+    np.testing.assert_allclose(L.cpu().numpy(), oL, rtol=4e-16)
+    d_sigma = torch.as_tensor(sigma).cuda()
+    for level in range(5):
+        ntri, _ = oracle.rule_info(0, level)
+        nrect, _ = oracle.rule_info(1, level)
+        stride = max(ntri if n_tri else 0, nrect if n_rect else 0)
+        out = torch.full((n * stride, 4), float("nan"), dtype=torch.float64, device="cuda")
+        got_stride = b.bemcub_expand_points(g.ctx.handle, d_sigma, level, out)
+        torch.cuda.synchronize()
+        assert got_stride == stride
+        got = out.cpu().numpy().reshape(n, stride, 4)
+        ref = oracle.points(etype, verts, sigma, level)  # concatenated, N_e points per element
+        pos = 0
+        for e in range(n):
+            N = ntri if etype[e] == 0 else nrect
+            np.testing.assert_allclose(got[e, :N, :3], ref[pos:pos + N, :3], rtol=0, atol=5e-16)
+            np.testing.assert_allclose(got[e, :N, 3], ref[pos:pos + N, 3], rtol=5e-16, atol=0)
+            assert np.all(got[e, N:, 3] == 0.0)            # padding carries no charge
+            np.testing.assert_allclose(got[e, N:, :3], np.broadcast_to(ocen[e], (stride - N, 3)), atol=4e-16)
+            pos += N
+        assert pos == len(ref)
+    g.close()
+
+
+# ------------------------------------------------------------------ configs 1 and 2, fixed rules
+def test_cfg1_icosphere_n7_f64():
+    c = synth.config1()
+    g = Gpu(c["etype"], c["verts"])
+    phi, E = g.eval(c["sigma"], c["pts"], 1)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], 1)
+    assert_parity(phi, E, ref, TOL_F64, "cfg1")
+    # exact sphere: Phi = k Q_tot / r up to the l >= 6 multipoles of the icosphere
+    _, area, _ = oracle.geometry(c["etype"], c["verts"])
+    r = np.linalg.norm(c["pts"], axis=1)
+    point = oracle.coulomb_k() * 1e-9 * area.sum() / r
+    assert np.max(np.abs(phi / point - 1.0)) < 2e-5
+    assert g.stats()["point_interactions"] == 1280 * 7 * 1000
+    g.close()
+
+
+@pytest.mark.parametrize("level", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_cfg2_cube_all_rules(level, precision):
+    m = 10000 if level <= 1 else 3000
+    c = synth.config2(m=m)
+    g = Gpu(c["etype"], c["verts"])
+    phi, E = g.eval(c["sigma"], c["pts"], level, precision=precision)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], level)
+    assert_parity(phi, E, ref, TOL_F64 if precision == 0 else TOL_F32, f"cfg2 L{level} p{precision}")
+    g.close()
+
+
+# ------------------------------------------------------------------ ragged / edge shapes
+@pytest.mark.parametrize("n_tri,n_rect,m", [(1, 0, 1), (0, 1, 5), (3, 2, 33), (129, 70, 257), (700, 613, 1031),
+                                              (5, 5, 20000)])
+@pytest.mark.parametrize("level", [1, 3])
+def test_ragged_shapes_fixed(n_tri, n_rect, m, level):
+    etype, verts = _mixed_mesh(n_tri, n_rect, 100 + n_tri)
+    sigma = np.random.default_rng(9).uniform(-1e-9, 1e-9, len(etype))
+    pts = _far_points(m, 17)
+    g = Gpu(etype, verts)
+    for precision, tol in ((0, TOL_F64), (1, TOL_F32)):
+        phi, E = g.eval(sigma, pts, level, precision=precision)
+        ref = oracle.evaluate(etype, verts, sigma, pts, level)
+        assert_parity(phi, E, ref, tol, f"ragged n={len(etype)} m={m} L{level} p{precision}")
+    # potential only (out_E = NULL) gives the same potential
+    phi2, _ = g.eval(sigma, pts, level, want_E=False)
+    assert np.array_equal(phi2, g.eval(sigma, pts, level)[0])
+    g.close()
+
+
+def test_empty_inputs():
+    etype, verts = _mixed_mesh(4, 4, 3)
+    g = Gpu(etype, verts)
+    phi, E = g.eval(np.ones(8), np.zeros((0, 3)), 1)           # m = 0: no-op
+    assert phi.shape == (0,) and E.shape == (0, 3)
+    g.close()
+    g0 = Gpu(np.zeros(0, dtype=np.uint8), np.zeros((0, 3, 3)))  # n = 0: zero potential and field
+    phi, E = g0.eval(np.zeros(0), _far_points(10, 1), 1)
+    assert np.all(phi == 0.0) and np.all(E == 0.0)
+    g0.close()
+
+
+def test_error_codes():
+    g = Gpu(*_mixed_mesh(2, 2, 8))
+    b, torch = g.b, g.torch
+    h = g.ctx.handle
+    bad = np.zeros((1, 3, 3))
+    bad[0, 1] = [1, 0, 0]
+    bad[0, 2] = [2, 0, 0]                                         # collinear triangle
+    for etype, verts, code in ((np.array([0], np.uint8), bad, b.ERR_DEGENERATE_ELEMENT),
+                               (np.array([1], np.uint8), np.array([[[0, 0, 0], [1, 0, 0], [0.5, 1, 0]]], float),
+                                b.ERR_NOT_RECTANGLE),
+                               (np.array([7], np.uint8), np.array([[[0, 0, 0], [1, 0, 0], [0, 1, 0]]], float),
+                                b.ERR_INVALID_ARG)):
+        with pytest.raises(b.BemcubError) as ei:
+            b.bemcub_set_elements(h, 1, torch.as_tensor(etype).cuda(), torch.as_tensor(verts).cuda())
+        assert ei.value.code == code
+        with pytest.raises(b.BemcubError) as ei:                  # the ctx holds no mesh after a failure
+            g.eval(np.ones(1), _far_points(3, 1), 1)
+        assert ei.value.code == b.ERR_NO_ELEMENTS
+    g.close()
+    g = Gpu(*_mixed_mesh(2, 2, 8))
+    with pytest.raises(g.b.BemcubError) as ei:
+        g.eval(np.ones(4), _far_points(3, 1), 9)
+    assert ei.value.code == g.b.ERR_BAD_RULE
+    with pytest.raises(g.b.BemcubError) as ei:
+        g.eval(np.ones(4), _far_points(3, 1), -1, policy=None)   # adaptive needs a policy
+    assert ei.value.code == g.b.ERR_INVALID_ARG
+    g.close()
+
+
+def test_host_entry_points_match_device_path():
+    c = synth.config1(m=500)
+    g = Gpu(c["etype"], c["verts"])
+    phi_d, E_d = g.eval(c["sigma"], c["pts"], 1)
+    b = g.b
+    ctx2 = b.Context(0)
+    b.bemcub_set_elements_host(ctx2.handle, len(c["etype"]), c["etype"], c["verts"])
+    phi_h, E_h = np.zeros(500), np.zeros((500, 3))
+    b.bemcub_eval_host(ctx2.handle, c["sigma"], 1, None, 500, c["pts"], phi_h, E_h)
+    assert np.array_equal(phi_h, phi_d) and np.array_equal(E_h, E_d)
+    ctx2.close()
+    g.close()
+
+
+# ------------------------------------------------------------------ a2 + a4: adaptive mode
+def _policy(b, want_field, allow_upgrade, mask=63, dr=None):
+    p = b.bemcub_default_policy(want_field)
+    if dr is not None:
+        p = b.make_policy(dr, allow_upgrade, mask)
+    p.allow_upgrade = int(allow_upgrade)
+    p.use_levels_mask = mask
+    return p
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+def test_cfg5_single_element_adaptive(kind, allow_upgrade):
+    """All six branches (analytic, N = 33 ... 4) on one element: DR log-uniform in [0.3, 1e4]."""
+    c = synth.config5(kind, m=20000, dr_lo=0.3, dr_hi=1e4)
+    g = Gpu(c["etype"], c["verts"])
+    pol = _policy(g.b, True, allow_upgrade)
+    dr = oracle.default_policy(True)
+    phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=dr, want_counts=True)
+    assert_parity(phi, E, ref, TOL_F64, f"cfg5 kind={kind} upgrade={allow_upgrade}")
+    st = g.stats()
+    if not allow_upgrade:                                           # exact per-pair policy: same work
+        assert st["point_interactions"] == int(ref["npi"].sum())
+    else:
+        assert st["point_interactions"] >= int(ref["npi"].sum())
+    assert st["analytic_pairs"] > 0
+    g.close()
+
+
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+@pytest.mark.parametrize("mask", [63, 0b110110])   # all levels | the paper's GPU set 7/12/33 + analytic (L239)
+def test_cfg4_small_mixed_adaptive(allow_upgrade, mask):
+    """Config 4 shrunk to ~2000 elements: elements are large, so field points see every band,
+    including the analytic one; triangles and rectangles mixed; several tiles and splits."""
+    c = synth.config4(scale=0.002, ntracks=40, npts_per_track=53)
+    g = Gpu(c["etype"], c["verts"])
+    pol = _policy(g.b, True, allow_upgrade, mask)
+    dr = oracle.default_policy(True)
+    phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=dr, levels_mask=mask,
+                          want_counts=True)
+    assert_parity(phi, E, ref, TOL_F64, f"cfg4-small upgrade={allow_upgrade} mask={mask}")
+    if not allow_upgrade:
+        assert g.stats()["point_interactions"] == int(ref["npi"].sum())
+    g.close()
+
+
+def test_adaptive_policy_potential_limits_and_custom():
+    """want_field = 0 limits (L159) and a custom policy with wide near bands."""
+    etype, verts = _mixed_mesh(150, 150, 77)
+    sigma = np.random.default_rng(1).uniform(-1e-9, 1e-9, 300)
+    rng = np.random.default_rng(2)
+    pts = np.ascontiguousarray(rng.uniform(-3.0, 4.0, (3001, 3)))
+    g = Gpu(etype, verts)
+    for dr, want_field in ((None, False), (np.array([[5, 12, 30, 120, 2500.0], [7, 18, 45, 200, 4000.0]]), True)):
+        for up in (0, 1):
+            pol = _policy(g.b, want_field, up, dr=dr)
+            odr = oracle.default_policy(want_field) if dr is None else dr
+            phi, E = g.eval(sigma, pts, -1, policy=pol)
+            ref = oracle.evaluate(etype, verts, sigma, pts, -1, dr=odr)
+            # points may fall inside the element cloud; the analytic branch handles them
+            err = parity_errors(phi, E, ref)
+            assert err["phi"] <= 1e-10 and err["E"] <= 1e-10, (err, up, want_field)
+    g.close()
+
+
+# ------------------------------------------------------------------ full-size config 4 (bench launch config)
+def test_cfg4_full_size_sampled():
+    """10^6 elements x 10^6 field points, adaptive, the exact call bench.py times; the oracle
+    recomputes 48 sampled field points one by one."""
+    c = synth.config4()
+    assert len(c["etype"]) == 1_000_000 and len(c["pts"]) == 1_000_000
+    g = Gpu(c["etype"], c["verts"])
+    pol = _policy(g.b, True, 1)
+    phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+    assert np.all(np.isfinite(phi)) and np.all(np.isfinite(E))
+    idx = np.random.default_rng(160603749).choice(len(phi), 48, replace=False)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx], -1, dr=oracle.default_policy(True))
+    assert_parity(phi[idx], E[idx], ref, TOL_F64, "cfg4 full")
+    g.close()
