@@ -190,23 +190,33 @@ int expand_level(bemcub_ctx* c, int level, const double* sigma, DevBuf& dst) {
 
 struct SplitPlan {
   int R;
-  int64_t ntiles, ctas_x;
+  int64_t ntiles;
   int nsplit;
   int64_t elems_per_split;
+  int64_t nitems;
+  int grid;
 };
 
-// Work decomposition: warp item = (tile of 32R field points) x (split of the elements).  Enough
-// CTAs for ~50 waves on all SMs at 2 CTAs/SM so the tail is small; splits are multiples of 32
-// elements (the adaptive kernel's batch) and at least 256 elements long.
-SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, bool allow_r2) {
+// Work decomposition of the persistent evaluation kernels: item = (tile of 32R field points) x
+// (split of the elements), pulled from an atomic queue by num_sms x 12 warps.  R (field points per
+// lane) is as large as the problem allows while still giving every warp several items; the splits
+// (multiples of 32 elements, the adaptive kernel's batch) make the items small enough that the
+// tail of the launch - at most one item per warp - stays around one percent.
+SplitPlan plan_splits(const bemcub_ctx* c, int64_t m) {
   SplitPlan s;
-  const int64_t slots = (int64_t)c->num_sms * 2;
-  s.R = (allow_r2 && m >= slots * kWarpsPerCta * 64) ? 2 : 1;
+  const int64_t warps = (int64_t)c->num_sms * kWarpsPerCta;
+  const int64_t max_by_len = std::max<int64_t>(1, c->n / 64);
+  s.R = 1;
+  for (int R = 4; R > 1; R >>= 1) {
+    const int64_t nt = (m + 32 * R - 1) / (32 * R);
+    if (nt * std::min<int64_t>(max_by_len, 64) >= 8 * warps) {
+      s.R = R;
+      break;
+    }
+  }
   s.ntiles = (m + 32 * s.R - 1) / (32 * s.R);
-  s.ctas_x = (s.ntiles + kWarpsPerCta - 1) / kWarpsPerCta;
-  const int64_t target = slots * 50;
-  int64_t ns = (target + s.ctas_x - 1) / s.ctas_x;
-  const int64_t max_by_len = std::max<int64_t>(1, c->n / 256);
+  const int64_t target = warps * 64;
+  int64_t ns = (target + s.ntiles - 1) / s.ntiles;
   const int64_t max_by_mem = std::max<int64_t>(1, (int64_t)(1ull << 31) / std::max<int64_t>(32 * m, 1));
   ns = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(ns, max_by_len), std::min<int64_t>(max_by_mem, 4096)));
   int64_t eps = (c->n + ns - 1) / ns;
@@ -214,6 +224,8 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, bool allow_r2) {
   if (eps < 32) eps = 32;
   s.elems_per_split = eps;
   s.nsplit = (int)std::max<int64_t>(1, (c->n + eps - 1) / eps);
+  s.nitems = s.ntiles * s.nsplit;
+  s.grid = (int)std::min<int64_t>(c->num_sms, (s.nitems + kWarpsPerCta - 1) / kWarpsPerCta);
   return s;
 }
 
@@ -221,8 +233,7 @@ template <typename T, int R>
 int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<T>();
   CUDA_TRY(cudaFuncSetAttribute(eval_fixed_kernel<T, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid((unsigned)sp.ctas_x, (unsigned)sp.nsplit);
-  eval_fixed_kernel<T, R><<<grid, kThreads, smem, c->stream>>>(fp);
+  eval_fixed_kernel<T, R><<<sp.grid, kThreads, smem, c->stream>>>(fp);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
@@ -232,8 +243,7 @@ template <int R>
 int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<double>();
   CUDA_TRY(cudaFuncSetAttribute(eval_adaptive_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  dim3 grid((unsigned)sp.ctas_x, (unsigned)sp.nsplit);
-  eval_adaptive_kernel<R><<<grid, kThreads, smem, c->stream>>>(ap);
+  eval_adaptive_kernel<R><<<sp.grid, kThreads, smem, c->stream>>>(ap);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
@@ -338,7 +348,7 @@ int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream) {
   c->num_sms = prop.multiProcessorCount;
   int rc = upload_tables();
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_status, sizeof(GeomStatus)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
-  if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, 2 * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
+  if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, 4 * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
   if (rc != BEMCUB_OK) {
     bemcub_destroy(c);
     return rc;
@@ -469,7 +479,7 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     if ((rc = expand_level<float>(c, rule_id, sigma, c->pts32[rule_id]))) return rc;
   }
 
-  const SplitPlan sp = plan_splits(c, m, true);
+  const SplitPlan sp = plan_splits(c, m);
   if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
   mark(c, 1);
 
@@ -483,8 +493,13 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     fp.partial = (double4*)c->partial.ptr;
     fp.split_stride = m;
     fp.ntiles = sp.ntiles;
-    if (precision == BEMCUB_F64) rc = sp.R == 2 ? launch_fixed<double, 2>(c, fp, sp) : launch_fixed<double, 1>(c, fp, sp);
-    else rc = sp.R == 2 ? launch_fixed<float, 2>(c, fp, sp) : launch_fixed<float, 1>(c, fp, sp);
+    fp.nitems = sp.nitems;
+    fp.queue = c->d_counters + 2;
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    if (precision == BEMCUB_F64)
+      rc = sp.R == 4 ? launch_fixed<double, 4>(c, fp, sp) : sp.R == 2 ? launch_fixed<double, 2>(c, fp, sp) : launch_fixed<double, 1>(c, fp, sp);
+    else
+      rc = sp.R == 4 ? launch_fixed<float, 4>(c, fp, sp) : sp.R == 2 ? launch_fixed<float, 2>(c, fp, sp) : launch_fixed<float, 1>(c, fp, sp);
     if (rc) return rc;
     // point-charge interactions of a fixed rule: every element's own N at every field point
     c->stats.point_interactions =
@@ -509,9 +524,11 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     ap.partial = (double4*)c->partial.ptr;
     ap.split_stride = m;
     ap.ntiles = sp.ntiles;
+    ap.nitems = sp.nitems;
+    ap.queue = c->d_counters + 2;
     ap.counters = c->d_counters;
-    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 2 * sizeof(unsigned long long), c->stream));
-    rc = sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    rc = sp.R == 4 ? launch_adaptive<4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
     if (rc) return rc;
     c->counters_pending = true;
   }
@@ -566,9 +583,9 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   const int64_t coltiles = (c->n + 31) / 32, rowtiles = (nrows + 31) / 32;
   // rows on grid.x would exceed no limit either way; y is limited to 65535 tiles = 2.1 M rows per call
   if (rowtiles > 65535) return BEMCUB_ERR_INVALID_ARG;
-  dim3 grid((unsigned)((coltiles + kWarpsPerCta - 1) / kWarpsPerCta), (unsigned)rowtiles);
+  dim3 grid((unsigned)((coltiles + kAsmWarps - 1) / kAsmWarps), (unsigned)rowtiles);
   mark(c, 1);
-  assemble_kernel<<<grid, kThreads, assemble_smem_bytes(), c->stream>>>(ap);
+  assemble_kernel<<<grid, kAsmThreads, assemble_smem_bytes(), c->stream>>>(ap);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   mark(c, 2);

@@ -29,8 +29,10 @@ struct AssembleParams {
   unsigned long long* counters;
 };
 
+constexpr int kAsmWarps = 8;
+constexpr int kAsmThreads = kAsmWarps * 32;
 constexpr int kTilePad = 33;
-constexpr size_t assemble_smem_bytes() { return (size_t)kWarpsPerCta * 32 * kTilePad * sizeof(double); }
+constexpr size_t assemble_smem_bytes() { return (size_t)kAsmWarps * 32 * kTilePad * sizeof(double); }
 
 // Potential-only term of Eq. 4.1: 12 FP64-pipe instructions (3 DADD + 3 DMUL + 6 DFMA).
 __device__ __forceinline__ double phi_one(const double4 s, double q, double px, double py, double pz, double acc) {
@@ -39,10 +41,10 @@ __device__ __forceinline__ double phi_one(const double4 s, double q, double px, 
   return __fma_rn(q, rsqrt_f64(r2), acc);
 }
 
-__global__ void __launch_bounds__(kThreads, 2) assemble_kernel(const __grid_constant__ AssembleParams p) {
+__global__ void __launch_bounds__(kAsmThreads, 2) assemble_kernel(const __grid_constant__ AssembleParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t ct = (int64_t)blockIdx.x * kWarpsPerCta + warp;  // column tile
+  const int64_t ct = (int64_t)blockIdx.x * kAsmWarps + warp;  // column tile
   const int64_t j0 = ct * 32;
   if (j0 >= p.n) return;
   const int64_t r0 = (int64_t)blockIdx.y * 32;  // first row of the tile, relative to row0

@@ -2,14 +2,19 @@
 // at many field points, with either one fixed rule or the distance-ratio
 // choice of Sec. 4 (L159).
 //
-// Execution model (both kernels): every WARP is an autonomous worker.  It owns 32*R field points
-// in registers (lane l holds points tile*32R + r*32 + l, r < R), walks one contiguous range of
-// elements ("split") and streams the packed (x,y,z,q) point records of those elements through its
-// private double-buffered shared-memory window, filled by 1-D bulk TMA copies
-// (cp.async.bulk -> UBLKCP) that complete on a per-warp mbarrier.  There is no __syncthreads in
-// the loop.  The inner loop reads one point with two broadcast LDS.128 and applies it to the R
+// Execution model (both kernels): PERSISTENT grid, one CTA of 12 warps per SM, every WARP an
+// autonomous worker that pulls work items from a global atomic queue until it is empty.  One item
+// = (tile of 32*R field points) x (one contiguous range of elements, a "split").  The warp keeps
+// its 32*R field points in registers (lane l holds points tile*32R + r*32 + l, r < R) and streams
+// the packed (x,y,z,q) point records of the split through its private double-buffered shared-memory
+// window, filled by 1-D bulk TMA copies (cp.async.bulk -> UBLKCP) that complete on a per-warp
+// mbarrier.  There is no __syncthreads anywhere: warps never wait for each other, so a tile that
+// needs high-order rules (more points) delays nobody, and the tail of the launch is at most one
+// item long.  The inner loop reads one point with two broadcast LDS.128 and applies it to the R
 // field points of each lane: 18 FP64-pipe instructions per point-charge interaction
-// (4 DADD + 6 DMUL + 8 DFMA = 26 flop) plus one MUFU.RSQ64H.
+// (4 DADD + 6 DMUL + 8 DFMA = 26 flop) plus one MUFU.RSQ64H.  R = 4 gives four independent
+// dependency chains per lane; with 3 warps per scheduler that saturates the FP64 pipe (measured
+// with the bare loop: 101-103 % of the DFMA-only rate at R = 4, 97 % at R = 2).
 //
 // Adaptive kernel: per batch of 32 elements each lane classifies ONE element against the bounding
 // sphere of the warp's field points (conservative in both directions), so the rule of an element
@@ -25,14 +30,31 @@
 
 namespace bemcub {
 
-constexpr int kWarpsPerCta = 8;
+constexpr int kWarpsPerCta = 12;  // 1 CTA per SM, 3 warps per scheduler, <= 168 registers per thread
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kBuf = 128;  // points per stage of a warp's window
 constexpr int kStages = 2;
 
+// Per-warp bookkeeping kept in shared memory (not registers): bounding sphere of the current tile
+// and the interaction tallies.
+struct WarpScratch {
+  double cx, cy, cz, rho, mag;
+  unsigned long long n_inter, n_ana;
+  int nvalid, pad;
+};
+
+// shared memory of one CTA: [warps][stages][kBuf] points | [warps][stages] mbarriers | [warps] scratch
 template <typename T>
 constexpr size_t eval_smem_bytes() {
-  return (size_t)kWarpsPerCta * kStages * kBuf * sizeof(typename Point4<T>::type) + (size_t)kWarpsPerCta * kStages * 8;
+  return (size_t)kWarpsPerCta * kStages * kBuf * sizeof(typename Point4<T>::type) + (size_t)kWarpsPerCta * kStages * 8 +
+         (size_t)kWarpsPerCta * sizeof(WarpScratch);
+}
+
+// Next work item of the persistent loop (lane 0 pulls, the warp shares it).
+__device__ __forceinline__ int64_t next_item(unsigned long long* queue, int lane) {
+  unsigned long long it = 0;
+  if (lane == 0) it = atomicAdd(queue, 1ull);
+  return (int64_t)__shfl_sync(kFullMask, it, 0);
 }
 
 template <typename T, int R>
@@ -78,19 +100,23 @@ __device__ __forceinline__ void interact(const P4 s, const T (&px)[R], const T (
   for (int r = 0; r < R; ++r) interact_one(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], a.ex[r], a.ey[r], a.ez[r]);
 }
 
-// All `cnt` points of a filled window applied to the warp's field points.
+// All `cnt` points of a filled window applied to the warp's field points, U points per trip so
+// that a lane always has >= 4 independent interaction chains in flight.
 template <typename T, int R, typename P4>
 __device__ __forceinline__ void consume(const P4* __restrict__ buf, int cnt, const T (&px)[R], const T (&py)[R],
                                         const T (&pz)[R], Accum<T, R>& a) {
+  constexpr int U = R >= 4 ? 1 : (R >= 2 ? 2 : 4);
   int i = 0;
 #pragma unroll 1
-  for (; i + 2 <= cnt; i += 2) {
-    const P4 s0 = buf[i];
-    const P4 s1 = buf[i + 1];
-    interact<T, R>(s0, px, py, pz, a);
-    interact<T, R>(s1, px, py, pz, a);
+  for (; i + U <= cnt; i += U) {
+    P4 s[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) s[u] = buf[i + u];
+#pragma unroll
+    for (int u = 0; u < U; ++u) interact<T, R>(s[u], px, py, pz, a);
   }
-  if (i < cnt) interact<T, R>(buf[i], px, py, pz, a);
+#pragma unroll 1
+  for (; i < cnt; ++i) interact<T, R>(buf[i], px, py, pz, a);
 }
 
 // FP64: the window's sum goes straight into the running totals.  FP32: the window (<= kBuf
@@ -139,6 +165,34 @@ __device__ __forceinline__ void store_partial(double4* __restrict__ partial, int
 }
 
 // ------------------------------------------------------------------------------------------------
+// Shared-memory carve-up of the calling warp.
+template <typename P4>
+struct WarpSmem {
+  P4* win;           // [kStages][kBuf]
+  uint32_t win0;     // shared-space address of win
+  uint32_t bar0;     // shared-space address of the first of kStages mbarriers (8 bytes apart)
+  WarpScratch* scr;
+};
+template <typename P4>
+__device__ __forceinline__ WarpSmem<P4> warp_smem(unsigned char* smem_raw, int warp, int lane) {
+  WarpSmem<P4> w;
+  w.win = reinterpret_cast<P4*>(smem_raw) + (size_t)warp * kStages * kBuf;
+  unsigned char* after = smem_raw + (size_t)kWarpsPerCta * kStages * kBuf * sizeof(P4);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(after) + warp * kStages;
+  w.scr = reinterpret_cast<WarpScratch*>(after + (size_t)kWarpsPerCta * kStages * 8) + warp;
+  w.win0 = smem_u32(w.win);
+  w.bar0 = smem_u32(bars);
+  if (lane == 0) {
+    mbar_init(w.bar0, 1);
+    mbar_init(w.bar0 + 8, 1);
+    mbar_fence_init();
+    w.scr->n_inter = 0;
+    w.scr->n_ana = 0;
+  }
+  __syncwarp();
+  return w;
+}
+
 struct FixedParams {
   const void* pts;          // Point4<T>[npts], one rule level
   int64_t npts;             // n * stride
@@ -148,57 +202,52 @@ struct FixedParams {
   double4* partial;         // [nsplit][split_stride]
   int64_t split_stride;
   int64_t ntiles;           // ceil(m / (32 R))
+  int64_t nitems;           // ntiles * nsplit; item = split * ntiles + tile
+  unsigned long long* queue;  // work-item counter, zeroed before the launch
 };
 
 template <typename T, int R>
-__global__ void __launch_bounds__(kThreads, 2) eval_fixed_kernel(const __grid_constant__ FixedParams p) {
+__global__ void __launch_bounds__(kThreads, 1) eval_fixed_kernel(const __grid_constant__ FixedParams p) {
   typedef typename Point4<T>::type P4;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + warp;
-  if (tile >= p.ntiles) return;  // whole warp; no block-level barrier is ever used
-
-  P4* win = reinterpret_cast<P4*>(smem_raw) + (size_t)warp * kStages * kBuf;
-  uint64_t* bars =
-      reinterpret_cast<uint64_t*>(smem_raw + (size_t)kWarpsPerCta * kStages * kBuf * sizeof(P4)) + warp * kStages;
-  const uint32_t bar0 = smem_u32(bars), win0 = smem_u32(win);
-  if (lane == 0) {
-    mbar_init(bar0, 1);
-    mbar_init(bar0 + 8, 1);
-    mbar_fence_init();
-  }
-  __syncwarp();
-
-  T px[R], py[R], pz[R];
-  load_field_points<T, R>(p.field, p.m, tile, lane, px, py, pz);
-
-  const int64_t q0 = (int64_t)blockIdx.y * p.pts_per_split;
-  const int64_t q1 = min(p.npts, q0 + p.pts_per_split);
+  const WarpSmem<P4> ws = warp_smem<P4>(smem_raw, warp, lane);
   const P4* src = reinterpret_cast<const P4*>(p.pts);
-  const int64_t nchunks = (q1 - q0 + kBuf - 1) / kBuf;
+  uint32_t phases = 0;  // parity of each stage's mbarrier, carried across items
 
-  Accum<double, R> tot;
-  tot.zero();
-  auto fill = [&](int64_t c, int stage) {
-    if (lane == 0) {
-      const int64_t a = q0 + c * kBuf;
-      const uint32_t bytes = (uint32_t)(min((int64_t)kBuf, q1 - a) * sizeof(P4));
-      mbar_arrive_expect_tx(bar0 + 8 * stage, bytes);
-      tma_load_1d(win0 + stage * (uint32_t)(kBuf * sizeof(P4)), src + a, bytes, bar0 + 8 * stage);
+  for (;;) {
+    const int64_t item = next_item(p.queue, lane);
+    if (item >= p.nitems) break;
+    const int64_t split = item / p.ntiles, tile = item - split * p.ntiles;
+
+    T px[R], py[R], pz[R];
+    load_field_points<T, R>(p.field, p.m, tile, lane, px, py, pz);
+    const int64_t q0 = split * p.pts_per_split;
+    const int64_t q1 = min(p.npts, q0 + p.pts_per_split);
+    const int64_t nchunks = (q1 - q0 + kBuf - 1) / kBuf;
+
+    Accum<double, R> tot;
+    tot.zero();
+    auto fill = [&](int64_t c, int stage) {
+      if (lane == 0) {
+        const int64_t a = q0 + c * kBuf;
+        const uint32_t bytes = (uint32_t)(min((int64_t)kBuf, q1 - a) * sizeof(P4));
+        mbar_arrive_expect_tx(ws.bar0 + 8 * stage, bytes);
+        tma_load_1d(ws.win0 + stage * (uint32_t)(kBuf * sizeof(P4)), src + a, bytes, ws.bar0 + 8 * stage);
+      }
+    };
+    if (nchunks > 0) fill(0, 0);
+    for (int64_t c = 0; c < nchunks; ++c) {
+      const int stage = (int)(c & 1);
+      if (c + 1 < nchunks) fill(c + 1, stage ^ 1);
+      mbar_wait(ws.bar0 + 8 * stage, (phases >> stage) & 1u);
+      phases ^= 1u << stage;
+      const int cnt = (int)min((int64_t)kBuf, q1 - (q0 + c * kBuf));
+      consume_into<R>(ws.win + stage * kBuf, cnt, px, py, pz, tot);
+      __syncwarp();  // every lane is done with this stage before it is refilled
     }
-  };
-  if (nchunks > 0) fill(0, 0);
-  uint32_t phases = 0;
-  for (int64_t c = 0; c < nchunks; ++c) {
-    const int stage = (int)(c & 1);
-    if (c + 1 < nchunks) fill(c + 1, stage ^ 1);
-    mbar_wait(bar0 + 8 * stage, (phases >> stage) & 1u);
-    phases ^= 1u << stage;
-    const int cnt = (int)min((int64_t)kBuf, q1 - (q0 + c * kBuf));
-    consume_into<R>(win + stage * kBuf, cnt, px, py, pz, tot);
-    __syncwarp();  // every lane is done with this stage before it is refilled
+    store_partial<R>(p.partial + split * p.split_stride, p.m, tile, lane, tot);
   }
-  store_partial<R>(p.partial + (int64_t)blockIdx.y * p.split_stride, p.m, tile, lane, tot);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -241,18 +290,23 @@ struct AdaptiveParams {
   double4* partial;
   int64_t split_stride;
   int64_t ntiles;
+  int64_t nitems;
+  unsigned long long* queue;
   unsigned long long* counters;  // [0] point-charge interactions, [1] analytic pairs
 };
 
+// Field points of the warp's current tile.
 template <int R>
 struct WarpTile {
   double px[R], py[R], pz[R];
-  bool ok[R];  // field point exists (not a clamped duplicate)
-  double cx, cy, cz, rho, mag;  // bounding sphere of the tile, coordinate magnitude
-  int nvalid;                   // field points of this tile that exist
+  int64_t first;  // index of the tile's first field point
+  int64_t m;
+  __device__ __forceinline__ bool ok(int r, int lane) const { return first + r * 32 + lane < m; }
 };
 
-// Element `e` evaluated analytically at every field point of the tile (a4).
+__device__ __forceinline__ int warp_sum(int v) { return __reduce_add_sync(kFullMask, v); }
+
+// Element `e` evaluated analytically at the field points of the tile selected by `take` (a4).
 template <int R>
 __device__ __forceinline__ void analytic_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, const bool (&take)[R],
                                               Accum<double, R>& tot) {
@@ -272,10 +326,11 @@ __device__ __forceinline__ void analytic_element(const AdaptiveParams& p, int64_
   }
 }
 
-// Element `e` with the exact per-pair rule choice (tile straddles a band limit, allow_upgrade = 0).
+// Element `e` with the exact per-pair rule choice (tile straddles a band limit and the policy
+// does not allow, or the analytic limit forbids, an upgrade).
 template <int R>
-__device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, Accum<double, R>& tot,
-                                           unsigned long long& n_inter, unsigned long long& n_ana) {
+__device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, int lane,
+                                           Accum<double, R>& tot, WarpScratch* scr) {
   const double4 c = ldg4(p.cenL + e);
   const int t = __ldg(p.type + e);
   int lev[R];
@@ -293,199 +348,200 @@ __device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e
     for (int r = 0; r < R; ++r) {
       take[r] = (lev[r] == l);
       any |= take[r];
-      mine += (take[r] && w.ok[r]) ? 1 : 0;
+      mine += (take[r] && w.ok(r, lane)) ? 1 : 0;
     }
     if (!__any_sync(kFullMask, any)) continue;
+    const int all = warp_sum(mine);
     if (l == 5) {
       analytic_element<R>(p, e, w, take, tot);
-      n_ana += mine;
+      if (lane == 0) scr->n_ana += (unsigned long long)all;
     } else {
       const int N = rule_npts(t, l);
       const double4* src = p.lvl_pts[l] + e * p.stride[l];
+      double4 s = ldg4(src);
+#pragma unroll 1
       for (int i = 0; i < N; ++i) {
-        const double4 s = ldg4(src + i);
+        const double4 nxt = ldg4(src + min(i + 1, N - 1));  // prefetch: hides the global-load latency
 #pragma unroll
         for (int r = 0; r < R; ++r)
           interact_one(s.x, s.y, s.z, take[r] ? s.w : 0.0, w.px[r], w.py[r], w.pz[r], tot.phi[r], tot.ex[r], tot.ey[r],
                        tot.ez[r]);
+        s = nxt;
       }
-      n_inter += (unsigned long long)mine * N;
+      if (lane == 0) scr->n_inter += (unsigned long long)all * N;
     }
   }
 }
 
 template <int R>
-__global__ void __launch_bounds__(kThreads, 2) eval_adaptive_kernel(const __grid_constant__ AdaptiveParams p) {
+__global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid_constant__ AdaptiveParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + warp;
-  if (tile >= p.ntiles) return;
-
-  double4* win = reinterpret_cast<double4*>(smem_raw) + (size_t)warp * kStages * kBuf;
-  uint64_t* bars =
-      reinterpret_cast<uint64_t*>(smem_raw + (size_t)kWarpsPerCta * kStages * kBuf * sizeof(double4)) + warp * kStages;
-  const uint32_t bar0 = smem_u32(bars), win0 = smem_u32(win);
-  if (lane == 0) {
-    mbar_init(bar0, 1);
-    mbar_init(bar0 + 8, 1);
-    mbar_fence_init();
-  }
-  __syncwarp();
-
-  WarpTile<R> w;
-  load_field_points<double, R>(p.field, p.m, tile, lane, w.px, w.py, w.pz);
-  {
-    double lox = w.px[0], hix = w.px[0], loy = w.py[0], hiy = w.py[0], loz = w.pz[0], hiz = w.pz[0];
-    int cntok = 0;
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-      w.ok[r] = (tile * (32 * R) + r * 32 + lane) < p.m;
-      cntok += w.ok[r] ? 1 : 0;
-      lox = fmin(lox, w.px[r]); hix = fmax(hix, w.px[r]);
-      loy = fmin(loy, w.py[r]); hiy = fmax(hiy, w.py[r]);
-      loz = fmin(loz, w.pz[r]); hiz = fmax(hiz, w.pz[r]);
-    }
-    lox = warp_min(lox); hix = warp_max(hix);
-    loy = warp_min(loy); hiy = warp_max(hiy);
-    loz = warp_min(loz); hiz = warp_max(hiz);
-    w.cx = 0.5 * (lox + hix);
-    w.cy = 0.5 * (loy + hiy);
-    w.cz = 0.5 * (loz + hiz);
-    double d2 = 0.0;
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-      const double dx = w.px[r] - w.cx, dy = w.py[r] - w.cy, dz = w.pz[r] - w.cz;
-      d2 = fmax(d2, dx * dx + dy * dy + dz * dz);
-    }
-    w.rho = sqrt(warp_max(d2));
-    w.mag = fmax(fmax(fabs(w.cx), fabs(w.cy)), fabs(w.cz)) + w.rho;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) cntok += __shfl_xor_sync(kFullMask, cntok, o);
-    w.nvalid = cntok;
-  }
-
-  const int64_t e_begin = (int64_t)blockIdx.y * p.elems_per_split;
-  const int64_t e_end = min(p.n, e_begin + p.elems_per_split);
-
-  Accum<double, R> tot;
-  tot.zero();
-  unsigned long long n_inter = 0, n_ana = 0;  // per-lane tallies, summed at the end
-
-  // state of the current 32-element batch: lane l holds element batch0 + l
-  int64_t batch_next = e_begin;
-  int cnt = 0, pre = 0, total = 0, lvl = 0, cursor = 32;
-  const double4* src = nullptr;
-
-  // Fills `stage` with the next round of whole elements; returns the number of points (0 = done).
-  auto produce = [&](int stage) -> int {
-    for (;;) {
-      if (cursor < 32) {
-        const int base = __shfl_sync(kFullMask, pre, cursor);
-        const bool after = lane >= cursor;
-        const unsigned nofit = __ballot_sync(kFullMask, after && (pre + cnt - base > kBuf));
-        const int next = nofit ? (__ffs(nofit) - 1) : 32;
-        const int pre_next = __shfl_sync(kFullMask, pre, next & 31);
-        const int endp = (next < 32) ? pre_next : total;
-        const int nstage = endp - base;
-        const bool inc = after && lane < next && cnt > 0;
-        const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
-        const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
-        // a lane continues its predecessor's copy if that one ends exactly where this one starts
-        const bool cont = inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == p.stride[lvl];
-        const unsigned heads = __ballot_sync(kFullMask, inc && !cont);
-        const unsigned higher = heads & ~((2u << lane) - 1u);
-        const int h2 = higher ? (__ffs(higher) - 1) : 32;
-        const int pre_h2 = __shfl_sync(kFullMask, pre, h2 & 31);
-        const int run_end = (h2 < 32) ? pre_h2 : endp;
-        cursor = next;
-        if (nstage == 0) continue;
-        if (lane == 0) mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
-        __syncwarp();
-        if (inc && !cont)
-          tma_load_1d(win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
-                      (uint32_t)((run_end - pre) * sizeof(double4)), bar0 + 8 * stage);
-        if (lane == 0) n_inter += (unsigned long long)nstage * w.nvalid;
-        return nstage;
-      }
-      if (batch_next >= e_end) return 0;
-      // ---- a2: classify 32 elements, one per lane, against the tile's bounding sphere
-      const int64_t batch0 = batch_next;
-      const int64_t e = batch0 + lane;
-      batch_next += 32;
-      cnt = 0;
-      lvl = -1;
-      bool is_ana = false, is_mixed = false;
-      if (e < e_end) {
-        const double4 c = p.cenL[e];
-        const int t = p.type[e];
-        const double dx = w.cx - c.x, dy = w.cy - c.y, dz = w.cz - c.z;
-        const double Dc = sqrt(dx * dx + dy * dy + dz * dz);
-        const double slack =
-            1e-9 * (Dc + w.rho) + 1e-12 * (w.mag + fmax(fmax(fabs(c.x), fabs(c.y)), fabs(c.z)));
-        const double Dhi = Dc + w.rho + slack;
-        const double Dlo = fmax(Dc - w.rho - slack, 0.0);
-        const int lfar = p.pol.map[want_level(Dhi * Dhi, c.w, p.pol.dr[t])];
-        const int lnear = p.pol.map[want_level(Dlo * Dlo, c.w, p.pol.dr[t])];
-        // A tile that straddles a band limit: per-pair choice, or (allow_upgrade) the more accurate
-        // cubature rule for the whole tile.  The analytic formula is never an "upgrade": its
-        // rounding error grows with the distance ratio (Figs. 2-4), so a tile that
-        // straddles the analytic limit is always resolved pair by pair.
-        if (lnear != lfar && (!p.pol.allow_upgrade || lnear == 5)) {
-          is_mixed = true;
-        } else {
-          lvl = lnear;  // the more accurate end of the tile's range
-          if (lvl == 5) {
-            is_ana = true;
-          } else {
-            cnt = rule_npts(t, lvl);
-            src = p.lvl_pts[lvl] + e * p.stride[lvl];
-          }
-        }
-      }
-      pre = warp_excl_scan(cnt, lane, &total);
-      cursor = 0;
-      unsigned amask = __ballot_sync(kFullMask, is_ana), xmask = __ballot_sync(kFullMask, is_mixed);
-      while (amask) {
-        const int l = __ffs(amask) - 1;
-        amask &= amask - 1;
-        analytic_element<R>(p, batch0 + l, w, w.ok, tot);
-        if (lane == 0) n_ana += w.nvalid;
-      }
-      while (xmask) {
-        const int l = __ffs(xmask) - 1;
-        xmask &= xmask - 1;
-        mixed_element<R>(p, batch0 + l, w, tot, n_inter, n_ana);
-      }
-    }
-  };
-
-  // software pipeline with a single produce() call site: fill stage s^1, then consume stage s
-  int cur = 0, stage = 1;
+  const WarpSmem<double4> ws = warp_smem<double4>(smem_raw, warp, lane);
+  WarpScratch* const scr = ws.scr;
   uint32_t phases = 0;
+
   for (;;) {
-    const int nxt = produce(stage ^ 1);
-    if (cur > 0) {
-      mbar_wait(bar0 + 8 * stage, (phases >> stage) & 1u);
-      phases ^= 1u << stage;
-      consume_into<R>(win + stage * kBuf, cur, w.px, w.py, w.pz, tot);
+    const int64_t item = next_item(p.queue, lane);
+    if (item >= p.nitems) break;
+    const int64_t split = item / p.ntiles, tile = item - split * p.ntiles;
+
+    WarpTile<R> w;
+    w.first = tile * (32 * R);
+    w.m = p.m;
+    load_field_points<double, R>(p.field, p.m, tile, lane, w.px, w.py, w.pz);
+    {  // bounding sphere of the tile (clamped duplicates lie inside it by construction)
+      double lox = w.px[0], hix = w.px[0], loy = w.py[0], hiy = w.py[0], loz = w.pz[0], hiz = w.pz[0];
+      int cntok = 0;
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        cntok += w.ok(r, lane) ? 1 : 0;
+        lox = fmin(lox, w.px[r]); hix = fmax(hix, w.px[r]);
+        loy = fmin(loy, w.py[r]); hiy = fmax(hiy, w.py[r]);
+        loz = fmin(loz, w.pz[r]); hiz = fmax(hiz, w.pz[r]);
+      }
+      lox = warp_min(lox); hix = warp_max(hix);
+      loy = warp_min(loy); hiy = warp_max(hiy);
+      loz = warp_min(loz); hiz = warp_max(hiz);
+      const double cx = 0.5 * (lox + hix), cy = 0.5 * (loy + hiy), cz = 0.5 * (loz + hiz);
+      double d2 = 0.0;
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const double dx = w.px[r] - cx, dy = w.py[r] - cy, dz = w.pz[r] - cz;
+        d2 = fmax(d2, dx * dx + dy * dy + dz * dz);
+      }
+      const double rho = sqrt(warp_max(d2));
+      cntok = warp_sum(cntok);
+      __syncwarp();
+      if (lane == 0) {
+        scr->cx = cx; scr->cy = cy; scr->cz = cz; scr->rho = rho;
+        scr->mag = fmax(fmax(fabs(cx), fabs(cy)), fabs(cz)) + rho;
+        scr->nvalid = cntok;
+      }
       __syncwarp();
     }
-    if (nxt == 0) break;
-    stage ^= 1;
-    cur = nxt;
-  }
-  store_partial<R>(p.partial + (int64_t)blockIdx.y * p.split_stride, p.m, tile, lane, tot);
 
-  if (p.counters) {
+    const int64_t e_begin = split * p.elems_per_split;
+    const int64_t e_end = min(p.n, e_begin + p.elems_per_split);
+
+    Accum<double, R> tot;
+    tot.zero();
+
+    // state of the current 32-element batch: lane l holds element batch0 + l
+    int64_t batch_next = e_begin;
+    int cnt = 0, pre = 0, total = 0, lvl = 0, cursor = 32;
+    const double4* src = nullptr;
+
+    // Fills `stage` with the next round of whole elements; returns the number of points (0 = done).
+    auto produce = [&](int stage) -> int {
+      for (;;) {
+        if (cursor < 32) {
+          const int base = __shfl_sync(kFullMask, pre, cursor);
+          const bool after = lane >= cursor;
+          const unsigned nofit = __ballot_sync(kFullMask, after && (pre + cnt - base > kBuf));
+          const int next = nofit ? (__ffs(nofit) - 1) : 32;
+          const int pre_next = __shfl_sync(kFullMask, pre, next & 31);
+          const int endp = (next < 32) ? pre_next : total;
+          const int nstage = endp - base;
+          const bool inc = after && lane < next && cnt > 0;
+          const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
+          const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
+          // a lane continues its predecessor's copy if that one ends exactly where this one starts
+          const bool cont = inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == p.stride[lvl];
+          const unsigned heads = __ballot_sync(kFullMask, inc && !cont);
+          const unsigned higher = heads & ~((2u << lane) - 1u);
+          const int h2 = higher ? (__ffs(higher) - 1) : 32;
+          const int pre_h2 = __shfl_sync(kFullMask, pre, h2 & 31);
+          const int run_end = (h2 < 32) ? pre_h2 : endp;
+          cursor = next;
+          if (nstage == 0) continue;
+          if (lane == 0) mbar_arrive_expect_tx(ws.bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
+          __syncwarp();
+          if (inc && !cont)
+            tma_load_1d(ws.win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
+                        (uint32_t)((run_end - pre) * sizeof(double4)), ws.bar0 + 8 * stage);
+          if (lane == 0) scr->n_inter += (unsigned long long)nstage * scr->nvalid;
+          return nstage;
+        }
+        if (batch_next >= e_end) return 0;
+        // ---- a2: classify 32 elements, one per lane, against the tile's bounding sphere
+        const int64_t batch0 = batch_next;
+        const int64_t e = batch0 + lane;
+        batch_next += 32;
+        cnt = 0;
+        lvl = -1;
+        bool is_ana = false, is_mixed = false;
+        if (e < e_end) {
+          const double4 c = p.cenL[e];
+          const int t = p.type[e];
+          const double rho = scr->rho;
+          const double dx = scr->cx - c.x, dy = scr->cy - c.y, dz = scr->cz - c.z;
+          const double Dc = sqrt(dx * dx + dy * dy + dz * dz);
+          const double slack =
+              1e-9 * (Dc + rho) + 1e-12 * (scr->mag + fmax(fmax(fabs(c.x), fabs(c.y)), fabs(c.z)));
+          const double Dhi = Dc + rho + slack;
+          const double Dlo = fmax(Dc - rho - slack, 0.0);
+          const int lfar = p.pol.map[want_level(Dhi * Dhi, c.w, p.pol.dr[t])];
+          const int lnear = p.pol.map[want_level(Dlo * Dlo, c.w, p.pol.dr[t])];
+          // A tile that straddles a band limit: per-pair choice, or (allow_upgrade) the more accurate
+          // cubature rule for the whole tile.  The analytic formula is never an "upgrade": its
+          // rounding error grows with the distance ratio (Figs. 2-4), so a tile that
+          // straddles the analytic limit is always resolved pair by pair.
+          if (lnear != lfar && (!p.pol.allow_upgrade || lnear == 5)) {
+            is_mixed = true;
+          } else {
+            lvl = lnear;  // the more accurate end of the tile's range
+            if (lvl == 5) {
+              is_ana = true;
+            } else {
+              cnt = rule_npts(t, lvl);
+              src = p.lvl_pts[lvl] + e * p.stride[lvl];
+            }
+          }
+        }
+        pre = warp_excl_scan(cnt, lane, &total);
+        cursor = 0;
+        unsigned amask = __ballot_sync(kFullMask, is_ana), xmask = __ballot_sync(kFullMask, is_mixed);
+        if (amask) {
+          bool all_ok[R];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      n_inter += __shfl_xor_sync(kFullMask, n_inter, o);
-      n_ana += __shfl_xor_sync(kFullMask, n_ana, o);
+          for (int r = 0; r < R; ++r) all_ok[r] = w.ok(r, lane);
+          if (lane == 0) scr->n_ana += (unsigned long long)__popc(amask) * scr->nvalid;
+          while (amask) {
+            const int l = __ffs(amask) - 1;
+            amask &= amask - 1;
+            analytic_element<R>(p, batch0 + l, w, all_ok, tot);
+          }
+        }
+        while (xmask) {
+          const int l = __ffs(xmask) - 1;
+          xmask &= xmask - 1;
+          mixed_element<R>(p, batch0 + l, w, lane, tot, scr);
+        }
+      }
+    };
+
+    // software pipeline with a single produce() call site: fill stage s^1, then consume stage s
+    int cur = 0, stage = 1;
+    for (;;) {
+      const int nxt = produce(stage ^ 1);
+      if (cur > 0) {
+        mbar_wait(ws.bar0 + 8 * stage, (phases >> stage) & 1u);
+        phases ^= 1u << stage;
+        consume_into<R>(ws.win + stage * kBuf, cur, w.px, w.py, w.pz, tot);
+        __syncwarp();
+      }
+      if (nxt == 0) break;
+      stage ^= 1;
+      cur = nxt;
     }
-    if (lane == 0) {
-      atomicAdd(p.counters, n_inter);
-      if (n_ana) atomicAdd(p.counters + 1, n_ana);
-    }
+    store_partial<R>(p.partial + split * p.split_stride, p.m, tile, lane, tot);
+  }
+
+  __syncwarp();
+  if (p.counters && lane == 0) {
+    if (scr->n_inter) atomicAdd(p.counters, scr->n_inter);
+    if (scr->n_ana) atomicAdd(p.counters + 1, scr->n_ana);
   }
 }
 

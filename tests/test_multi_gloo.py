@@ -1,0 +1,95 @@
+"""N > 1 path on the CPU: world_size-2 `gloo` processes exercise the host-side sharding logic
+(SURVEY.md §8(e)): field points / matrix rows are split by `multi.my_range`, every rank evaluates its
+own range against the full mesh, there is no data-path collective, and the gathered result equals
+the single-process one.  The per-rank evaluation is done by the CPU oracle here (no GPU in this
+tier of the tests); on a GPU box each rank calls bemcub_eval / bemcub_assemble_rows on its range
+exactly the same way (bench.py)."""
+from __future__ import annotations
+
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank: int, ws: int, port: int, q):
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+
+    import oracle
+    from paper_1606_03743_b200 import multi, synth
+
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=ws)
+    try:
+        c = synth.config1(level=1, m=101)          # 80 triangles, 101 field points: ragged split 51 / 50
+        lo, hi = multi.my_range(len(c["pts"]))
+        ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][lo:hi], 1)
+        local = torch.as_tensor(np.concatenate([ref["phi"][:, None], ref["E"]], axis=1))
+        full = multi.gather_rows(local, len(c["pts"]))
+        # matrix rows shard the same way
+        n = len(c["etype"])
+        rlo, rhi = multi.my_range(n)
+        rows, _ = oracle.assemble_rows(c["etype"], c["verts"], np.arange(rlo, rhi), oracle.default_policy(False))
+        mat = multi.gather_rows(torch.as_tensor(rows), n)
+        t = multi.max_over_ranks(10.0 + rank)
+        u = multi.sum_over_ranks(float(hi - lo))
+        dist.barrier()
+        if rank == 0:
+            q.put((lo, hi, full.numpy(), mat.numpy(), t, u))
+        else:
+            assert full is None and mat is None
+            q.put((lo, hi, None, None, t, u))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_shard_range_covers_everything():
+    from paper_1606_03743_b200 import synth
+    for total in (0, 1, 7, 100, 1_000_003):
+        for ws in (1, 2, 3, 8):
+            edges = [synth.shard_range(total, r, ws) for r in range(ws)]
+            assert edges[0][0] == 0 and edges[-1][1] == total
+            assert all(a[1] == b[0] for a, b in zip(edges, edges[1:]))
+            sizes = [hi - lo for lo, hi in edges]
+            assert max(sizes) - min(sizes) <= 1
+
+
+@pytest.mark.timeout(180)
+def test_two_rank_gloo_field_point_and_row_sharding():
+    import torch.multiprocessing as mp
+
+    import oracle
+    from paper_1606_03743_b200 import synth
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = [q.get(timeout=150) for _ in procs]
+    for p in procs:
+        p.join(timeout=30)
+        assert p.exitcode == 0
+    got.sort(key=lambda g: g[0])
+    (lo0, hi0, full, mat, t0, u0), (lo1, hi1, _, _, t1, u1) = got
+    assert (lo0, hi0, lo1, hi1) == (0, 51, 51, 101)
+    assert t0 == t1 == 11.0                 # max over ranks
+    assert u0 == u1 == 101.0                # whole-job units
+    c = synth.config1(level=1, m=101)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], 1)
+    # per-point results do not depend on how the points were sharded: bit-identical
+    assert np.array_equal(full[:, 0], ref["phi"]) and np.array_equal(full[:, 1:], ref["E"])
+    rows, _ = oracle.assemble_rows(c["etype"], c["verts"], np.arange(len(c["etype"])), oracle.default_policy(False))
+    assert np.array_equal(mat, rows)
