@@ -13,6 +13,7 @@
 #include "kernels_assemble.cuh"
 #include "kernels_eval.cuh"
 #include "kernels_pre.cuh"
+#include "kernels_sort.cuh"
 #include "rules.h"
 
 using namespace bemcub;
@@ -47,6 +48,7 @@ struct bemcub_ctx {
   int stride[5] = {4, 7, 12, 19, 33};
   // scratch
   DevBuf partial;
+  DevBuf sort_key[2], sort_idx[2], sort_hist, sort_pts, sort_box;  // a2: Morton order of the field points
   DevBuf host_stage[5];  // device copies of host inputs/outputs for the *_host entry points
   unsigned long long* d_counters = nullptr;
   bemcub_stats stats{};
@@ -249,6 +251,45 @@ int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp
   return BEMCUB_OK;
 }
 
+// a2 (first half): Morton order of the field points.  On success *perm is the device array with
+// perm[j] = caller index of the j-th point in evaluation order and *sorted the permuted points.
+int sort_field_points(bemcub_ctx* c, int64_t m, const double* field, const uint32_t** perm, const double** sorted) {
+  int rc;
+  const int nblocks = (int)((m + kSortChunk - 1) / kSortChunk);
+  const size_t hist_entries = (size_t)kRadix * nblocks;
+  for (int i = 0; i < 2; ++i)
+    if ((rc = ensure(c->sort_key[i], (size_t)m * 4)) || (rc = ensure(c->sort_idx[i], (size_t)m * 4))) return rc;
+  if ((rc = ensure(c->sort_hist, hist_entries * 4)) || (rc = ensure(c->sort_pts, (size_t)m * 24)) ||
+      (rc = ensure(c->sort_box, 6 * sizeof(unsigned long long))))
+    return rc;
+  unsigned long long* box = (unsigned long long*)c->sort_box.ptr;
+  CUDA_TRY(cudaMemsetAsync(box, 0xff, 3 * sizeof(unsigned long long), c->stream));
+  CUDA_TRY(cudaMemsetAsync(box + 3, 0x00, 3 * sizeof(unsigned long long), c->stream));
+  const int threads = 256;
+  const unsigned mblocks = (unsigned)((m + threads - 1) / threads);
+  bbox_kernel<<<std::min<unsigned>(mblocks, (unsigned)c->num_sms * 8), threads, 0, c->stream>>>(m, field, box);
+  uint32_t* key[2] = {(uint32_t*)c->sort_key[0].ptr, (uint32_t*)c->sort_key[1].ptr};
+  uint32_t* idx[2] = {(uint32_t*)c->sort_idx[0].ptr, (uint32_t*)c->sort_idx[1].ptr};
+  morton_key_kernel<<<mblocks, threads, 0, c->stream>>>(m, field, box, key[0], idx[0]);
+  count_launch(c, 2);
+  int cur = 0;
+  for (int shift = 0; shift < 30; shift += kRadixBits) {
+    uint32_t* hist = (uint32_t*)c->sort_hist.ptr;
+    radix_hist_kernel<<<nblocks, 32, 0, c->stream>>>(m, key[cur], shift, nblocks, hist);
+    radix_scan_kernel<<<1, 1024, 0, c->stream>>>((int64_t)hist_entries, hist);
+    radix_scatter_kernel<<<nblocks, 32, 0, c->stream>>>(m, key[cur], idx[cur], shift, nblocks, hist, key[cur ^ 1],
+                                                        idx[cur ^ 1]);
+    count_launch(c, 3);
+    cur ^= 1;
+  }
+  gather_points_kernel<<<mblocks, threads, 0, c->stream>>>(m, field, idx[cur], (double*)c->sort_pts.ptr);
+  count_launch(c);
+  CUDA_TRY(cudaGetLastError());
+  *perm = idx[cur];
+  *sorted = (const double*)c->sort_pts.ptr;
+  return BEMCUB_OK;
+}
+
 // ev[0] call start, ev[1] before the dominant kernel, ev[2] after it, ev[3] call end
 void mark(bemcub_ctx* c, int i) {
   if (c->timing) cudaEventRecord(c->ev[i], c->stream);
@@ -363,6 +404,8 @@ int bemcub_destroy(bemcub_ctx* c) {
   cudaStreamSynchronize(c->stream);
   release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial);
   for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); }
+  for (int i = 0; i < 2; ++i) { release(c->sort_key[i]); release(c->sort_idx[i]); }
+  release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
   if (c->d_status) cudaFree(c->d_status);
   if (c->d_counters) cudaFree(c->d_counters);
   for (int i = 0; i < 4; ++i)
@@ -481,6 +524,11 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
 
   const SplitPlan sp = plan_splits(c, m);
   if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
+  // a2: tiles of spatially close field points (adaptive mode; a fixed rule has nothing to choose)
+  const uint32_t* perm = nullptr;
+  if (adaptive && m > 32 && m < ((int64_t)1 << 31)) {
+    if ((rc = sort_field_points(c, m, field_pts, &perm, &field_pts))) return rc;
+  }
   mark(c, 1);
 
   if (!adaptive) {
@@ -537,7 +585,7 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   // a6: cross-split reduction and the 1/(4 pi eps0) prefactor
   const int threads = 256;
   reduce_scale_kernel<<<(unsigned)((m + threads - 1) / threads), threads, 0, c->stream>>>(
-      m, sp.nsplit, m, (const double4*)c->partial.ptr, coulomb_k(), out_phi, out_E);
+      m, sp.nsplit, m, (const double4*)c->partial.ptr, coulomb_k(), perm, out_phi, out_E);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   mark(c, 3);

@@ -128,10 +128,12 @@ __global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* _
 }
 
 // Step a6: sum the per-split partial results in split order and apply k = 1/(4 pi eps0) once
-// (Eq. 4.1 prefactor, L141).
+// (Eq. 4.1 prefactor, L141).  `perm` (may be null) maps the evaluation order back to the caller's
+// field-point order (kernels_sort.cuh).
 __global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride, const double4* __restrict__ partial,
-                                    double k, double* __restrict__ phi, double* __restrict__ E) {
-  const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+                                    double k, const uint32_t* __restrict__ perm, double* __restrict__ phi,
+                                    double* __restrict__ E) {
+  int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (j >= m) return;
   double4 s = partial[j];
   for (int sp = 1; sp < nsplit; ++sp) {
@@ -141,6 +143,7 @@ __global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride,
     s.z += p.z;
     s.w += p.w;
   }
+  if (perm) j = perm[j];
   if (phi) phi[j] = k * s.x;
   if (E) {
     E[3 * j] = k * s.y;
