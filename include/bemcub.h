@@ -158,9 +158,17 @@ int bemcub_expand_points(bemcub_ctx* ctx, const double* sigma, int rule_id, doub
 /* Centroid [n][3], area [n], L [n] of the current mesh (any pointer may be NULL).  Asynchronous. */
 int bemcub_get_geometry(bemcub_ctx* ctx, double* out_cen, double* out_area, double* out_L);
 
-/* Roofline denominator: runs a dependent-chain-free DFMA kernel on all SMs for about `seconds`
- * and returns the sustained rate in FP64 FMA/s (flop/s = 2x).  Synchronises. */
+/* Roofline denominator: runs a DFMA-only kernel (16 independent chains per thread; at 16 and at 32
+ * warps per SM, the better of the two counts) on all SMs for about `seconds` and returns the
+ * sustained rate in FP64 FMA/s (flop/s = 2x).  Synchronises. */
 int bemcub_fp64_peak(bemcub_ctx* ctx, double seconds, double* host_dfma_per_s);
+
+/* Second roofline reference: the evaluation kernels' own inner loop (Eq. 4.1: 18 FP64
+ * instructions + one MUFU per point-charge interaction, 4 field points per lane, 12 warps per SM)
+ * run for about `seconds` on data resident in shared memory, with no streaming, no rule selection
+ * and no work queue.  Returns point-charge interactions per second: what the instruction mix of
+ * the method itself allows on this GPU.  Synchronises. */
+int bemcub_inner_loop_rate(bemcub_ctx* ctx, double seconds, double* host_interactions_per_s);
 
 /* Device timing of the dominant kernel.  bemcub_set_timing(ctx, 1) makes every following
  * bemcub_eval / bemcub_assemble* call record CUDA events on the ctx stream: around the whole call

@@ -66,6 +66,7 @@ def _load() -> C.CDLL:
         "bemcub_expand_points": [vp, vp, C.c_int, vp, C.POINTER(C.c_int)],
         "bemcub_get_geometry": [vp, vp, vp, vp],
         "bemcub_fp64_peak": [vp, dbl, C.POINTER(dbl)],
+        "bemcub_inner_loop_rate": [vp, dbl, C.POINTER(dbl)],
         "bemcub_get_stats": [vp, C.POINTER(bemcub_stats)],
         "bemcub_reset_stats": [vp],
         "bemcub_set_timing": [vp, C.c_int],
@@ -84,7 +85,7 @@ _lib = _load()
 EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval",
             "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
             "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
-            "bemcub_fp64_peak", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
+            "bemcub_fp64_peak", "bemcub_inner_loop_rate", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
             "bemcub_get_timing", "bemcub_strerror"]
 
 
@@ -217,6 +218,12 @@ def bemcub_get_geometry(ctx, out_cen, out_area, out_L) -> None:
 def bemcub_fp64_peak(ctx, seconds: float) -> float:
     v = C.c_double()
     _check(_lib.bemcub_fp64_peak(ctx, seconds, C.byref(v)), "bemcub_fp64_peak")
+    return v.value
+
+
+def bemcub_inner_loop_rate(ctx, seconds: float) -> float:
+    v = C.c_double()
+    _check(_lib.bemcub_inner_loop_rate(ctx, seconds, C.byref(v)), "bemcub_inner_loop_rate")
     return v.value
 
 

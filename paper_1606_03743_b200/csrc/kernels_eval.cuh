@@ -545,4 +545,29 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Measurement helper (bemcub_inner_loop_rate): the very same consume() loop as the kernels above,
+// fed from a window that is filled once - no TMA, no classification, no work queue.  Its rate is
+// the ceiling the instruction mix of Eq. 4.1 allows on this GPU (register-file bandwidth and
+// dependent-issue latency included), reported next to the DFMA-only peak.
+template <int R>
+__global__ void __launch_bounds__(kThreads, 1) inner_loop_kernel(const double4* __restrict__ pts, const double* __restrict__ field,
+                                                                 int cnt, int trips, double4* __restrict__ out) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double4* win = reinterpret_cast<double4*>(smem_raw) + (size_t)warp * kStages * kBuf;
+  for (int i = lane; i < kStages * kBuf; i += 32) win[i] = pts[i];
+  __syncwarp();
+  const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + warp;
+  double px[R], py[R], pz[R];
+  load_field_points<double, R>(field, (int64_t)gridDim.x * kWarpsPerCta * 32 * R, tile, lane, px, py, pz);
+  Accum<double, R> tot;
+  tot.zero();
+  for (int t = 0; t < trips; ++t) {
+    consume_into<R>(win + (t & 1) * kBuf, cnt, px, py, pz, tot);
+    __syncwarp();
+  }
+  store_partial<R>(out, (int64_t)gridDim.x * kWarpsPerCta * 32 * R, tile, lane, tot);
+}
+
 }  // namespace bemcub

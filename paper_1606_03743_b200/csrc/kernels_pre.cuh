@@ -170,4 +170,16 @@ __global__ void dfma_peak_kernel(double* out, int iters, double a, double b) {
   out[blockIdx.x * (int64_t)blockDim.x + threadIdx.x] = s;
 }
 
+// Resident synthetic data of bemcub_inner_loop_rate: field points 3..4 m away from source points
+// in the unit cube (values only need to be finite and distinct).
+__global__ void fill_synthetic_kernel(int64_t nfield, double* __restrict__ field, int nsrc, double4* __restrict__ src) {
+  const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (j < nfield) {
+    field[3 * j] = 3.0 + 1e-4 * (double)(j % 9973);
+    field[3 * j + 1] = 2.0 + 1e-4 * (double)(j % 7919);
+    field[3 * j + 2] = 1.0 + 1e-4 * (double)(j % 6007);
+  }
+  if (j < nsrc) src[j] = make_double4(0.001 * (double)j, 0.5 - 0.0007 * (double)j, 0.3 + 0.0003 * (double)j, 1e-9 * (double)(1 + j % 7));
+}
+
 }  // namespace bemcub
