@@ -626,12 +626,18 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   ap.ld = ld;
   ap.k = coulomb_k();
   ap.counters = c->d_counters;
-  CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 2 * sizeof(unsigned long long), c->stream));
+  ap.queue = c->d_counters + 2;
+  CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
   CUDA_TRY(cudaFuncSetAttribute(assemble_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)assemble_smem_bytes()));
-  const int64_t coltiles = (c->n + 31) / 32, rowtiles = (nrows + 31) / 32;
-  // rows on grid.x would exceed no limit either way; y is limited to 65535 tiles = 2.1 M rows per call
-  if (rowtiles > 65535) return BEMCUB_ERR_INVALID_ARG;
-  dim3 grid((unsigned)((coltiles + kAsmWarps - 1) / kAsmWarps), (unsigned)rowtiles);
+  // items = (128-row tile) x (split of the columns, a multiple of 32): about 32 per warp
+  const int64_t warps = (int64_t)c->num_sms * kAsmWarps;
+  ap.nrowtiles = (nrows + kAsmRows - 1) / kAsmRows;
+  const int64_t batches = (c->n + 31) / 32;
+  int64_t nsplit = std::max<int64_t>(1, std::min<int64_t>(batches, (32 * warps + ap.nrowtiles - 1) / ap.nrowtiles));
+  ap.cols_per_split = ((batches + nsplit - 1) / nsplit) * 32;
+  nsplit = (c->n + ap.cols_per_split - 1) / ap.cols_per_split;
+  ap.nitems = ap.nrowtiles * nsplit;
+  const int grid = (int)std::min<int64_t>(c->num_sms, (ap.nitems + kAsmWarps - 1) / kAsmWarps);
   mark(c, 1);
   assemble_kernel<<<grid, kAsmThreads, assemble_smem_bytes(), c->stream>>>(ap);
   count_launch(c);

@@ -3,12 +3,17 @@
 // each entry by the rule its distance ratio DR(i,j) = |c_i - c_j| / L_j asks for (L159), the
 // analytic integral below the first limit (self term: D = 0).
 //
-// One warp fills a 32 x 32 tile: lane l owns ROW i0+l (its field point c_i sits in registers) and,
-// for the classification, COLUMN j0+l.  Columns are then walked warp-uniformly: the rule of column
-// j against the bounding sphere of the 32 row centroids is the same for all lanes unless the tile
-// straddles a band limit (then: more accurate rule, or exact per-pair choice with masks).  The
-// 32 x 32 results go through a padded shared-memory tile and leave as 32 row segments of 256
-// contiguous bytes (coalesced row-major FP64 stores).
+// Same execution model as the evaluation kernels (kernels_eval.cuh): persistent CTAs, every warp
+// pulls items from an atomic queue.  One item = (tile of 128 rows) x (split of the columns).  A lane
+// owns rows i0 + 32 r + lane, r < 4 (their centroids sit in registers).  Columns are taken 32 at a
+// time: lane l classifies column j0+l against the bounding sphere of the row centroids, so the
+// rule of a column is warp-uniform unless the tile straddles a band limit (then: the more accurate
+// rule, or the exact per-pair choice with masks).  The point records of the batch's columns are
+// streamed through the warp's double-buffered shared-memory window by bulk TMA, whole elements per
+// stage, with a small segment table (column, first point, number of points) beside each stage.
+// Results of 8 consecutive columns go through a padded 128 x 8 shared-memory tile and leave as
+// 64-byte row segments (two full 32-byte sectors each, four rows per store instruction); the
+// rare analytic / pair-by-pair entries are stored directly while the first TMA copies fly.
 #pragma once
 #include "kernels_eval.cuh"
 
@@ -26,13 +31,28 @@ struct AssembleParams {
   double* out;
   int64_t ld;
   double k;
+  int64_t cols_per_split;     // multiple of 32
+  int64_t nrowtiles, nitems;  // item = split * nrowtiles + rowtile
+  unsigned long long* queue;
   unsigned long long* counters;
 };
 
-constexpr int kAsmWarps = 8;
+constexpr int kAsmWarps = 12;
 constexpr int kAsmThreads = kAsmWarps * 32;
-constexpr int kTilePad = 33;
-constexpr size_t assemble_smem_bytes() { return (size_t)kAsmWarps * 32 * kTilePad * sizeof(double); }
+constexpr int kAsmR = 4;              // rows per lane
+constexpr int kAsmRows = 32 * kAsmR;  // rows per tile
+constexpr int kGroupCols = 8;          // columns per output group: 64-byte row segments = two full sectors
+constexpr int kTilePad = kGroupCols + 1;
+
+// per-warp shared memory: window | output tile | segment tables | mbarriers | scratch
+struct AsmWarpSmem {
+  double4 win[kStages][kBuf];
+  double tile[kAsmRows * kTilePad];
+  uint32_t seg[kStages][32];  // col | npts << 8 | first << 16
+  uint64_t bar[kStages];
+  WarpScratch scr;
+};
+constexpr size_t assemble_smem_bytes() { return (size_t)kAsmWarps * sizeof(AsmWarpSmem); }
 
 // Potential-only term of Eq. 4.1: 12 FP64-pipe instructions (3 DADD + 3 DMUL + 6 DFMA).
 __device__ __forceinline__ double phi_one(const double4 s, double q, double px, double py, double pz, double acc) {
@@ -41,102 +61,325 @@ __device__ __forceinline__ double phi_one(const double4 s, double q, double px, 
   return __fma_rn(q, rsqrt_f64(r2), acc);
 }
 
-__global__ void __launch_bounds__(kAsmThreads, 2) assemble_kernel(const __grid_constant__ AssembleParams p) {
+// One element's points (already in shared memory) against the lane's kAsmR rows: the same loop
+// shape as the evaluation kernels (one point per trip, kAsmR independent chains).
+__device__ __forceinline__ void phi_segment(const double4* __restrict__ pts, int npts, const double (&px)[kAsmR],
+                                            const double (&py)[kAsmR], const double (&pz)[kAsmR], double (&acc)[kAsmR]) {
+  double acc2[kAsmR];
+#pragma unroll
+  for (int r = 0; r < kAsmR; ++r) acc[r] = acc2[r] = 0.0;
+  int i = 0;
+#pragma unroll 1
+  for (; i + 2 <= npts; i += 2) {  // two points per trip: 2 * kAsmR independent chains
+    const double4 s0 = pts[i], s1 = pts[i + 1];
+#pragma unroll
+    for (int r = 0; r < kAsmR; ++r) acc[r] = phi_one(s0, s0.w, px[r], py[r], pz[r], acc[r]);
+#pragma unroll
+    for (int r = 0; r < kAsmR; ++r) acc2[r] = phi_one(s1, s1.w, px[r], py[r], pz[r], acc2[r]);
+  }
+  if (i < npts) {
+    const double4 s = pts[i];
+#pragma unroll
+    for (int r = 0; r < kAsmR; ++r) acc[r] = phi_one(s, s.w, px[r], py[r], pz[r], acc[r]);
+  }
+#pragma unroll
+  for (int r = 0; r < kAsmR; ++r) acc[r] += acc2[r];
+}
+
+__global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_constant__ AssembleParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t ct = (int64_t)blockIdx.x * kAsmWarps + warp;  // column tile
-  const int64_t j0 = ct * 32;
-  if (j0 >= p.n) return;
-  const int64_t r0 = (int64_t)blockIdx.y * 32;  // first row of the tile, relative to row0
-  double* tile = reinterpret_cast<double*>(smem_raw) + (size_t)warp * 32 * kTilePad;
-
-  // rows: field points = centroids
-  const int64_t nrow_here = min((int64_t)32, p.nrows - r0);
-  const int64_t irow = p.row0 + r0 + min((int64_t)lane, nrow_here - 1);
-  const double4 ci = p.cenL[irow];
-  const double px = ci.x, py = ci.y, pz = ci.z;
-  const double lox = warp_min(px), hix = warp_max(px), loy = warp_min(py), hiy = warp_max(py), loz = warp_min(pz),
-               hiz = warp_max(pz);
-  const double cx = 0.5 * (lox + hix), cy = 0.5 * (loy + hiy), cz = 0.5 * (loz + hiz);
-  const double rho = sqrt(warp_max((px - cx) * (px - cx) + (py - cy) * (py - cy) + (pz - cz) * (pz - cz)));
-  const double mag = fmax(fmax(fabs(cx), fabs(cy)), fabs(cz)) + rho;
-
-  // columns: classify element j0 + lane against the row tile's bounding sphere
-  int lnear = 0, lfar = 0, tcol = 0;
-  double4 cj = make_double4(0, 0, 0, 1);
-  if (j0 + lane < p.n) {
-    cj = p.cenL[j0 + lane];
-    tcol = p.type[j0 + lane];
-    const double dx = cx - cj.x, dy = cy - cj.y, dz = cz - cj.z;
-    const double Dc = sqrt(dx * dx + dy * dy + dz * dz);
-    const double slack = 1e-9 * (Dc + rho) + 1e-12 * (mag + fmax(fmax(fabs(cj.x), fabs(cj.y)), fabs(cj.z)));
-    const double Dhi = Dc + rho + slack, Dlo = fmax(Dc - rho - slack, 0.0);
-    lfar = p.pol.map[want_level(Dhi * Dhi, cj.w, p.pol.dr[tcol])];
-    lnear = p.pol.map[want_level(Dlo * Dlo, cj.w, p.pol.dr[tcol])];
-    // the analytic formula is never an "upgrade" (see eval_adaptive_kernel): a tile straddling
-    // the analytic limit keeps the exact per-pair choice
-    if (p.pol.allow_upgrade && lnear != 5) lfar = lnear;
+  AsmWarpSmem& sm = reinterpret_cast<AsmWarpSmem*>(smem_raw)[warp];
+  const uint32_t bar0 = smem_u32(&sm.bar[0]), win0 = smem_u32(&sm.win[0][0]);
+  if (lane == 0) {
+    mbar_init(bar0, 1);
+    mbar_init(bar0 + 8, 1);
+    mbar_fence_init();
+    sm.scr.n_inter = 0;
+    sm.scr.n_ana = 0;
   }
+  __syncwarp();
+  uint32_t phases = 0;
+  const unsigned lt_mask = (1u << lane) - 1u;
 
-  unsigned long long n_inter = 0, n_ana = 0;
-  const int ncol_here = (int)min((int64_t)32, p.n - j0);
-  for (int jj = 0; jj < ncol_here; ++jj) {
-    const int64_t j = j0 + jj;
-    const int ln = __shfl_sync(kFullMask, lnear, jj), lf = __shfl_sync(kFullMask, lfar, jj);
-    const int t = __shfl_sync(kFullMask, tcol, jj);
-    double val = 0.0;
-    int lev = ln;
-    if (ln != lf) {  // exact per-pair choice
-      const double ex = __shfl_sync(kFullMask, cj.x, jj), ey = __shfl_sync(kFullMask, cj.y, jj),
-                   ez = __shfl_sync(kFullMask, cj.z, jj), Lj = __shfl_sync(kFullMask, cj.w, jj);
-      const double dx = __dsub_rn(px, ex), dy = __dsub_rn(py, ey), dz = __dsub_rn(pz, ez);
-      const double D2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-      lev = p.pol.map[want_level(D2, Lj, p.pol.dr[t])];
+  for (;;) {
+    const int64_t item = next_item(p.queue, lane);
+    if (item >= p.nitems) break;
+    const int64_t split = item / p.nrowtiles, rt = item - split * p.nrowtiles;
+    const int64_t r0 = rt * kAsmRows;  // first row of the tile, relative to row0
+    const int nrow_here = (int)min((int64_t)kAsmRows, p.nrows - r0);
+
+    // rows: field points = centroids (clamped duplicates compute harmlessly and are never stored)
+    double px[kAsmR], py[kAsmR], pz[kAsmR];
+    bool ok[kAsmR];
+#pragma unroll
+    for (int r = 0; r < kAsmR; ++r) {
+      ok[r] = r * 32 + lane < nrow_here;
+      const double4 ci = p.cenL[p.row0 + r0 + min(r * 32 + lane, nrow_here - 1)];
+      px[r] = ci.x; py[r] = ci.y; pz[r] = ci.z;
     }
-    for (int l = lf; l <= ln; ++l) {  // lf <= ln: the near end needs the more accurate level
-      const bool take = (lev == l);
-      if (!__any_sync(kFullMask, take)) continue;
-      if (l == 5) {
-        if (take) {
-          Vec3 V[4];
-          const int nv = load_polygon(p.type, p.verts, j, V);
+    double lox = px[0], hix = px[0], loy = py[0], hiy = py[0], loz = pz[0], hiz = pz[0];
+#pragma unroll
+    for (int r = 1; r < kAsmR; ++r) {
+      lox = fmin(lox, px[r]); hix = fmax(hix, px[r]);
+      loy = fmin(loy, py[r]); hiy = fmax(hiy, py[r]);
+      loz = fmin(loz, pz[r]); hiz = fmax(hiz, pz[r]);
+    }
+    lox = warp_min(lox); hix = warp_max(hix);
+    loy = warp_min(loy); hiy = warp_max(hiy);
+    loz = warp_min(loz); hiz = warp_max(hiz);
+    const double cx = 0.5 * (lox + hix), cy = 0.5 * (loy + hiy), cz = 0.5 * (loz + hiz);
+    double d2 = 0.0;
+#pragma unroll
+    for (int r = 0; r < kAsmR; ++r)
+      d2 = fmax(d2, (px[r] - cx) * (px[r] - cx) + (py[r] - cy) * (py[r] - cy) + (pz[r] - cz) * (pz[r] - cz));
+    const double rho = sqrt(warp_max(d2));
+    const double mag = fmax(fmax(fabs(cx), fabs(cy)), fabs(cz)) + rho;
+
+    const int64_t col_begin = split * p.cols_per_split;
+    const int64_t col_end = min(p.n, col_begin + p.cols_per_split);
+    for (int64_t j0 = col_begin; j0 < col_end; j0 += 32) {
+      const int ncol = (int)min((int64_t)32, col_end - j0);
+      // ---- classify column j0 + lane against the row tile's bounding sphere
+      const int64_t e = j0 + lane;
+      int cnt = 0, lvl = -1;
+      bool is_ana = false, is_mixed = false, is_fix = false;
+      const double4* src = nullptr;
+      if (lane < ncol) {
+        const double4 c = p.cenL[e];
+        const int t = p.type[e];
+        const double dx = cx - c.x, dy = cy - c.y, dz = cz - c.z;
+        const double Dc = sqrt(dx * dx + dy * dy + dz * dz);
+        const double slack = 1e-9 * (Dc + rho) + 1e-12 * (mag + fmax(fmax(fabs(c.x), fabs(c.y)), fabs(c.z)));
+        const double Dhi = Dc + rho + slack, Dlo = fmax(Dc - rho - slack, 0.0);
+        const int lfar = p.pol.map[want_level(Dhi * Dhi, c.w, p.pol.dr[t])];
+        const int lnear = p.pol.map[want_level(Dlo * Dlo, c.w, p.pol.dr[t])];
+        // the analytic formula is never an "upgrade" (see eval_adaptive_kernel): a tile straddling
+        // the analytic limit keeps the exact per-pair choice
+        if (lnear != lfar && lnear == 5 && p.pol.allow_upgrade && p.pol.map[4] != 5) {
+          // tile straddles the analytic limit: the column is streamed with the most accurate
+          // cubature rule, and the rows below the limit are overwritten analytically afterwards
+          is_fix = true;
+          lvl = p.pol.map[4];
+          cnt = rule_npts(t, lvl);
+          src = p.lvl_pts[lvl] + e * p.stride[lvl];
+        } else if (lnear != lfar && (!p.pol.allow_upgrade || lnear == 5)) {
+          is_mixed = true;
+        } else {
+          lvl = lnear;
+          if (lvl == 5) {
+            is_ana = true;
+          } else {
+            cnt = rule_npts(t, lvl);
+            src = p.lvl_pts[lvl] + e * p.stride[lvl];
+          }
+        }
+      }
+      int total;
+      const int pre = warp_excl_scan(cnt, lane, &total);
+      int cursor = 0;
+
+      // Fills `stage` with the next whole elements of the batch; returns how many (0 = batch done).
+      auto fill = [&](int stage) -> int {
+        for (;;) {
+          if (cursor >= 32) return 0;
+          const int base = __shfl_sync(kFullMask, pre, cursor);
+          const bool after = lane >= cursor;
+          const unsigned nofit = __ballot_sync(kFullMask, after && (pre + cnt - base > kBuf));
+          const int next = nofit ? (__ffs(nofit) - 1) : 32;
+          const int pre_next = __shfl_sync(kFullMask, pre, next & 31);
+          const int endp = (next < 32) ? pre_next : total;
+          const int nstage = endp - base;
+          const bool inc = after && lane < next && cnt > 0;
+          const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
+          const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
+          const bool cont = inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == p.stride[lvl];
+          const unsigned incmask = __ballot_sync(kFullMask, inc);
+          const unsigned heads = __ballot_sync(kFullMask, inc && !cont);
+          const unsigned higher = heads & ~((2u << lane) - 1u);
+          const int h2 = higher ? (__ffs(higher) - 1) : 32;
+          const int pre_h2 = __shfl_sync(kFullMask, pre, h2 & 31);
+          const int run_end = (h2 < 32) ? pre_h2 : endp;
+          cursor = next;
+          if (nstage == 0) continue;
+          if (inc) sm.seg[stage][__popc(incmask & lt_mask)] = (uint32_t)lane | ((uint32_t)cnt << 8) | ((uint32_t)(pre - base) << 16);
+          if (lane == 0) {
+            mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
+            sm.scr.n_inter += (unsigned long long)nstage * nrow_here;
+          }
+          __syncwarp();
+          if (inc && !cont)
+            tma_load_1d(win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
+                        (uint32_t)((run_end - pre) * sizeof(double4)), bar0 + 8 * stage);
+          return __popc(incmask);
+        }
+      };
+      // output group (8 consecutive columns) being collected in sm.tile, and which of its columns
+      int cur_group = -1;
+      unsigned gmask = 0;
+      auto flush_group = [&]() {
+        __syncwarp();
+        if (cur_group >= 0) {
+          const int c = lane & (kGroupCols - 1);
+          const int64_t j = j0 + cur_group * kGroupCols + c;
+          if ((gmask >> c) & 1u) {
+#pragma unroll 4
+            for (int row = lane >> 3; row < nrow_here; row += 4) p.out[(r0 + row) * p.ld + j] = sm.tile[row * kTilePad + c];
+          }
+        }
+        __syncwarp();
+      };
+      auto consume_stage = [&](int stage, int nseg) {
+        mbar_wait(bar0 + 8 * stage, (phases >> stage) & 1u);
+        phases ^= 1u << stage;
+        for (int k = 0; k < nseg; ++k) {
+          const uint32_t d = sm.seg[stage][k];
+          const int col = (int)(d & 31u);
+          if ((col >> 3) != cur_group) {
+            flush_group();
+            cur_group = col >> 3;
+            gmask = 0;
+          }
+          double acc[kAsmR];
+          phi_segment(&sm.win[stage][d >> 16], (int)((d >> 8) & 255u), px, py, pz, acc);
+#pragma unroll
+          for (int r = 0; r < kAsmR; ++r) sm.tile[(r * 32 + lane) * kTilePad + (col & (kGroupCols - 1))] = p.k * acc[r];
+          gmask |= 1u << (col & (kGroupCols - 1));
+        }
+        __syncwarp();
+      };
+
+      int na = fill(0);
+      int nb = na ? fill(1) : 0;
+      // while the first copies fly: this batch's special columns, stored directly
+      unsigned amask = __ballot_sync(kFullMask, is_ana), xmask = __ballot_sync(kFullMask, is_mixed);
+      if (amask && lane == 0) sm.scr.n_ana += (unsigned long long)__popc(amask) * nrow_here;
+      while (amask) {
+        const int l = __ffs(amask) - 1;
+        amask &= amask - 1;
+        Vec3 V[4];
+        const int nv = load_polygon(p.type, p.verts, j0 + l, V);
+#pragma unroll
+        for (int r = 0; r < kAsmR; ++r) {
           double ip;
           Vec3 ie;
-          analytic_integrals<false>(V, nv, Vec3{px, py, pz}, ip, ie);
-          val = ip;
-          if (lane < nrow_here) n_ana += 1;
+          analytic_integrals<false>(V, nv, Vec3{px[r], py[r], pz[r]}, ip, ie);
+          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j0 + l] = p.k * ip;
         }
-      } else {
-        const int N = rule_npts(t, l);
-        const double4* src = p.lvl_pts[l] + j * p.stride[l];
-        double acc = 0.0;
-#pragma unroll 4
-        for (int i = 0; i < N; ++i) {
-          const double4 s = ldg4(src + i);
-          acc = phi_one(s, s.w, px, py, pz, acc);
+      }
+      while (xmask) {  // exact per-pair choice
+        const int l = __ffs(xmask) - 1;
+        xmask &= xmask - 1;
+        const int64_t j = j0 + l;
+        const double4 c = ldg4(p.cenL + j);
+        const int t = __ldg(p.type + j);
+        int lev[kAsmR];
+        double val[kAsmR];
+#pragma unroll
+        for (int r = 0; r < kAsmR; ++r) {
+          const double dx = __dsub_rn(px[r], c.x), dy = __dsub_rn(py[r], c.y), dz = __dsub_rn(pz[r], c.z);
+          const double D2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+          lev[r] = p.pol.map[want_level(D2, c.w, p.pol.dr[t])];
+          val[r] = 0.0;
         }
-        if (take) {
-          val = acc;
-          if (lane < nrow_here) n_inter += N;
+        for (int lv = 0; lv <= 5; ++lv) {
+          bool take[kAsmR];
+          bool any = false;
+          int mine = 0;
+#pragma unroll
+          for (int r = 0; r < kAsmR; ++r) {
+            take[r] = lev[r] == lv;
+            any |= take[r];
+            mine += (take[r] && ok[r]) ? 1 : 0;
+          }
+          if (!__any_sync(kFullMask, any)) continue;
+          const int all = warp_sum(mine);
+          if (lv == 5) {
+            Vec3 V[4];
+            const int nv = load_polygon(p.type, p.verts, j, V);
+#pragma unroll
+            for (int r = 0; r < kAsmR; ++r) {
+              if (!take[r]) continue;
+              double ip;
+              Vec3 ie;
+              analytic_integrals<false>(V, nv, Vec3{px[r], py[r], pz[r]}, ip, ie);
+              val[r] = ip;
+            }
+            if (lane == 0) sm.scr.n_ana += (unsigned long long)all;
+          } else {
+            const int N = rule_npts(t, lv);
+            const double4* sp = p.lvl_pts[lv] + j * p.stride[lv];
+            double acc[kAsmR];
+#pragma unroll
+            for (int r = 0; r < kAsmR; ++r) acc[r] = 0.0;
+            double4 s = ldg4(sp);
+#pragma unroll 1
+            for (int i = 0; i < N; ++i) {
+              const double4 nxt = ldg4(sp + min(i + 1, N - 1));
+#pragma unroll
+              for (int r = 0; r < kAsmR; ++r) acc[r] = phi_one(s, s.w, px[r], py[r], pz[r], acc[r]);
+              s = nxt;
+            }
+#pragma unroll
+            for (int r = 0; r < kAsmR; ++r)
+              if (take[r]) val[r] = acc[r];
+            if (lane == 0) sm.scr.n_inter += (unsigned long long)all * N;
+          }
+        }
+#pragma unroll
+        for (int r = 0; r < kAsmR; ++r)
+          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j] = p.k * val[r];
+      }
+      // ---- streamed columns
+      for (;;) {
+        if (!na) break;
+        consume_stage(0, na);
+        na = fill(0);
+        if (!nb) break;
+        consume_stage(1, nb);
+        nb = fill(1);
+      }
+      flush_group();
+      // ---- rows of the straddling columns that lie below the analytic limit (exact per-pair test)
+      unsigned fmask = __ballot_sync(kFullMask, is_fix);
+      while (fmask) {
+        const int l = __ffs(fmask) - 1;
+        fmask &= fmask - 1;
+        const int64_t j = j0 + l;
+        const double4 c = ldg4(p.cenL + j);
+        const int t = __ldg(p.type + j);
+        bool take[kAsmR];
+        bool any = false;
+        int mine = 0;
+#pragma unroll
+        for (int r = 0; r < kAsmR; ++r) {
+          const double dx = __dsub_rn(px[r], c.x), dy = __dsub_rn(py[r], c.y), dz = __dsub_rn(pz[r], c.z);
+          const double D2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+          take[r] = p.pol.map[want_level(D2, c.w, p.pol.dr[t])] == 5;
+          any |= take[r];
+          mine += (take[r] && ok[r]) ? 1 : 0;
+        }
+        if (!__any_sync(kFullMask, any)) continue;
+        const int all = warp_sum(mine);
+        if (lane == 0) sm.scr.n_ana += (unsigned long long)all;
+        Vec3 V[4];
+        const int nv = load_polygon(p.type, p.verts, j, V);
+#pragma unroll
+        for (int r = 0; r < kAsmR; ++r) {
+          if (!take[r]) continue;
+          double ip;
+          Vec3 ie;
+          analytic_integrals<false>(V, nv, Vec3{px[r], py[r], pz[r]}, ip, ie);
+          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j] = p.k * ip;
         }
       }
     }
-    tile[lane * kTilePad + jj] = p.k * val;
   }
+
   __syncwarp();
-  for (int rr = 0; rr < (int)nrow_here; ++rr) {
-    if (lane < ncol_here) p.out[(r0 + rr) * p.ld + j0 + lane] = tile[rr * kTilePad + lane];
-  }
-  if (p.counters) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      n_inter += __shfl_xor_sync(kFullMask, n_inter, o);
-      n_ana += __shfl_xor_sync(kFullMask, n_ana, o);
-    }
-    if (lane == 0) {
-      atomicAdd(p.counters, n_inter);
-      if (n_ana) atomicAdd(p.counters + 1, n_ana);
-    }
+  if (p.counters && lane == 0) {
+    if (sm.scr.n_inter) atomicAdd(p.counters, sm.scr.n_inter);
+    if (sm.scr.n_ana) atomicAdd(p.counters + 1, sm.scr.n_ana);
   }
 }
 
