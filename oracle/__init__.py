@@ -143,6 +143,24 @@ def evaluate(etype, verts, sigma, pts, level: int, dr=None, levels_mask: int = A
     return out
 
 
+CUBATURE_LEVELS = 0b011111
+
+
+def evaluate_gradient(etype, verts, sigma, pts, level: int, dr=None, levels_mask: int = CUBATURE_LEVELS):
+    """Field gradient G_ij = dE_i/dx_j of the Eq. 4.1 point charges, long double.
+    Returns dict(G[m][6] in the order xx, yy, zz, xy, xz, yz; SG[m] = k*sum|q_i|/r_i^3)."""
+    etype = np.ascontiguousarray(etype, dtype=np.uint8)
+    verts, sigma, pts = _f64(verts), _f64(sigma), _f64(pts)
+    n, m = len(etype), len(pts)
+    G, SG = np.zeros((m, 6)), np.zeros(m)
+    drp = None if dr is None else _f64(dr)
+    rc = lib().orc_eval_gradient(C.c_int64(n), _p(etype, C.c_uint8), _p(verts), _p(sigma), level, _p(drp),
+                                 levels_mask, C.c_int64(m), _p(pts), _p(G), _p(SG))
+    if rc:
+        raise ValueError(f"orc_eval_gradient rc={rc}")
+    return dict(G=G, SG=SG)
+
+
 def _single(fn, etype, verts9, P, *extra):
     verts9, P = _f64(verts9).reshape(9), _f64(P).reshape(3)
     ip = C.c_double()

@@ -434,6 +434,61 @@ int eval_impl(int64_t n, const uint8_t* etype, const double* verts, const double
     return ERR_OK;
 }
 
+// ---------------------------------------------------------------------------------------
+// Field gradient from the same point charges (L273: "higher derivatives of the field ... can be
+// easily computed from the point charges"): differentiating the E-term of Eq. 4.1 (L141),
+//     G_ij(P) = dE_i/dx_j = k sum q_i [ delta_ij / r^3 - 3 d_i d_j / r^5 ],   d = P - Q_i, r = |d|.
+// Output order per field point: xx, yy, zz, xy, xz, yz (G is symmetric, and traceless away from
+// the charges).  SG = k sum |q_i| / r^3 is the parity denominator.  Cubature levels only: the
+// paper gives no analytic expression for derivatives, so levels_mask must not contain bit 5.
+template <class T>
+int grad_impl(int64_t n, const uint8_t* etype, const double* verts, const double* sigma, int level,
+              const double* dr, int levels_mask, int64_t m, const double* pts, double* G, double* SG) {
+    if (n < 0 || m < 0 || !G) return ERR_INVALID;
+    if (level < -1 || level > 4) return ERR_BAD_RULE;
+    if (level == -1 && (!dr || (levels_mask & 31) == 0 || (levels_mask & 32))) return ERR_INVALID;
+    for (int64_t e = 0; e < n; ++e) {
+        Geom<T> g;
+        int rc = make_geom<T>(etype[e], verts + 9 * e, g);
+        if (rc) return rc;
+    }
+    const T k = (T)coulomb_k();
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t j = 0; j < m; ++j) {
+        const V3<T> P{(T)pts[3 * j], (T)pts[3 * j + 1], (T)pts[3 * j + 2]};
+        T a[6] = {0, 0, 0, 0, 0, 0}, sg = 0;
+        std::vector<Pt<T>> pv;
+        for (int64_t e = 0; e < n; ++e) {
+            Geom<T> g;
+            make_geom<T>(etype[e], verts + 9 * e, g);
+            int lv = level;
+            if (level == -1) {
+                double dx = pts[3 * j] - (double)g.cen.x, dy = pts[3 * j + 1] - (double)g.cen.y, dz = pts[3 * j + 2] - (double)g.cen.z;
+                lv = choose_level(dx * dx + dy * dy + dz * dz, (double)g.L, dr + 5 * g.type, levels_mask);
+            }
+            element_points<T>(g, lv, pv);
+            const T q = (T)sigma[e] * g.area;
+            for (const Pt<T>& p : pv) {
+                const T qi = p.w * q;
+                const T dx = P.x - p.x, dy = P.y - p.y, dz = P.z - p.z;
+                const T r2 = dx * dx + dy * dy + dz * dz;
+                const T inv = (T)1 / tsqrt<T>(r2);
+                const T inv3 = inv * inv * inv, inv5 = inv3 * inv * inv;
+                a[0] += qi * (inv3 - 3 * dx * dx * inv5);
+                a[1] += qi * (inv3 - 3 * dy * dy * inv5);
+                a[2] += qi * (inv3 - 3 * dz * dz * inv5);
+                a[3] += qi * (-3 * dx * dy * inv5);
+                a[4] += qi * (-3 * dx * dz * inv5);
+                a[5] += qi * (-3 * dy * dz * inv5);
+                sg += tabs(qi) * inv3;
+            }
+        }
+        for (int c = 0; c < 6; ++c) G[6 * j + c] = (double)(k * a[c]);
+        if (SG) SG[j] = (double)(k * sg);
+    }
+    return ERR_OK;
+}
+
 }  // namespace orc
 
 using namespace orc;
@@ -538,6 +593,12 @@ int orc_eval(int64_t n, const uint8_t* etype, const double* verts, const double*
     if (precision == 0)
         return eval_impl<long double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
     return eval_impl<double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
+}
+
+// Field gradient (L273), long double, cubature levels only.
+int orc_eval_gradient(int64_t n, const uint8_t* etype, const double* verts, const double* sigma, int level,
+                      const double* dr, int levels_mask, int64_t m, const double* pts, double* G, double* SG) {
+    return grad_impl<long double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, G, SG);
 }
 
 // Unit-sigma integrals of Eq. 2.1 without the 1/(4 pi eps0) prefactor, three ways.
