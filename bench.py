@@ -35,6 +35,7 @@ if ROOT not in sys.path:
 
 FLOP_PER_INTERACTION = 26      # 8 DFMA + 6 DMUL + 4 DADD per point charge, Phi + E
 FLOP_PER_INTERACTION_PHI = 18  # 6 DFMA + 3 DMUL + 3 DADD, potential only (matrix fill)
+FLOP_PER_INTERACTION_GRAD = 41  # + 5 DFMA + 4 DMUL + 1 DADD for the gradient sums (28 FP64 instructions)
 METRIC = "FP64 Phi+E element.point interactions/s"
 UNIT = "element.point interactions/s"
 
@@ -49,6 +50,8 @@ def parse_args():
     ap.add_argument("--scale", type=float, default=1.0, help="config-4 size factor (profiling only)")
     ap.add_argument("--rule", type=int, default=1, help="fixed rule level of --workload cfg2")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="--workload cfg2 only")
+    ap.add_argument("--gradient", action="store_true",
+                    help="also compute the field gradient (bemcub_eval_gradient; cubature levels only) - not the bench line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -247,7 +250,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         pol = b.bemcub_default_policy(True) if c["rule"] == -1 else None
         phi = torch.empty(m, dtype=torch.float64, device=dev)
         E = torch.empty((m, 3), dtype=torch.float64, device=dev)
-        step = lambda: b.bemcub_eval(h, d_sigma, c["rule"], pol, m, d_pts, phi, E, precision)
+        if args.gradient:
+            if pol is not None:
+                pol.use_levels_mask = 0b011111          # derivatives exist for the point charges only (L273)
+            G = torch.empty((m, 6), dtype=torch.float64, device=dev)
+            step = lambda: b.bemcub_eval_gradient(h, d_sigma, c["rule"], pol, m, d_pts, phi, E, G)
+        else:
+            step = lambda: b.bemcub_eval(h, d_sigma, c["rule"], pol, m, d_pts, phi, E, precision)
 
     # roofline denominator: sustained DFMA rate of this GPU, measured in this run
     dfma_per_s = b.bemcub_fp64_peak(h, 2.0)
@@ -283,7 +292,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     # dominant kernel against the FP64-ALU roofline
     k_ms = sum(kernel_ms) / max(len(kernel_ms), 1)
     inter = float(st["point_interactions"])          # point-charge interactions of the last step
-    flop = inter * (FLOP_PER_INTERACTION_PHI if is_matrix else FLOP_PER_INTERACTION)
+    fpi = FLOP_PER_INTERACTION_PHI if is_matrix else (FLOP_PER_INTERACTION_GRAD if args.gradient else FLOP_PER_INTERACTION)
+    ipi = 12 if is_matrix else (28 if args.gradient else 18)   # FP64 instructions per interaction
+    flop = inter * fpi
     if precision == b.F32:
         roof = {"bound": "alu", "achieved": flop / (k_ms * 1e-3) / 1e12, "peak": None, "unit": "TFLOP/s", "frac": None,
                 "traffic": None, "note": "FP32 variant: reported, no FP32 peak measured"}
@@ -294,10 +305,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                 ("eval_adaptive_kernel" if c["rule"] == -1 else "eval_fixed_kernel"),
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms,
                 "point_interactions_per_launch": inter,
-                "flop_per_interaction": FLOP_PER_INTERACTION_PHI if is_matrix else FLOP_PER_INTERACTION,
+                "flop_per_interaction": fpi,
                 "peak_source": "bemcub_fp64_peak: sustained all-SM DFMA-only loop (best of 16 / 32 warps per SM), 2 s, same run (x2 flop/FMA); "
                                "MEASURED_PEAKS.json has no FP64 entry",
-                "fp64_pipe_frac": (inter * (12 if is_matrix else 18) / (k_ms * 1e-3)) / dfma_per_s,
+                "fp64_pipe_frac": (inter * ipi / (k_ms * 1e-3)) / dfma_per_s,
                 "inner_loop_ceiling": {"interactions_per_s": loop_rate,
                                        "frac_of_peak": loop_rate * FLOP_PER_INTERACTION / (2.0 * dfma_per_s),
                                        "kernel_over_ceiling": None if is_matrix else (inter / (k_ms * 1e-3)) / loop_rate,
@@ -306,7 +317,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 
     # end to end through the host-buffer C-ABI calls: H2D of the inputs, compute, D2H of Phi/E
     e2e = None
-    if not args.no_e2e and not is_matrix:
+    if not args.no_e2e and not is_matrix and not args.gradient:
         o_phi = torch.empty(m, dtype=torch.float64).pin_memory()
         o_E = torch.empty((m, 3), dtype=torch.float64).pin_memory()
         ctx2 = b.Context(local_rank)

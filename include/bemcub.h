@@ -128,6 +128,17 @@ int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const d
 int bemcub_eval(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
                 int64_t m, const double* field_pts, double* out_phi, double* out_E, int precision);
 
+/* Field gradient from the same point charges (L273: derivatives of the field "can be easily
+ * computed from the point charges"): out_G[m][6] = G_xx, G_yy, G_zz, G_xy, G_xz, G_yz with
+ *     G_ab(P) = dE_a/dx_b = k sum_i q_i [ delta_ab / r_i^3 - 3 d_a d_b / r_i^5 ],  d = P - Q_i,
+ * symmetric and traceless (G_zz is formed as -(G_xx + G_yy)); V/m^2.  Same arguments as
+ * bemcub_eval (out_phi / out_E may be NULL; they are computed in the same pass), FP64 only.
+ * Cubature rules only: in adaptive mode the policy must not enable the analytic branch
+ * (use_levels_mask without bit 5, else INVALID_ARG) - the distance-ratio choice then ends at the
+ * most accurate cubature rule.  28 FP64 instructions per point-charge interaction.  Asynchronous. */
+int bemcub_eval_gradient(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
+                         int64_t m, const double* field_pts, double* out_phi, double* out_E, double* out_G);
+
 /* Dense collocation matrix (L34): out_matrix[i*ld + j] = k * Int_{element j} dS / |c_i - Q| (unit
  * sigma), c_i = centroid of element i, rule per pair by the policy (DR(i,j) uses L of element j;
  * the self term has D = 0 and is analytic).  Units V m^2 / C.  ld >= n.  The policy's

@@ -47,7 +47,7 @@ struct bemcub_ctx {
   DevBuf pts64[5], pts32[5];
   int stride[5] = {4, 7, 12, 19, 33};
   // scratch
-  DevBuf partial;
+  DevBuf partial, partial_g;
   DevBuf sort_key[2], sort_idx[2], sort_hist, sort_pts, sort_box;  // a2: Morton order of the field points
   DevBuf host_stage[5];  // device copies of host inputs/outputs for the *_host entry points
   unsigned long long* d_counters = nullptr;
@@ -204,12 +204,12 @@ struct SplitPlan {
 // lane) is as large as the problem allows while still giving every warp several items; the splits
 // (multiples of 32 elements, the adaptive kernel's batch) make the items small enough that the
 // tail of the launch - at most one item per warp - stays around one percent.
-SplitPlan plan_splits(const bemcub_ctx* c, int64_t m) {
+SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r = 4) {
   SplitPlan s;
   const int64_t warps = (int64_t)c->num_sms * kWarpsPerCta;
   const int64_t max_by_len = std::max<int64_t>(1, c->n / 64);
   s.R = 1;
-  for (int R = 4; R > 1; R >>= 1) {
+  for (int R = max_r; R > 1; R >>= 1) {
     const int64_t nt = (m + 32 * R - 1) / (32 * R);
     if (nt * std::min<int64_t>(max_by_len, 64) >= 8 * warps) {
       s.R = R;
@@ -231,21 +231,21 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m) {
   return s;
 }
 
-template <typename T, int R>
+template <typename T, int R, bool GRAD = false>
 int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<T>();
-  CUDA_TRY(cudaFuncSetAttribute(eval_fixed_kernel<T, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  eval_fixed_kernel<T, R><<<sp.grid, kThreads, smem, c->stream>>>(fp);
+  CUDA_TRY(cudaFuncSetAttribute(eval_fixed_kernel<T, R, GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  eval_fixed_kernel<T, R, GRAD><<<sp.grid, kThreads, smem, c->stream>>>(fp);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
 }
 
-template <int R>
+template <int R, bool GRAD = false>
 int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<double>();
-  CUDA_TRY(cudaFuncSetAttribute(eval_adaptive_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  eval_adaptive_kernel<R><<<sp.grid, kThreads, smem, c->stream>>>(ap);
+  CUDA_TRY(cudaFuncSetAttribute(eval_adaptive_kernel<R, GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  eval_adaptive_kernel<R, GRAD><<<sp.grid, kThreads, smem, c->stream>>>(ap);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
@@ -402,7 +402,7 @@ int bemcub_destroy(bemcub_ctx* c) {
   if (!c) return BEMCUB_OK;
   DeviceGuard g(c->device);
   cudaStreamSynchronize(c->stream);
-  release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial);
+  release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial); release(c->partial_g);
   for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); }
   for (int i = 0; i < 2; ++i) { release(c->sort_key[i]); release(c->sort_idx[i]); }
   release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
@@ -480,20 +480,29 @@ int bemcub_expand_points(bemcub_ctx* c, const double* sigma, int rule_id, double
   return BEMCUB_OK;
 }
 
-int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
-                const double* field_pts, double* out_phi, double* out_E, int precision) {
+}  // extern "C"
+
+namespace {
+
+// bemcub_eval and bemcub_eval_gradient (out_G != nullptr) share everything but the accumulators.
+int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
+                const double* field_pts, double* out_phi, double* out_E, double* out_G, int precision) {
   if (!c || m < 0) return BEMCUB_ERR_INVALID_ARG;
   if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
   if (rule_id < -1 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
   if (precision != BEMCUB_F64 && precision != BEMCUB_F32) return BEMCUB_ERR_INVALID_ARG;
   if (m == 0) return BEMCUB_OK;
-  if (!field_pts || (!out_phi && !out_E) || (c->n > 0 && !sigma)) return BEMCUB_ERR_INVALID_ARG;
+  if (!field_pts || (!out_phi && !out_E && !out_G) || (c->n > 0 && !sigma)) return BEMCUB_ERR_INVALID_ARG;
   const bool adaptive = rule_id == BEMCUB_RULE_ADAPTIVE;
+  const bool grad = out_G != nullptr;
+  if (grad && precision != BEMCUB_F64) return BEMCUB_ERR_INVALID_ARG;  // the gradient is FP64 only
   PolicyDev pol;
   if (adaptive) {
     if (precision != BEMCUB_F64) return BEMCUB_ERR_INVALID_ARG;  // the adaptive path is FP64 only
     int rc = build_policy(host_policy, &pol);
     if (rc) return rc;
+    // derivatives exist for the point charges only (L273): no analytic branch in a gradient call
+    if (grad && (host_policy->use_levels_mask & (1 << BEMCUB_LEVEL_ANALYTIC))) return BEMCUB_ERR_INVALID_ARG;
   }
   DeviceGuard g(c->device);
   c->stats.last_eval_launches = 0;
@@ -502,6 +511,7 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   if (c->n == 0) {  // empty mesh: zero potential and field
     if (out_phi) CUDA_TRY(cudaMemsetAsync(out_phi, 0, (size_t)m * 8, c->stream));
     if (out_E) CUDA_TRY(cudaMemsetAsync(out_E, 0, (size_t)m * 24, c->stream));
+    if (out_G) CUDA_TRY(cudaMemsetAsync(out_G, 0, (size_t)m * 48, c->stream));
     c->stats.point_interactions = 0;
     c->stats.analytic_pairs = 0;
     return BEMCUB_OK;
@@ -522,8 +532,9 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     if ((rc = expand_level<float>(c, rule_id, sigma, c->pts32[rule_id]))) return rc;
   }
 
-  const SplitPlan sp = plan_splits(c, m);
+  const SplitPlan sp = plan_splits(c, m, grad ? 2 : 4);
   if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
+  if (grad && (rc = ensure(c->partial_g, (size_t)sp.nsplit * (size_t)m * 48))) return rc;
   // a2: tiles of spatially close field points (adaptive mode; a fixed rule has nothing to choose)
   const uint32_t* perm = nullptr;
   if (adaptive && m > 32 && m < ((int64_t)1 << 31)) {
@@ -539,12 +550,15 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     fp.field = field_pts;
     fp.m = m;
     fp.partial = (double4*)c->partial.ptr;
+    fp.partial_g = (double*)c->partial_g.ptr;
     fp.split_stride = m;
     fp.ntiles = sp.ntiles;
     fp.nitems = sp.nitems;
     fp.queue = c->d_counters + 2;
     CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
-    if (precision == BEMCUB_F64)
+    if (grad)
+      rc = sp.R == 2 ? launch_fixed<double, 2, true>(c, fp, sp) : launch_fixed<double, 1, true>(c, fp, sp);
+    else if (precision == BEMCUB_F64)
       rc = sp.R == 4 ? launch_fixed<double, 4>(c, fp, sp) : sp.R == 2 ? launch_fixed<double, 2>(c, fp, sp) : launch_fixed<double, 1>(c, fp, sp);
     else
       rc = sp.R == 4 ? launch_fixed<float, 4>(c, fp, sp) : sp.R == 2 ? launch_fixed<float, 2>(c, fp, sp) : launch_fixed<float, 1>(c, fp, sp);
@@ -570,13 +584,15 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     ap.field = field_pts;
     ap.m = m;
     ap.partial = (double4*)c->partial.ptr;
+    ap.partial_g = (double*)c->partial_g.ptr;
     ap.split_stride = m;
     ap.ntiles = sp.ntiles;
     ap.nitems = sp.nitems;
     ap.queue = c->d_counters + 2;
     ap.counters = c->d_counters;
     CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
-    rc = sp.R == 4 ? launch_adaptive<4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
+    if (grad) rc = sp.R == 2 ? launch_adaptive<2, true>(c, ap, sp) : launch_adaptive<1, true>(c, ap, sp);
+    else rc = sp.R == 4 ? launch_adaptive<4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
     if (rc) return rc;
     c->counters_pending = true;
   }
@@ -585,12 +601,27 @@ int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   // a6: cross-split reduction and the 1/(4 pi eps0) prefactor
   const int threads = 256;
   reduce_scale_kernel<<<(unsigned)((m + threads - 1) / threads), threads, 0, c->stream>>>(
-      m, sp.nsplit, m, (const double4*)c->partial.ptr, coulomb_k(), perm, out_phi, out_E);
+      m, sp.nsplit, m, (const double4*)c->partial.ptr, (const double*)c->partial_g.ptr, coulomb_k(), perm, out_phi, out_E, out_G);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   mark(c, 3);
   c->timing_valid = c->timing;
   return BEMCUB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
+                const double* field_pts, double* out_phi, double* out_E, int precision) {
+  return eval_common(c, sigma, rule_id, host_policy, m, field_pts, out_phi, out_E, nullptr, precision);
+}
+
+int bemcub_eval_gradient(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
+                         const double* field_pts, double* out_phi, double* out_E, double* out_G) {
+  if (!out_G) return BEMCUB_ERR_INVALID_ARG;
+  return eval_common(c, sigma, rule_id, host_policy, m, field_pts, out_phi, out_E, out_G, BEMCUB_F64);
 }
 
 int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_t row0, int64_t nrows, double* out_rows,

@@ -131,8 +131,8 @@ __global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* _
 // (Eq. 4.1 prefactor, L141).  `perm` (may be null) maps the evaluation order back to the caller's
 // field-point order (kernels_sort.cuh).
 __global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride, const double4* __restrict__ partial,
-                                    double k, const uint32_t* __restrict__ perm, double* __restrict__ phi,
-                                    double* __restrict__ E) {
+                                    const double* __restrict__ partial_g, double k, const uint32_t* __restrict__ perm,
+                                    double* __restrict__ phi, double* __restrict__ E, double* __restrict__ G) {
   int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (j >= m) return;
   double4 s = partial[j];
@@ -143,12 +143,27 @@ __global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride,
     s.z += p.z;
     s.w += p.w;
   }
+  double g[6] = {0, 0, 0, 0, 0, 0};
+  if (G) {
+    for (int sp = 0; sp < nsplit; ++sp)
+#pragma unroll
+      for (int c = 0; c < 6; ++c) g[c] += partial_g[(sp * split_stride + j) * 6 + c];
+  }
   if (perm) j = perm[j];
   if (phi) phi[j] = k * s.x;
   if (E) {
     E[3 * j] = k * s.y;
     E[3 * j + 1] = k * s.z;
     E[3 * j + 2] = k * s.w;
+  }
+  if (G) {  // G_ab = k (delta_ab sg - s_ab); traceless: G_zz = -(G_xx + G_yy)
+    const double gxx = k * (g[0] - g[1]), gyy = k * (g[0] - g[2]);
+    G[6 * j] = gxx;
+    G[6 * j + 1] = gyy;
+    G[6 * j + 2] = -(gxx + gyy);
+    G[6 * j + 3] = -k * g[3];
+    G[6 * j + 4] = -k * g[4];
+    G[6 * j + 5] = -k * g[5];
   }
 }
 
