@@ -71,7 +71,8 @@ enum {
   BEMCUB_ERR_BAD_RULE = -4,
   BEMCUB_ERR_CUDA = -5,
   BEMCUB_ERR_NOMEM = -6,
-  BEMCUB_ERR_NO_ELEMENTS = -7         /* eval/assemble before a successful set_elements    */
+  BEMCUB_ERR_NO_ELEMENTS = -7,        /* eval/assemble before a successful set_elements    */
+  BEMCUB_ERR_NOT_CONVERGED = -8       /* bemcub_solve: mat-vec limit reached (outputs valid) */
 };
 
 /* Distance-ratio policy (Sec. 4).  dr[t][b], t = element type, are the UPPER distance-ratio
@@ -148,6 +149,18 @@ int bemcub_eval_gradient(bemcub_ctx* ctx, const double* sigma, int rule_id, cons
 int bemcub_assemble(bemcub_ctx* ctx, const bemcub_policy* host_policy, double* out_matrix, int64_t ld);
 int bemcub_assemble_rows(bemcub_ctx* ctx, const bemcub_policy* host_policy, int64_t row0, int64_t nrows,
                          double* out_rows, int64_t ld);
+
+/* Matrix-free solve of the collocation system (L34; "shell matrices ... not stored", L200):
+ *     sum_j A_ij sigma_j = rhs_potential[i],  A as bemcub_assemble defines it (never formed),
+ * by right-preconditioned (diagonal = analytic self terms) restarted GMRES(30); every mat-vec is
+ * one potential-only adaptive evaluation at the n element centroids under `host_policy` (use
+ * bemcub_default_policy(.., 0): the potential limits).  sigma[n]: initial guess on entry (zeros
+ * are fine), solution on exit.  Stops when |rhs - A sigma|_2 <= rel_tol |rhs|_2 or after
+ * max_matvecs mat-vecs (then BEMCUB_ERR_NOT_CONVERGED, with the best iterate in sigma).
+ * host_matvecs / host_rel_residual (HOST, may be NULL): mat-vecs used, final true relative residual.
+ * Synchronous.  The policy's allow_upgrade changes the operator only at the rules' truncation level. */
+int bemcub_solve(bemcub_ctx* ctx, const bemcub_policy* host_policy, const double* rhs_potential, double* sigma,
+                 double rel_tol, int max_matvecs, int* host_matvecs, double* host_rel_residual);
 
 /* Same as bemcub_set_elements / bemcub_eval with HOST buffers: copies the inputs to ctx-owned
  * device memory, runs, copies phi / E back and synchronises (the end-to-end path bench.py times). */

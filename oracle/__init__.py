@@ -143,6 +143,15 @@ def evaluate(etype, verts, sigma, pts, level: int, dr=None, levels_mask: int = A
     return out
 
 
+def solve(etype, verts, potential, dr, levels_mask: int = ALL_LEVELS):
+    """Charge densities of the BEM collocation system: sum_j A_ij sigma_j = V_i with
+    A from assemble_rows (per-pair rule by distance ratio, analytic self/near terms), solved
+    directly (LAPACK via numpy) - the plain definition of what the iterative GPU solver converges to."""
+    n = len(etype)
+    A, _ = assemble_rows(etype, verts, np.arange(n), dr, levels_mask)
+    return np.linalg.solve(A, _f64(potential)), A
+
+
 CUBATURE_LEVELS = 0b011111
 
 

@@ -16,7 +16,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libbemcub.so"
 SOURCES = [CSRC / "bemcub.cu"]
-DEPS = sorted(CSRC.glob("*.cu*")) + sorted(CSRC.glob("*.h")) + [PKG.parent / "include" / "bemcub.h"]
+DEPS = sorted(CSRC.glob("*.cu*")) + sorted(CSRC.glob("*.h")) + sorted(CSRC.glob("*.inl")) + [PKG.parent / "include" / "bemcub.h"]
 
 NVCC_FLAGS = [
     "-shared", "-Xcompiler", "-fPIC", "-O3", "-std=c++17",

@@ -13,6 +13,7 @@
 #include "kernels_assemble.cuh"
 #include "kernels_eval.cuh"
 #include "kernels_pre.cuh"
+#include "kernels_solve.cuh"
 #include "kernels_sort.cuh"
 #include "rules.h"
 
@@ -49,6 +50,10 @@ struct bemcub_ctx {
   // scratch
   DevBuf partial, partial_g;
   DevBuf sort_key[2], sort_idx[2], sort_hist, sort_pts, sort_box;  // a2: Morton order of the field points
+  const uint32_t* sort_perm = nullptr;  // result of the last sort, reusable by the solver for the same points
+  const double* sort_src = nullptr;
+  int64_t sort_m = 0;
+  DevBuf solve_buf[6];  // GMRES: centroids, diagonal, basis, w, z/residual, small coefficient block
   DevBuf host_stage[5];  // device copies of host inputs/outputs for the *_host entry points
   unsigned long long* d_counters = nullptr;
   bemcub_stats stats{};
@@ -231,21 +236,21 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r = 4) {
   return s;
 }
 
-template <typename T, int R, bool GRAD = false>
+template <typename T, int R, int MODE = kModePhiE>
 int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<T>();
-  CUDA_TRY(cudaFuncSetAttribute(eval_fixed_kernel<T, R, GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  eval_fixed_kernel<T, R, GRAD><<<sp.grid, kThreads, smem, c->stream>>>(fp);
+  CUDA_TRY(cudaFuncSetAttribute(eval_fixed_kernel<T, R, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  eval_fixed_kernel<T, R, MODE><<<sp.grid, kThreads, smem, c->stream>>>(fp);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
 }
 
-template <int R, bool GRAD = false>
+template <int R, int MODE = kModePhiE>
 int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<double>();
-  CUDA_TRY(cudaFuncSetAttribute(eval_adaptive_kernel<R, GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  eval_adaptive_kernel<R, GRAD><<<sp.grid, kThreads, smem, c->stream>>>(ap);
+  CUDA_TRY(cudaFuncSetAttribute(eval_adaptive_kernel<R, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  eval_adaptive_kernel<R, MODE><<<sp.grid, kThreads, smem, c->stream>>>(ap);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
@@ -320,6 +325,7 @@ const char* bemcub_strerror(int code) {
     case BEMCUB_ERR_CUDA: return "CUDA error";
     case BEMCUB_ERR_NOMEM: return "out of device memory";
     case BEMCUB_ERR_NO_ELEMENTS: return "no mesh: call bemcub_set_elements first";
+    case BEMCUB_ERR_NOT_CONVERGED: return "iteration stopped at the mat-vec limit before reaching the tolerance";
   }
   return "unknown error code";
 }
@@ -406,6 +412,7 @@ int bemcub_destroy(bemcub_ctx* c) {
   for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); }
   for (int i = 0; i < 2; ++i) { release(c->sort_key[i]); release(c->sort_idx[i]); }
   release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
+  for (int i = 0; i < 6; ++i) release(c->solve_buf[i]);
   if (c->d_status) cudaFree(c->d_status);
   if (c->d_counters) cudaFree(c->d_counters);
   for (int i = 0; i < 4; ++i)
@@ -419,6 +426,7 @@ int bemcub_set_elements(bemcub_ctx* c, int64_t n, const uint8_t* type, const dou
   DeviceGuard g(c->device);
   c->has_mesh = false;
   c->n = 0;
+  c->sort_perm = nullptr;
   int rc;
   const size_t nn = (size_t)std::max<int64_t>(n, 1);
   if ((rc = ensure(c->type, nn)) || (rc = ensure(c->verts, nn * 72)) || (rc = ensure(c->cenL, nn * sizeof(double4))) ||
@@ -486,7 +494,8 @@ namespace {
 
 // bemcub_eval and bemcub_eval_gradient (out_G != nullptr) share everything but the accumulators.
 int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
-                const double* field_pts, double* out_phi, double* out_E, double* out_G, int precision) {
+                const double* field_pts, double* out_phi, double* out_E, double* out_G, int precision,
+                bool reuse_sort = false) {
   if (!c || m < 0) return BEMCUB_ERR_INVALID_ARG;
   if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
   if (rule_id < -1 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
@@ -538,7 +547,17 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   // a2: tiles of spatially close field points (adaptive mode; a fixed rule has nothing to choose)
   const uint32_t* perm = nullptr;
   if (adaptive && m > 32 && m < ((int64_t)1 << 31)) {
-    if ((rc = sort_field_points(c, m, field_pts, &perm, &field_pts))) return rc;
+    if (reuse_sort && c->sort_perm && c->sort_src == field_pts && c->sort_m == m) {
+      perm = c->sort_perm;  // the solver evaluates at the same centroids every iteration
+      field_pts = (const double*)c->sort_pts.ptr;
+    } else {
+      const double* src = field_pts;
+      c->sort_perm = nullptr;
+      if ((rc = sort_field_points(c, m, field_pts, &perm, &field_pts))) return rc;
+      c->sort_perm = perm;
+      c->sort_src = src;
+      c->sort_m = m;
+    }
   }
   mark(c, 1);
 
@@ -556,10 +575,15 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     fp.nitems = sp.nitems;
     fp.queue = c->d_counters + 2;
     CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    const bool phi_only = !grad && !out_E;
     if (grad)
-      rc = sp.R == 2 ? launch_fixed<double, 2, true>(c, fp, sp) : launch_fixed<double, 1, true>(c, fp, sp);
+      rc = sp.R == 2 ? launch_fixed<double, 2, kModeGrad>(c, fp, sp) : launch_fixed<double, 1, kModeGrad>(c, fp, sp);
+    else if (precision == BEMCUB_F64 && phi_only)
+      rc = sp.R == 4 ? launch_fixed<double, 4, kModePhi>(c, fp, sp) : sp.R == 2 ? launch_fixed<double, 2, kModePhi>(c, fp, sp) : launch_fixed<double, 1, kModePhi>(c, fp, sp);
     else if (precision == BEMCUB_F64)
       rc = sp.R == 4 ? launch_fixed<double, 4>(c, fp, sp) : sp.R == 2 ? launch_fixed<double, 2>(c, fp, sp) : launch_fixed<double, 1>(c, fp, sp);
+    else if (phi_only)
+      rc = sp.R == 4 ? launch_fixed<float, 4, kModePhi>(c, fp, sp) : sp.R == 2 ? launch_fixed<float, 2, kModePhi>(c, fp, sp) : launch_fixed<float, 1, kModePhi>(c, fp, sp);
     else
       rc = sp.R == 4 ? launch_fixed<float, 4>(c, fp, sp) : sp.R == 2 ? launch_fixed<float, 2>(c, fp, sp) : launch_fixed<float, 1>(c, fp, sp);
     if (rc) return rc;
@@ -591,7 +615,8 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     ap.queue = c->d_counters + 2;
     ap.counters = c->d_counters;
     CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
-    if (grad) rc = sp.R == 2 ? launch_adaptive<2, true>(c, ap, sp) : launch_adaptive<1, true>(c, ap, sp);
+    if (grad) rc = sp.R == 2 ? launch_adaptive<2, kModeGrad>(c, ap, sp) : launch_adaptive<1, kModeGrad>(c, ap, sp);
+    else if (!out_E) rc = sp.R == 4 ? launch_adaptive<4, kModePhi>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2, kModePhi>(c, ap, sp) : launch_adaptive<1, kModePhi>(c, ap, sp);
     else rc = sp.R == 4 ? launch_adaptive<4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
     if (rc) return rc;
     c->counters_pending = true;
@@ -623,6 +648,12 @@ int bemcub_eval_gradient(bemcub_ctx* c, const double* sigma, int rule_id, const 
   if (!out_G) return BEMCUB_ERR_INVALID_ARG;
   return eval_common(c, sigma, rule_id, host_policy, m, field_pts, out_phi, out_E, out_G, BEMCUB_F64);
 }
+
+}  // extern "C"
+
+#include "bemcub_solve.inl"
+
+extern "C" {
 
 int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_t row0, int64_t nrows, double* out_rows,
                          int64_t ld) {

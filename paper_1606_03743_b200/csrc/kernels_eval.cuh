@@ -57,11 +57,15 @@ __device__ __forceinline__ int64_t next_item(unsigned long long* queue, int lane
   return (int64_t)__shfl_sync(kFullMask, it, 0);
 }
 
-// Running sums of one lane.  GRAD adds the six sums the field gradient needs:
+// What a kernel accumulates per field point: Phi and E (Eq. 4.1), Phi, E and the field gradient
+// (L273), or the potential alone (the mat-vec of a BEM solve, L34; any call without out_E).
+constexpr int kModePhiE = 0, kModeGrad = 1, kModePhi = 2;
+
+// Running sums of one lane.  kModeGrad adds the six sums the field gradient needs:
 // sg = sum q/r^3 and s_ab = sum 3 q d_a d_b / r^5, from which G_ab = k (delta_ab sg - s_ab).
-template <typename T, int R, bool GRAD = false>
+template <typename T, int R, int MODE = kModePhiE>
 struct Accum {
-  static constexpr int RG = GRAD ? R : 1;
+  static constexpr int RG = (MODE == kModeGrad) ? R : 1;
   T phi[R], ex[R], ey[R], ez[R];
   T sg[RG], sxx[RG], syy[RG], sxy[RG], sxz[RG], syz[RG];
   __device__ __forceinline__ void zero() {
@@ -85,6 +89,17 @@ __device__ __forceinline__ void interact_one(double sx, double sy, double sz, do
   ex = __fma_rn(dx, g, ex);
   ey = __fma_rn(dy, g, ey);
   ez = __fma_rn(dz, g, ez);
+}
+// Potential only: 12 FP64-pipe instructions (3 DADD + 3 DMUL + 6 DFMA).
+__device__ __forceinline__ void interact_one_phi(double sx, double sy, double sz, double q, double px, double py, double pz,
+                                                 double& phi) {
+  const double dx = __dsub_rn(px, sx), dy = __dsub_rn(py, sy), dz = __dsub_rn(pz, sz);
+  const double r2 = __fma_rn(dx, dx, __fma_rn(dy, dy, __dmul_rn(dz, dz)));
+  phi = __fma_rn(q, rsqrt_f64(r2), phi);
+}
+__device__ __forceinline__ void interact_one_phi(float sx, float sy, float sz, float q, float px, float py, float pz, float& phi) {
+  const float dx = px - sx, dy = py - sy, dz = pz - sz;
+  phi = fmaf(q, rsqrt_f32(fmaf(dx, dx, fmaf(dy, dy, dz * dz))), phi);
 }
 // The same term plus its derivative sums: 10 more FP64 instructions (4 DMUL + 1 DADD + 5 DFMA).
 // s_zz is never formed: h r^2 = 3 g makes the gradient traceless, G_zz = -(G_xx + G_yy).
@@ -123,14 +138,16 @@ __device__ __forceinline__ void interact_one(float sx, float sy, float sz, float
   ez = fmaf(dz, g, ez);
 }
 
-template <typename T, int R, bool GRAD, typename P4>
+template <typename T, int R, int MODE, typename P4>
 __device__ __forceinline__ void interact(const P4 s, const T (&px)[R], const T (&py)[R], const T (&pz)[R],
-                                         Accum<T, R, GRAD>& a) {
+                                         Accum<T, R, MODE>& a) {
 #pragma unroll
   for (int r = 0; r < R; ++r) {
-    if constexpr (GRAD)
+    if constexpr (MODE == kModeGrad)
       interact_one_grad(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], a.ex[r], a.ey[r], a.ez[r], a.sg[r], a.sxx[r],
                         a.syy[r], a.sxy[r], a.sxz[r], a.syz[r]);
+    else if constexpr (MODE == kModePhi)
+      interact_one_phi(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r]);
     else
       interact_one(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], a.ex[r], a.ey[r], a.ez[r]);
   }
@@ -138,9 +155,9 @@ __device__ __forceinline__ void interact(const P4 s, const T (&px)[R], const T (
 
 // All `cnt` points of a filled window applied to the warp's field points, U points per trip so
 // that a lane always has >= 4 independent interaction chains in flight.
-template <typename T, int R, bool GRAD, typename P4>
+template <typename T, int R, int MODE, typename P4>
 __device__ __forceinline__ void consume(const P4* __restrict__ buf, int cnt, const T (&px)[R], const T (&py)[R],
-                                        const T (&pz)[R], Accum<T, R, GRAD>& a) {
+                                        const T (&pz)[R], Accum<T, R, MODE>& a) {
   constexpr int U = R >= 4 ? 1 : (R >= 2 ? 2 : 4);
   int i = 0;
 #pragma unroll 1
@@ -149,26 +166,26 @@ __device__ __forceinline__ void consume(const P4* __restrict__ buf, int cnt, con
 #pragma unroll
     for (int u = 0; u < U; ++u) s[u] = buf[i + u];
 #pragma unroll
-    for (int u = 0; u < U; ++u) interact<T, R, GRAD>(s[u], px, py, pz, a);
+    for (int u = 0; u < U; ++u) interact<T, R, MODE>(s[u], px, py, pz, a);
   }
 #pragma unroll 1
-  for (; i < cnt; ++i) interact<T, R, GRAD>(buf[i], px, py, pz, a);
+  for (; i < cnt; ++i) interact<T, R, MODE>(buf[i], px, py, pz, a);
 }
 
 // FP64: the window's sum goes straight into the running totals.  FP32: the window (<= kBuf
 // terms) is summed in FP32 and the block sum is added to FP64 totals (reading 11).
-template <int R, bool GRAD>
+template <int R, int MODE>
 __device__ __forceinline__ void consume_into(const double4* buf, int cnt, const double (&px)[R], const double (&py)[R],
-                                             const double (&pz)[R], Accum<double, R, GRAD>& tot) {
-  consume<double, R, GRAD>(buf, cnt, px, py, pz, tot);
+                                             const double (&pz)[R], Accum<double, R, MODE>& tot) {
+  consume<double, R, MODE>(buf, cnt, px, py, pz, tot);
 }
-template <int R, bool GRAD>
+template <int R, int MODE>
 __device__ __forceinline__ void consume_into(const float4* buf, int cnt, const float (&px)[R], const float (&py)[R],
-                                             const float (&pz)[R], Accum<double, R, GRAD>& tot) {
-  static_assert(!GRAD, "the field gradient is FP64 only");
-  Accum<float, R> a;
+                                             const float (&pz)[R], Accum<double, R, MODE>& tot) {
+  static_assert(MODE != kModeGrad, "the field gradient is FP64 only");
+  Accum<float, R, MODE> a;
   a.zero();
-  consume<float, R, false>(buf, cnt, px, py, pz, a);
+  consume<float, R, MODE>(buf, cnt, px, py, pz, a);
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     tot.phi[r] += (double)a.phi[r];
@@ -191,16 +208,16 @@ __device__ __forceinline__ void load_field_points(const double* __restrict__ fie
   }
 }
 
-// partial_g (GRAD only): [m][6] = sg, sxx, syy, sxy, sxz, syz of this split
-template <int R, bool GRAD>
+// partial_g (gradient mode only): [m][6] = sg, sxx, syy, sxy, sxz, syz of this split
+template <int R, int MODE>
 __device__ __forceinline__ void store_partial(double4* __restrict__ partial, double* __restrict__ partial_g, int64_t m,
-                                              int64_t tile, int lane, const Accum<double, R, GRAD>& tot) {
+                                              int64_t tile, int lane, const Accum<double, R, MODE>& tot) {
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     const int64_t j = tile * (32 * R) + r * 32 + lane;
     if (j < m) {
       partial[j] = make_double4(tot.phi[r], tot.ex[r], tot.ey[r], tot.ez[r]);
-      if constexpr (GRAD) {
+      if constexpr (MODE == kModeGrad) {
         double2* g = reinterpret_cast<double2*>(partial_g + 6 * j);
         g[0] = make_double2(tot.sg[r], tot.sxx[r]);
         g[1] = make_double2(tot.syy[r], tot.sxy[r]);
@@ -246,14 +263,14 @@ struct FixedParams {
   const double* field;      // [m][3]
   int64_t m;
   double4* partial;         // [nsplit][split_stride]
-  double* partial_g;        // [nsplit][split_stride][6], gradient sums (GRAD kernels only)
+  double* partial_g;        // [nsplit][split_stride][6], gradient sums (gradient kernels only)
   int64_t split_stride;
   int64_t ntiles;           // ceil(m / (32 R))
   int64_t nitems;           // ntiles * nsplit; item = split * ntiles + tile
   unsigned long long* queue;  // work-item counter, zeroed before the launch
 };
 
-template <typename T, int R, bool GRAD = false>
+template <typename T, int R, int MODE = kModePhiE>
 __global__ void __launch_bounds__(kThreads, 1) eval_fixed_kernel(const __grid_constant__ FixedParams p) {
   typedef typename Point4<T>::type P4;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -273,7 +290,7 @@ __global__ void __launch_bounds__(kThreads, 1) eval_fixed_kernel(const __grid_co
     const int64_t q1 = min(p.npts, q0 + p.pts_per_split);
     const int64_t nchunks = (q1 - q0 + kBuf - 1) / kBuf;
 
-    Accum<double, R, GRAD> tot;
+    Accum<double, R, MODE> tot;
     tot.zero();
     auto fill = [&](int64_t c, int stage) {
       if (lane == 0) {
@@ -290,10 +307,10 @@ __global__ void __launch_bounds__(kThreads, 1) eval_fixed_kernel(const __grid_co
       mbar_wait(ws.bar0 + 8 * stage, (phases >> stage) & 1u);
       phases ^= 1u << stage;
       const int cnt = (int)min((int64_t)kBuf, q1 - (q0 + c * kBuf));
-      consume_into<R, GRAD>(ws.win + stage * kBuf, cnt, px, py, pz, tot);
+      consume_into<R, MODE>(ws.win + stage * kBuf, cnt, px, py, pz, tot);
       __syncwarp();  // every lane is done with this stage before it is refilled
     }
-    store_partial<R, GRAD>(p.partial + split * p.split_stride, GRAD ? p.partial_g + split * p.split_stride * 6 : nullptr, p.m,
+    store_partial<R, MODE>(p.partial + split * p.split_stride, (MODE == kModeGrad) ? p.partial_g + split * p.split_stride * 6 : nullptr, p.m,
                            tile, lane, tot);
   }
 }
@@ -336,7 +353,7 @@ struct AdaptiveParams {
   const double* field;
   int64_t m;
   double4* partial;
-  double* partial_g;  // gradient sums (GRAD kernels only)
+  double* partial_g;  // gradient sums (gradient kernels only)
   int64_t split_stride;
   int64_t ntiles;
   int64_t nitems;
@@ -356,9 +373,9 @@ struct WarpTile {
 __device__ __forceinline__ int warp_sum(int v) { return __reduce_add_sync(kFullMask, v); }
 
 // Element `e` evaluated analytically at the field points of the tile selected by `take` (a4).
-template <int R, bool GRAD>
+template <int R, int MODE>
 __device__ __forceinline__ void analytic_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, const bool (&take)[R],
-                                              Accum<double, R, GRAD>& tot) {
+                                              Accum<double, R, MODE>& tot) {
   Vec3 V[4];
   const int nv = load_polygon(p.type, p.verts, e, V);
   const double sg = __ldg(p.sigma + e);
@@ -367,19 +384,24 @@ __device__ __forceinline__ void analytic_element(const AdaptiveParams& p, int64_
     if (!take[r]) continue;
     double ip;
     Vec3 ie;
-    analytic_integrals<true>(V, nv, Vec3{w.px[r], w.py[r], w.pz[r]}, ip, ie);
-    tot.phi[r] += sg * ip;
-    tot.ex[r] += sg * ie.x;
-    tot.ey[r] += sg * ie.y;
-    tot.ez[r] += sg * ie.z;
+    if constexpr (MODE == kModePhi) {
+      analytic_integrals<false>(V, nv, Vec3{w.px[r], w.py[r], w.pz[r]}, ip, ie);
+      tot.phi[r] += sg * ip;
+    } else {
+      analytic_integrals<true>(V, nv, Vec3{w.px[r], w.py[r], w.pz[r]}, ip, ie);
+      tot.phi[r] += sg * ip;
+      tot.ex[r] += sg * ie.x;
+      tot.ey[r] += sg * ie.y;
+      tot.ez[r] += sg * ie.z;
+    }
   }
 }
 
 // Element `e` with the exact per-pair rule choice (tile straddles a band limit and the policy
 // does not allow, or the analytic limit forbids, an upgrade).
-template <int R, bool GRAD>
+template <int R, int MODE>
 __device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, int lane,
-                                           Accum<double, R, GRAD>& tot, WarpScratch* scr) {
+                                           Accum<double, R, MODE>& tot, WarpScratch* scr) {
   const double4 c = ldg4(p.cenL + e);
   const int t = __ldg(p.type + e);
   int lev[R];
@@ -402,32 +424,47 @@ __device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e
     if (!__any_sync(kFullMask, any)) continue;
     const int all = warp_sum(mine);
     if (l == 5) {
-      analytic_element<R, GRAD>(p, e, w, take, tot);  // never reached with GRAD: the host rejects such policies
+      analytic_element<R, MODE>(p, e, w, take, tot);  // never reached in gradient mode: the host rejects such policies
       if (lane == 0) scr->n_ana += (unsigned long long)all;
     } else {
       const int N = rule_npts(t, l);
       const double4* src = p.lvl_pts[l] + e * p.stride[l];
+      // The level's sum is formed for every field point of the lane and then SELECTED, not masked
+      // by a zero charge: a field point that does not take this level may sit exactly on one of its
+      // nodes (an element's own centroid is a node of the 7- and 19-point rules), and 0 * inf = NaN.
+      Accum<double, R, MODE> part;
+      part.zero();
       double4 s = ldg4(src);
 #pragma unroll 1
       for (int i = 0; i < N; ++i) {
         const double4 nxt = ldg4(src + min(i + 1, N - 1));  // prefetch: hides the global-load latency
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-          if constexpr (GRAD)
-            interact_one_grad(s.x, s.y, s.z, take[r] ? s.w : 0.0, w.px[r], w.py[r], w.pz[r], tot.phi[r], tot.ex[r], tot.ey[r],
-                              tot.ez[r], tot.sg[r], tot.sxx[r], tot.syy[r], tot.sxy[r], tot.sxz[r], tot.syz[r]);
-          else
-            interact_one(s.x, s.y, s.z, take[r] ? s.w : 0.0, w.px[r], w.py[r], w.pz[r], tot.phi[r], tot.ex[r], tot.ey[r],
-                         tot.ez[r]);
-        }
+        interact<double, R, MODE>(s, w.px, w.py, w.pz, part);
         s = nxt;
+      }
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        if (!take[r]) continue;
+        tot.phi[r] += part.phi[r];
+        if constexpr (MODE != kModePhi) {
+          tot.ex[r] += part.ex[r];
+          tot.ey[r] += part.ey[r];
+          tot.ez[r] += part.ez[r];
+        }
+        if constexpr (MODE == kModeGrad) {
+          tot.sg[r] += part.sg[r];
+          tot.sxx[r] += part.sxx[r];
+          tot.syy[r] += part.syy[r];
+          tot.sxy[r] += part.sxy[r];
+          tot.sxz[r] += part.sxz[r];
+          tot.syz[r] += part.syz[r];
+        }
       }
       if (lane == 0) scr->n_inter += (unsigned long long)all * N;
     }
   }
 }
 
-template <int R, bool GRAD = false>
+template <int R, int MODE = kModePhiE>
 __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid_constant__ AdaptiveParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -478,7 +515,7 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     const int64_t e_begin = split * p.elems_per_split;
     const int64_t e_end = min(p.n, e_begin + p.elems_per_split);
 
-    Accum<double, R, GRAD> tot;
+    Accum<double, R, MODE> tot;
     tot.zero();
 
     // state of the current 32-element batch: lane l holds element batch0 + l
@@ -564,13 +601,13 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
           while (amask) {
             const int l = __ffs(amask) - 1;
             amask &= amask - 1;
-            analytic_element<R, GRAD>(p, batch0 + l, w, all_ok, tot);
+            analytic_element<R, MODE>(p, batch0 + l, w, all_ok, tot);
           }
         }
         while (xmask) {
           const int l = __ffs(xmask) - 1;
           xmask &= xmask - 1;
-          mixed_element<R, GRAD>(p, batch0 + l, w, lane, tot, scr);
+          mixed_element<R, MODE>(p, batch0 + l, w, lane, tot, scr);
         }
       }
     };
@@ -582,14 +619,14 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
       if (cur > 0) {
         mbar_wait(ws.bar0 + 8 * stage, (phases >> stage) & 1u);
         phases ^= 1u << stage;
-        consume_into<R, GRAD>(ws.win + stage * kBuf, cur, w.px, w.py, w.pz, tot);
+        consume_into<R, MODE>(ws.win + stage * kBuf, cur, w.px, w.py, w.pz, tot);
         __syncwarp();
       }
       if (nxt == 0) break;
       stage ^= 1;
       cur = nxt;
     }
-    store_partial<R, GRAD>(p.partial + split * p.split_stride, GRAD ? p.partial_g + split * p.split_stride * 6 : nullptr, p.m,
+    store_partial<R, MODE>(p.partial + split * p.split_stride, (MODE == kModeGrad) ? p.partial_g + split * p.split_stride * 6 : nullptr, p.m,
                            tile, lane, tot);
   }
 
@@ -619,10 +656,10 @@ __global__ void __launch_bounds__(kThreads, 1) inner_loop_kernel(const double4* 
   Accum<double, R> tot;
   tot.zero();
   for (int t = 0; t < trips; ++t) {
-    consume_into<R, false>(win + (t & 1) * kBuf, cnt, px, py, pz, tot);
+    consume_into<R, kModePhiE>(win + (t & 1) * kBuf, cnt, px, py, pz, tot);
     __syncwarp();
   }
-  store_partial<R, false>(out, nullptr, (int64_t)gridDim.x * kWarpsPerCta * 32 * R, tile, lane, tot);
+  store_partial<R, kModePhiE>(out, nullptr, (int64_t)gridDim.x * kWarpsPerCta * 32 * R, tile, lane, tot);
 }
 
 }  // namespace bemcub

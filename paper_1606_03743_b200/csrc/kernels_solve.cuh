@@ -1,0 +1,78 @@
+// matrix-free solve of the BEM collocation system
+//     sum_j A_ij sigma_j = V_i,   A_ij = k Int_{element j} dS / |c_i - Q|,
+// for the unknown charge densities, without ever storing A ("shell matrices", L200): the mat-vec
+// is the potential-only adaptive evaluation kernel at the element centroids (analytic self and
+// near terms by the distance-ratio policy, L159).  This file holds the small vector kernels of
+// the restarted GMRES iteration around it; all reductions are deterministic (fixed tree, no
+// atomics), so a solve is reproducible bit for bit.
+#pragma once
+#include "analytic.cuh"
+#include "device_utils.cuh"
+
+namespace bemcub {
+
+// diag[i] = A_ii = k * (analytic potential integral of element i at its own centroid); the right
+// (Jacobi) preconditioner of the iteration.
+__global__ void self_term_kernel(int64_t n, const uint8_t* __restrict__ type, const double* __restrict__ verts,
+                                 const double4* __restrict__ cenL, double k, double* __restrict__ diag) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Vec3 V[4];
+  const int nv = load_polygon(type, verts, i, V);
+  const double4 c = cenL[i];
+  double ip;
+  Vec3 ie;
+  analytic_integrals<false>(V, nv, Vec3{c.x, c.y, c.z}, ip, ie);
+  diag[i] = k * ip;
+}
+
+// out[v] = V[v] . w for v < nvec (one block per vector; V[v] = basis + v * ld)
+__global__ void __launch_bounds__(1024) vec_dots_kernel(int64_t n, const double* __restrict__ basis, int64_t ld,
+                                                        const double* __restrict__ w, double* __restrict__ out) {
+  __shared__ double red[32];
+  const double* v = basis + (int64_t)blockIdx.x * ld;
+  double s = 0.0;
+  for (int64_t i = threadIdx.x; i < n; i += blockDim.x) s = fma(v[i], w[i], s);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(kFullMask, s, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    s = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(kFullMask, s, o);
+    if (threadIdx.x == 0) out[blockIdx.x] = s;
+  }
+}
+
+// w += sign * sum_{v < nvec} coef[v] * V[v]      (coef in device memory)
+__global__ void vec_combine_kernel(int64_t n, int nvec, const double* __restrict__ basis, int64_t ld,
+                                   const double* __restrict__ coef, double sign, double* __restrict__ w) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double s = 0.0;
+  for (int v = 0; v < nvec; ++v) s = fma(coef[v], basis[(int64_t)v * ld + i], s);
+  w[i] = fma(sign, s, w[i]);
+}
+
+// dst = alpha * a / (d ? d : 1)          (scaling of a basis vector; preconditioner application)
+__global__ void vec_scale_kernel(int64_t n, double alpha, const double* __restrict__ a, const double* __restrict__ d,
+                                 double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  dst[i] = d ? alpha * a[i] / d[i] : alpha * a[i];
+}
+
+// dst = a - b
+__global__ void vec_sub_kernel(int64_t n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = a[i] - b[i];
+}
+
+// x += u / d
+__global__ void vec_add_scaled_kernel(int64_t n, const double* __restrict__ u, const double* __restrict__ d, double* __restrict__ x) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) x[i] += u[i] / d[i];
+}
+
+}  // namespace bemcub

@@ -107,9 +107,11 @@ def test_ragged_shapes_fixed(n_tri, n_rect, m, level):
         phi, E = g.eval(sigma, pts, level, precision=precision)
         ref = oracle.evaluate(etype, verts, sigma, pts, level)
         assert_parity(phi, E, ref, tol, f"ragged n={len(etype)} m={m} L{level} p{precision}")
-    # potential only (out_E = NULL) gives the same potential
+    # potential only (out_E = NULL) runs the 12-instruction kernel (q/r folded into one FMA): same
+    # potential up to the rounding of that one operation, and the same parity bar
     phi2, _ = g.eval(sigma, pts, level, want_E=False)
-    assert np.array_equal(phi2, g.eval(sigma, pts, level)[0])
+    assert_parity(phi2, None, ref, TOL_F64, "potential only")
+    assert np.all(np.abs(phi2 - g.eval(sigma, pts, level)[0]) <= 1e-14 * ref["Sphi"])
     g.close()
 
 
@@ -248,4 +250,38 @@ def test_cfg4_full_size_sampled():
     idx = np.random.default_rng(160603749).choice(len(phi), 48, replace=False)
     ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx], -1, dr=oracle.default_policy(True))
     assert_parity(phi[idx], E[idx], ref, TOL_F64, "cfg4 full")
+    g.close()
+
+
+# ------------------------------------------------------------------ potential only (out_E = NULL: 12-instruction kernels)
+@pytest.mark.parametrize("precision", [0, 1])
+def test_potential_only_fixed_matches_oracle(precision):
+    c = synth.config2()
+    g = Gpu(c["etype"], c["verts"])
+    phi, _ = g.eval(c["sigma"], c["pts"], 2, precision=precision, want_E=False)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], 2)
+    assert_parity(phi, None, ref, TOL_F32 if precision else TOL_F64, "cfg2 potential only")
+    g.close()
+
+
+@pytest.mark.parametrize("level", [2, 3])
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+def test_potential_only_adaptive_with_analytic_branch(allow_upgrade, level):
+    """Field points = element centroids of a sphere (the mat-vec of a BEM solve): self terms and
+    neighbours go through the analytic branch.  Level 3 is the regression case of a field point
+    sitting exactly on the centroid node of a rule that OTHER points of its tile use (0 * inf)."""
+    c = synth.config1(level=level, m=1)
+    cen = synth.element_centroids(c["etype"], c["verts"])
+    sigma = np.random.default_rng(5).uniform(0.5, 1.5, len(c["etype"]))
+    g = Gpu(c["etype"], c["verts"])
+    pol = _policy(g.b, False, allow_upgrade)
+    phi, _ = g.eval(sigma, cen, -1, policy=pol, want_E=False)
+    ref = oracle.evaluate(c["etype"], c["verts"], sigma, cen, -1, dr=oracle.default_policy(False))
+    err = parity_errors(phi, None, ref)
+    assert err["phi"] <= 1e-10, err          # analytic entries: BASELINE.json's 1e-10
+    # with E as well: same potential; E itself is not compared - on the element's own surface the
+    # normal field jumps by sigma/eps0 and its sign hangs on the rounding of h = n.(P - V0) ~ 1e-17
+    phi2, E2 = g.eval(sigma, cen, -1, policy=pol)
+    err2 = parity_errors(phi2, None, ref)
+    assert np.all(np.isfinite(E2)) and err2["phi"] <= 1e-10, err2
     g.close()
