@@ -46,7 +46,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg4", "cfg2", "cfg3"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg4", "cfg2", "cfg3", "solve"])
     ap.add_argument("--scale", type=float, default=1.0, help="config-4 size factor (profiling only)")
     ap.add_argument("--rule", type=int, default=1, help="fixed rule level of --workload cfg2")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="--workload cfg2 only")
@@ -131,6 +131,12 @@ def make_workload(args, rank: int):
         c["rule"] = args.rule
         c["desc"] = "config 2: unit-cube surface 6144 squares, 10^4 field points, fixed rule level %d, %s" % (
             args.rule, args.precision)
+    elif args.workload == "solve":
+        c = synth.config3()
+        c["pts"] = np.zeros((len(c["etype"]), 3))
+        c["rule"] = None
+        c["desc"] = ("matrix-free BEM solve of the level-5 icosphere (20480 triangles) at unit potential: GMRES(30), "
+                     "right Jacobi, rel. residual 1e-12; every mat-vec = potential-only adaptive evaluation at the centroids")
     else:
         c = synth.config3()
         c["pts"] = np.zeros((len(c["etype"]), 3))
@@ -224,7 +230,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     dev = torch.device("cuda", local_rank)
     c = make_workload(args, rank)
     n, m = len(c["etype"]), len(c["pts"])
-    is_matrix = args.workload == "cfg3"
+    is_matrix = args.workload in ("cfg3", "solve")
+    is_solve = args.workload == "solve"
     precision = b.F32 if (args.workload == "cfg2" and args.precision == "f32") else b.F64
 
     def barrier():
@@ -242,7 +249,17 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     d_type, d_verts = h_type.to(dev), h_verts.to(dev)
     d_sigma, d_pts = h_sigma.to(dev), h_pts.to(dev)
     b.bemcub_set_elements(h, n, d_type, d_verts)
-    if is_matrix:
+    solve_info = {}
+    if is_solve:
+        pol = b.bemcub_default_policy(False)
+        d_V = torch.ones(n, dtype=torch.float64, device=dev)
+        d_s = torch.zeros(n, dtype=torch.float64, device=dev)
+
+        def step():
+            d_s.zero_()
+            mv, res, ok = b.bemcub_solve(h, pol, d_V, d_s, 1e-12, 500)
+            solve_info.update(matvecs=mv, rel_residual=res, converged=ok)
+    elif is_matrix:
         pol = b.bemcub_default_policy(False)
         out = torch.empty((n, n), dtype=torch.float64, device=dev)
         step = lambda: b.bemcub_assemble(h, pol, out, n)
@@ -286,7 +303,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_max = float(t.item())
-    units_per_step = float(n) * float(n if is_matrix else m)
+    units_per_step = float(n) * float(n if is_matrix else m) * (solve_info.get("matvecs", 1) if is_solve else 1)
+    if is_solve:
+        areas = 0.5 * np.linalg.norm(np.cross(c["verts"][:, 1] - c["verts"][:, 0], c["verts"][:, 2] - c["verts"][:, 0]), axis=1)
+        q_tot = float((d_s.cpu().numpy() * areas).sum())
+        solve_info["capacitance_over_4pi_eps0_R"] = q_tot / (4 * np.pi * 8.8541878128e-12)
     value = units_per_step * world / (ms_max * 1e-3)
 
     # dominant kernel against the FP64-ALU roofline
@@ -301,7 +322,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     else:
         ach = flop / (k_ms * 1e-3) / 1e12
         roof = {"bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
-                "traffic": None, "kernel": "assemble_kernel" if is_matrix else
+                "traffic": None, "kernel": "eval_adaptive_kernel<kModePhi>" if is_solve else "assemble_kernel" if is_matrix else
                 ("eval_adaptive_kernel" if c["rule"] == -1 else "eval_fixed_kernel"),
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms,
                 "point_interactions_per_launch": inter,
@@ -348,7 +369,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                "note": "matrix stays on the device (3.36 GB); no host leg"}
 
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not is_solve:
         rate, cores, sample, dt, k = oracle_rate(c, args, target_seconds=15.0)
         cpu = {"value": rate, "unit": UNIT if not is_matrix else "matrix entries/s", "cores": cores, "kind": "oracle",
                "sample": sample, "seconds": dt}
@@ -369,6 +390,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(st["kernel_launches"]),
             "roofline": roof, "cpu_baseline": cpu,
         }
+        if is_solve:
+            line["metric"] = "FP64 potential-only element.point interactions/s inside bemcub_solve"
+            line["unit"] = "element.point interactions/s"
+            line["solve"] = solve_info
+            line["roofline"]["note"] = "kernel_ms / interactions are those of the LAST mat-vec of the solve"
         print(json.dumps(line), flush=True)
     ctx.close()
 
