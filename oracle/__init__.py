@@ -170,6 +170,22 @@ def evaluate_gradient(etype, verts, sigma, pts, level: int, dr=None, levels_mask
     return dict(G=G, SG=SG)
 
 
+def evaluate_linear(etype, verts, sigma_v, pts, level: int, dr=None, levels_mask: int = CUBATURE_LEVELS):
+    """Eq. 4.1 with a charge density that varies linearly over each element:
+    sigma_v[n][3] = values at the three stored vertices, q_i = w_i A sigma(Q_i).  Long double."""
+    etype = np.ascontiguousarray(etype, dtype=np.uint8)
+    verts, sigma_v, pts = _f64(verts), _f64(sigma_v), _f64(pts)
+    n, m = len(etype), len(pts)
+    assert sigma_v.shape == (n, 3)
+    phi, E, Sphi, SE = np.zeros(m), np.zeros((m, 3)), np.zeros(m), np.zeros(m)
+    drp = None if dr is None else _f64(dr)
+    rc = lib().orc_eval_linear(C.c_int64(n), _p(etype, C.c_uint8), _p(verts), _p(sigma_v), level, _p(drp),
+                               levels_mask, C.c_int64(m), _p(pts), _p(phi), _p(E), _p(Sphi), _p(SE))
+    if rc:
+        raise ValueError(f"orc_eval_linear rc={rc}")
+    return dict(phi=phi, E=E, Sphi=Sphi, SE=SE)
+
+
 def _single(fn, etype, verts9, P, *extra):
     verts9, P = _f64(verts9).reshape(9), _f64(P).reshape(3)
     ip = C.c_double()

@@ -489,6 +489,68 @@ int grad_impl(int64_t n, const uint8_t* etype, const double* verts, const double
     return ERR_OK;
 }
 
+// ---------------------------------------------------------------------------------------
+// Non-constant charge density (L275: "linear, quadratic etc. ... q_i = w_i A sigma(Q_i)"): sigma
+// varies linearly over the element, given by its values sv[3] at the three stored vertices
+// (triangle A,B,C; rectangle P0,P1,P3 - the fourth corner then carries sv[1]+sv[2]-sv[0]).
+// sigma(Q) is evaluated from the POSITION of the Gaussian point (in-plane coordinates by a 2x2
+// least-squares solve), not from the rule's reference coordinates.  Cubature levels only.
+template <class T>
+inline T sigma_at(const double* v9, const double* sv, const Pt<T>& Q) {
+    const V3<T> A{(T)v9[0], (T)v9[1], (T)v9[2]}, B{(T)v9[3], (T)v9[4], (T)v9[5]}, Cc{(T)v9[6], (T)v9[7], (T)v9[8]};
+    const V3<T> e1 = sub(B, A), e2 = sub(Cc, A), d = sub(V3<T>{Q.x, Q.y, Q.z}, A);
+    const T a11 = dot(e1, e1), a12 = dot(e1, e2), a22 = dot(e2, e2), b1 = dot(d, e1), b2 = dot(d, e2);
+    const T det = a11 * a22 - a12 * a12;
+    const T s = (b1 * a22 - b2 * a12) / det, t = (a11 * b2 - a12 * b1) / det;
+    return (T)sv[0] + s * ((T)sv[1] - (T)sv[0]) + t * ((T)sv[2] - (T)sv[0]);
+}
+
+template <class T>
+int linear_impl(int64_t n, const uint8_t* etype, const double* verts, const double* sigma_v, int level,
+                const double* dr, int levels_mask, int64_t m, const double* pts, double* phi, double* E,
+                double* Sphi, double* SE) {
+    if (n < 0 || m < 0) return ERR_INVALID;
+    if (level < -1 || level > 4) return ERR_BAD_RULE;
+    if (level == -1 && (!dr || (levels_mask & 31) == 0 || (levels_mask & 32))) return ERR_INVALID;
+    for (int64_t e = 0; e < n; ++e) {
+        Geom<T> g;
+        int rc = make_geom<T>(etype[e], verts + 9 * e, g);
+        if (rc) return rc;
+    }
+    const T k = (T)coulomb_k();
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t j = 0; j < m; ++j) {
+        const V3<T> P{(T)pts[3 * j], (T)pts[3 * j + 1], (T)pts[3 * j + 2]};
+        T aphi = 0, ax = 0, ay = 0, az = 0, sphi = 0, se = 0;
+        std::vector<Pt<T>> pv;
+        for (int64_t e = 0; e < n; ++e) {
+            Geom<T> g;
+            make_geom<T>(etype[e], verts + 9 * e, g);
+            int lv = level;
+            if (level == -1) {
+                double dx = pts[3 * j] - (double)g.cen.x, dy = pts[3 * j + 1] - (double)g.cen.y, dz = pts[3 * j + 2] - (double)g.cen.z;
+                lv = choose_level(dx * dx + dy * dy + dz * dz, (double)g.L, dr + 5 * g.type, levels_mask);
+            }
+            element_points<T>(g, lv, pv);
+            for (const Pt<T>& p : pv) {
+                const T qi = p.w * g.area * sigma_at<T>(verts + 9 * e, sigma_v + 3 * e, p);   // q_i = w_i A sigma(Q_i)
+                const T dx = P.x - p.x, dy = P.y - p.y, dz = P.z - p.z;
+                const T inv = (T)1 / tsqrt<T>(dx * dx + dy * dy + dz * dz);
+                const T inv3 = inv * inv * inv;
+                aphi += qi * inv;
+                ax += qi * dx * inv3; ay += qi * dy * inv3; az += qi * dz * inv3;
+                sphi += tabs(qi) * inv;
+                se += tabs(qi) * inv * inv;
+            }
+        }
+        if (phi) phi[j] = (double)(k * aphi);
+        if (E) { E[3 * j] = (double)(k * ax); E[3 * j + 1] = (double)(k * ay); E[3 * j + 2] = (double)(k * az); }
+        if (Sphi) Sphi[j] = (double)(k * sphi);
+        if (SE) SE[j] = (double)(k * se);
+    }
+    return ERR_OK;
+}
+
 }  // namespace orc
 
 using namespace orc;
@@ -593,6 +655,13 @@ int orc_eval(int64_t n, const uint8_t* etype, const double* verts, const double*
     if (precision == 0)
         return eval_impl<long double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
     return eval_impl<double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
+}
+
+// Linear sigma over each element (L275), long double, cubature levels only.
+int orc_eval_linear(int64_t n, const uint8_t* etype, const double* verts, const double* sigma_v, int level,
+                    const double* dr, int levels_mask, int64_t m, const double* pts, double* phi, double* E,
+                    double* Sphi, double* SE) {
+    return linear_impl<long double>(n, etype, verts, sigma_v, level, dr, levels_mask, m, pts, phi, E, Sphi, SE);
 }
 
 // Field gradient (L273), long double, cubature levels only.
