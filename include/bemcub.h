@@ -140,6 +140,15 @@ int bemcub_eval(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_
 int bemcub_eval_gradient(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
                          int64_t m, const double* field_pts, double* out_phi, double* out_E, double* out_G);
 
+/* Non-constant charge density (L275: "q_i = w_i A sigma(Q_i)"): sigma varies LINEARLY over each
+ * element.  sigma_vertex[n][3] = its values at the three stored vertices (triangle A, B, C;
+ * rectangle P0, P1, P3 - the implied fourth corner carries sigma_1 + sigma_3 - sigma_0).  Everything
+ * else as bemcub_eval; only the charges of the expanded points change (preprocessing, a1).
+ * Cubature rules only: in adaptive mode the policy must not enable the analytic branch (the
+ * closed form is for constant sigma), else INVALID_ARG.  Asynchronous. */
+int bemcub_eval_linear(bemcub_ctx* ctx, const double* sigma_vertex, int rule_id, const bemcub_policy* host_policy,
+                       int64_t m, const double* field_pts, double* out_phi, double* out_E, int precision);
+
 /* Dense collocation matrix (L34): out_matrix[i*ld + j] = k * Int_{element j} dS / |c_i - Q| (unit
  * sigma), c_i = centroid of element i, rule per pair by the policy (DR(i,j) uses L of element j;
  * the self term has D = 0 and is analytic).  Units V m^2 / C.  ld >= n.  The policy's

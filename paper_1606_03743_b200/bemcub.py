@@ -58,6 +58,7 @@ def _load() -> C.CDLL:
         "bemcub_set_elements": [vp, i64, vp, vp],
         "bemcub_eval": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
         "bemcub_eval_gradient": [vp, vp, C.c_int, PP, i64, vp, vp, vp, vp],
+        "bemcub_eval_linear": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
         "bemcub_solve": [vp, PP, vp, vp, dbl, C.c_int, C.POINTER(C.c_int), C.POINTER(dbl)],
         "bemcub_assemble": [vp, PP, vp, i64],
         "bemcub_assemble_rows": [vp, PP, i64, i64, vp, i64],
@@ -85,7 +86,7 @@ def _load() -> C.CDLL:
 
 _lib = _load()
 EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval",
-            "bemcub_eval_gradient", "bemcub_solve",
+            "bemcub_eval_gradient", "bemcub_eval_linear", "bemcub_solve",
             "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
             "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
             "bemcub_fp64_peak", "bemcub_inner_loop_rate", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
@@ -177,6 +178,12 @@ def bemcub_eval(ctx, sigma, rule_id: int, policy, m: int, field_pts, out_phi, ou
 def bemcub_eval_gradient(ctx, sigma, rule_id: int, policy, m: int, field_pts, out_phi, out_E, out_G) -> None:
     _check(_lib.bemcub_eval_gradient(ctx, _dptr(sigma), rule_id, _policy_ptr(policy), m, _dptr(field_pts),
                                      _dptr(out_phi), _dptr(out_E), _dptr(out_G)), "bemcub_eval_gradient")
+
+
+def bemcub_eval_linear(ctx, sigma_vertex, rule_id: int, policy, m: int, field_pts, out_phi, out_E,
+                       precision: int = F64) -> None:
+    _check(_lib.bemcub_eval_linear(ctx, _dptr(sigma_vertex), rule_id, _policy_ptr(policy), m, _dptr(field_pts),
+                                   _dptr(out_phi), _dptr(out_E), precision), "bemcub_eval_linear")
 
 
 ERR_NOT_CONVERGED = -8

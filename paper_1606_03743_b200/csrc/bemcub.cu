@@ -179,7 +179,7 @@ int build_policy(const bemcub_policy* hp, PolicyDev* out) {
 
 // Expanded points of one level, FP64 or FP32, into ctx-owned memory.
 template <typename T>
-int expand_level(bemcub_ctx* c, int level, const double* sigma, DevBuf& dst) {
+int expand_level(bemcub_ctx* c, int level, const double* sigma, DevBuf& dst, const double* sigma_v = nullptr) {
   typedef typename Point4<T>::type P4;
   const int64_t total = c->n * c->stride[level];
   int rc = ensure(dst, (size_t)std::max<int64_t>(total, 1) * sizeof(P4));
@@ -189,7 +189,7 @@ int expand_level(bemcub_ctx* c, int level, const double* sigma, DevBuf& dst) {
   const int64_t blocks = (total + threads - 1) / threads;
   expand_kernel<T><<<(unsigned)blocks, threads, 0, c->stream>>>(
       c->n, level, c->stride[level], (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr,
-      (const double4*)c->cenL.ptr, (const double*)c->area.ptr, sigma, (P4*)dst.ptr);
+      (const double4*)c->cenL.ptr, (const double*)c->area.ptr, sigma, sigma_v, (P4*)dst.ptr);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
@@ -495,13 +495,13 @@ namespace {
 // bemcub_eval and bemcub_eval_gradient (out_G != nullptr) share everything but the accumulators.
 int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
                 const double* field_pts, double* out_phi, double* out_E, double* out_G, int precision,
-                bool reuse_sort = false) {
+                bool reuse_sort = false, const double* sigma_v = nullptr) {
   if (!c || m < 0) return BEMCUB_ERR_INVALID_ARG;
   if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
   if (rule_id < -1 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
   if (precision != BEMCUB_F64 && precision != BEMCUB_F32) return BEMCUB_ERR_INVALID_ARG;
   if (m == 0) return BEMCUB_OK;
-  if (!field_pts || (!out_phi && !out_E && !out_G) || (c->n > 0 && !sigma)) return BEMCUB_ERR_INVALID_ARG;
+  if (!field_pts || (!out_phi && !out_E && !out_G) || (c->n > 0 && !sigma && !sigma_v)) return BEMCUB_ERR_INVALID_ARG;
   const bool adaptive = rule_id == BEMCUB_RULE_ADAPTIVE;
   const bool grad = out_G != nullptr;
   if (grad && precision != BEMCUB_F64) return BEMCUB_ERR_INVALID_ARG;  // the gradient is FP64 only
@@ -511,7 +511,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     int rc = build_policy(host_policy, &pol);
     if (rc) return rc;
     // derivatives exist for the point charges only (L273): no analytic branch in a gradient call
-    if (grad && (host_policy->use_levels_mask & (1 << BEMCUB_LEVEL_ANALYTIC))) return BEMCUB_ERR_INVALID_ARG;
+    if ((grad || sigma_v) && (host_policy->use_levels_mask & (1 << BEMCUB_LEVEL_ANALYTIC))) return BEMCUB_ERR_INVALID_ARG;
   }
   DeviceGuard g(c->device);
   c->stats.last_eval_launches = 0;
@@ -533,12 +533,12 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     for (int l = 0; l < 5; ++l) {
       bool used = false;
       for (int w = 0; w <= 5; ++w) used |= (pol.map[w] == l);
-      if (used && (rc = expand_level<double>(c, l, sigma, c->pts64[l]))) return rc;
+      if (used && (rc = expand_level<double>(c, l, sigma, c->pts64[l], sigma_v))) return rc;
     }
   } else if (precision == BEMCUB_F64) {
-    if ((rc = expand_level<double>(c, rule_id, sigma, c->pts64[rule_id]))) return rc;
+    if ((rc = expand_level<double>(c, rule_id, sigma, c->pts64[rule_id], sigma_v))) return rc;
   } else {
-    if ((rc = expand_level<float>(c, rule_id, sigma, c->pts32[rule_id]))) return rc;
+    if ((rc = expand_level<float>(c, rule_id, sigma, c->pts32[rule_id], sigma_v))) return rc;
   }
 
   const SplitPlan sp = plan_splits(c, m, grad ? 2 : 4);
@@ -641,6 +641,12 @@ extern "C" {
 int bemcub_eval(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
                 const double* field_pts, double* out_phi, double* out_E, int precision) {
   return eval_common(c, sigma, rule_id, host_policy, m, field_pts, out_phi, out_E, nullptr, precision);
+}
+
+int bemcub_eval_linear(bemcub_ctx* c, const double* sigma_vertex, int rule_id, const bemcub_policy* host_policy, int64_t m,
+                       const double* field_pts, double* out_phi, double* out_E, int precision) {
+  if (c && c->n > 0 && !sigma_vertex) return BEMCUB_ERR_INVALID_ARG;
+  return eval_common(c, nullptr, rule_id, host_policy, m, field_pts, out_phi, out_E, nullptr, precision, false, sigma_vertex);
 }
 
 int bemcub_eval_gradient(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,

@@ -85,18 +85,22 @@ __device__ __forceinline__ void store_point(float4* dst, double x, double y, dou
 
 // One thread per (element, slot); slot < stride.  Slots beyond the element's own N are padding:
 // zero charge at the centroid.  sigma == nullptr means unit sigma (matrix assembly, L34).
+// sigma_v != nullptr: the density varies linearly over the element (L275), sigma_v[e][3] = its
+// values at the three stored vertices, q_i = w_i A sigma(Q_i) with sigma(Q_i) from the rule's
+// reference coordinates (triangle: sum lambda_v sigma_v; rectangle: corner value + the two slopes).
 template <typename T>
 __global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* __restrict__ type,
                               const double* __restrict__ verts, const double4* __restrict__ cenL,
                               const double* __restrict__ area, const double* __restrict__ sigma,
-                              typename Point4<T>::type* __restrict__ out) {
+                              const double* __restrict__ sigma_v, typename Point4<T>::type* __restrict__ out) {
   const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (idx >= n * stride) return;
   const int64_t e = idx / stride;
   const int i = (int)(idx - e * stride);
   const int t = type[e];
   const double* v = verts + 9 * e;
-  const double q = (sigma ? sigma[e] : 1.0) * area[e];  // q = sigma A (L143)
+  const double q = (sigma ? sigma[e] : 1.0) * area[e];  // q = sigma A (L143); with sigma_v: q = A
+  const double* sv = sigma_v ? sigma_v + 3 * e : nullptr;
   if (t == 0) {
     const int N = c_tri_off[level + 1] - c_tri_off[level];
     if (i < N) {
@@ -106,7 +110,8 @@ __global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* _
       const double x = fma(lc, v[6], fma(lb, v[3], la * v[0]));
       const double y = fma(lc, v[7], fma(lb, v[4], la * v[1]));
       const double z = fma(lc, v[8], fma(lb, v[5], la * v[2]));
-      store_point(out + idx, x, y, z, r[3] * q);
+      const double sq = sv ? fma(lc, sv[2], fma(lb, sv[1], la * sv[0])) : 1.0;
+      store_point(out + idx, x, y, z, r[3] * q * sq);
       return;
     }
   } else {
@@ -119,7 +124,8 @@ __global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* _
       const double x = fma(ys, v[6] - v[0], fma(xs, v[3] - v[0], c.x));
       const double y = fma(ys, v[7] - v[1], fma(xs, v[4] - v[1], c.y));
       const double z = fma(ys, v[8] - v[2], fma(xs, v[5] - v[2], c.z));
-      store_point(out + idx, x, y, z, r[2] * q);
+      const double sq = sv ? fma(0.5 + ys, sv[2] - sv[0], fma(0.5 + xs, sv[1] - sv[0], sv[0])) : 1.0;
+      store_point(out + idx, x, y, z, r[2] * q * sq);
       return;
     }
   }
