@@ -697,7 +697,7 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   ap.queue = c->d_counters + 2;
   CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
   CUDA_TRY(cudaFuncSetAttribute(assemble_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)assemble_smem_bytes()));
-  // items = (128-row tile) x (split of the columns, a multiple of 32): about 32 per warp
+  // items = (64-row tile) x (split of the columns, a multiple of 32): about 32 per warp
   const int64_t warps = (int64_t)c->num_sms * kAsmWarps;
   ap.nrowtiles = (nrows + kAsmRows - 1) / kAsmRows;
   const int64_t batches = (c->n + 31) / 32;
