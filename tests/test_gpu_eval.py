@@ -285,3 +285,19 @@ def test_potential_only_adaptive_with_analytic_branch(allow_upgrade, level):
     err2 = parity_errors(phi2, None, ref)
     assert np.all(np.isfinite(E2)) and err2["phi"] <= 1e-10, err2
     g.close()
+
+
+def test_results_are_bit_reproducible():
+    """Work items are pulled from an atomic queue, so WHICH warp computes an item varies from run to
+    run; what an item computes, the split sums and their order do not: outputs are bit-identical."""
+    c = synth.config4(scale=0.01, ntracks=100, npts_per_track=100)
+    g = Gpu(c["etype"], c["verts"])
+    pol = _policy(g.b, True, 1)
+    a_phi, a_E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+    for _ in range(3):
+        b_phi, b_E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+        assert np.array_equal(a_phi, b_phi) and np.array_equal(a_E, b_E)
+    f_phi, f_E = g.eval(c["sigma"], c["pts"], 2)
+    f2_phi, f2_E = g.eval(c["sigma"], c["pts"], 2)
+    assert np.array_equal(f_phi, f2_phi) and np.array_equal(f_E, f2_E)
+    g.close()
