@@ -321,8 +321,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                 "traffic": None, "note": "FP32 variant: reported, no FP32 peak measured"}
     else:
         ach = flop / (k_ms * 1e-3) / 1e12
+        # DRAM bytes of ONE launch of the dominant kernel from the committed ncu capture of this very
+        # workload (profiles/r1_cfg4_full_eval_adaptive_counters.csv: 3.28 GB read + 0.55 GB written)
+        traffic = 3277495040 + 549181696 if (args.workload == "cfg4" and args.scale == 1.0 and not args.gradient) else None
         roof = {"bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
-                "traffic": None, "kernel": "eval_adaptive_kernel<kModePhi>" if is_solve else "assemble_kernel" if is_matrix else
+                "traffic": traffic, "kernel": "eval_adaptive_kernel<kModePhi>" if is_solve else "assemble_kernel" if is_matrix else
                 ("eval_adaptive_kernel" if c["rule"] == -1 else "eval_fixed_kernel"),
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms,
                 "point_interactions_per_launch": inter,
