@@ -481,25 +481,33 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     w.first = tile * (32 * R);
     w.m = p.m;
     load_field_points<double, R>(p.field, p.m, tile, lane, w.px, w.py, w.pz);
-    {  // bounding sphere of the tile (clamped duplicates lie inside it by construction)
-      double lox = w.px[0], hix = w.px[0], loy = w.py[0], hiy = w.py[0], loz = w.pz[0], hiz = w.pz[0];
+    {  // bounding sphere of the tile (clamped duplicates lie inside it by construction).  Points
+       // with a non-finite coordinate are left out: their own result is NaN whatever the rule, and
+       // they must not spoil the rule choice of the other points of the tile.
+      double lox = CUDART_INF, hix = -CUDART_INF, loy = CUDART_INF, hiy = -CUDART_INF, loz = CUDART_INF, hiz = -CUDART_INF;
       int cntok = 0;
+      bool fin[R];
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         cntok += w.ok(r, lane) ? 1 : 0;
-        lox = fmin(lox, w.px[r]); hix = fmax(hix, w.px[r]);
-        loy = fmin(loy, w.py[r]); hiy = fmax(hiy, w.py[r]);
-        loz = fmin(loz, w.pz[r]); hiz = fmax(hiz, w.pz[r]);
+        fin[r] = isfinite(w.px[r]) && isfinite(w.py[r]) && isfinite(w.pz[r]);
+        if (fin[r]) {
+          lox = fmin(lox, w.px[r]); hix = fmax(hix, w.px[r]);
+          loy = fmin(loy, w.py[r]); hiy = fmax(hiy, w.py[r]);
+          loz = fmin(loz, w.pz[r]); hiz = fmax(hiz, w.pz[r]);
+        }
       }
       lox = warp_min(lox); hix = warp_max(hix);
       loy = warp_min(loy); hiy = warp_max(hiy);
       loz = warp_min(loz); hiz = warp_max(hiz);
-      const double cx = 0.5 * (lox + hix), cy = 0.5 * (loy + hiy), cz = 0.5 * (loz + hiz);
+      const bool any_fin = lox <= hix;
+      const double cx = any_fin ? 0.5 * (lox + hix) : 0.0, cy = any_fin ? 0.5 * (loy + hiy) : 0.0,
+                   cz = any_fin ? 0.5 * (loz + hiz) : 0.0;
       double d2 = 0.0;
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         const double dx = w.px[r] - cx, dy = w.py[r] - cy, dz = w.pz[r] - cz;
-        d2 = fmax(d2, dx * dx + dy * dy + dz * dz);
+        if (fin[r]) d2 = fmax(d2, dx * dx + dy * dy + dz * dz);
       }
       const double rho = sqrt(warp_max(d2));
       cntok = warp_sum(cntok);

@@ -301,3 +301,22 @@ def test_results_are_bit_reproducible():
     f2_phi, f2_E = g.eval(c["sigma"], c["pts"], 2)
     assert np.array_equal(f_phi, f2_phi) and np.array_equal(f_E, f2_E)
     g.close()
+
+
+def test_non_finite_field_points_do_not_spoil_their_tile():
+    """A NaN / inf field point gives NaN for itself only: the other points of its tile keep the rule
+    choice (and the parity) they would have had."""
+    c = synth.config4(scale=0.002, ntracks=20, npts_per_track=50)
+    pts = c["pts"].copy()
+    bad = np.array([3, 200, 777])
+    pts[3, 0] = np.nan
+    pts[200, 1] = np.inf
+    pts[777] = [-np.inf, np.nan, 0.0]
+    g = Gpu(c["etype"], c["verts"])
+    pol = _policy(g.b, True, 1)
+    phi, E = g.eval(c["sigma"], pts, -1, policy=pol)
+    good = np.setdiff1d(np.arange(len(pts)), bad)
+    assert not np.any(np.isfinite(phi[bad]))
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], pts[good], -1, dr=oracle.default_policy(True))
+    assert_parity(phi[good], E[good], ref, TOL_F64, "tile mates of non-finite points")
+    g.close()
