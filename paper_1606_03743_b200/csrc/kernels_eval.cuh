@@ -13,8 +13,9 @@
 // item long.  The inner loop reads one point with two broadcast LDS.128 and applies it to the R
 // field points of each lane: 18 FP64-pipe instructions per point-charge interaction
 // (4 DADD + 6 DMUL + 8 DFMA = 26 flop) plus one MUFU.RSQ64H.  R = 4 gives four independent
-// dependency chains per lane; with 3 warps per scheduler that saturates the FP64 pipe (measured
-// with the bare loop: 101-103 % of the DFMA-only rate at R = 4, 97 % at R = 2).
+// dependency chains per lane; with 3 warps per scheduler that nearly saturates the FP64 pipe
+// (bare loop, field points from memory: 96 % of the DFMA-only issue rate at R = 4, 94 % at R = 2,
+// 88 % at R = 1; what is missing is register-file bandwidth, not issue slots).
 //
 // Adaptive kernel: per batch of 32 elements each lane classifies ONE element against the bounding
 // sphere of the warp's field points (conservative in both directions), so the rule of an element
