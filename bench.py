@@ -46,7 +46,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg4", "cfg2", "cfg3", "solve"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg4", "cfg2", "cfg3", "solve", "table3"])
     ap.add_argument("--scale", type=float, default=1.0, help="config-4 size factor (profiling only)")
     ap.add_argument("--rule", type=int, default=1, help="fixed rule level of --workload cfg2")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="--workload cfg2 only")
@@ -131,6 +131,14 @@ def make_workload(args, rank: int):
         c["rule"] = args.rule
         c["desc"] = "config 2: unit-cube surface 6144 squares, 10^4 field points, fixed rule level %d, %s" % (
             args.rule, args.precision)
+    elif args.workload == "table3":
+        # the SHAPE of the paper's GPU timing (Table 3: 1.5 M rectangles, 10^4 field points) on a
+        # synthetic cylinder; --rule 1 = the 7-point rule, --rule -1 = distance-ratio dependent
+        et, vt = synth.cylinder_rects(5.0, -10.0, 10.0, 1500, 1000)
+        c = dict(etype=et, verts=vt, sigma=synth.fourier_sigma(synth.element_centroids(et, vt)),
+                 pts=synth.helical_tracks(100, 100), rule=args.rule)
+        c["desc"] = ("Table-3 shape: cylinder of 1.5e6 rectangles, 1e4 helical-track field points, rule %s, Phi+E"
+                     % ("adaptive" if args.rule == -1 else "level %d" % args.rule))
     elif args.workload == "solve":
         c = synth.config3()
         c["pts"] = np.zeros((len(c["etype"]), 3))
