@@ -209,14 +209,19 @@ struct SplitPlan {
 // lane) is as large as the problem allows while still giving every warp several items; the splits
 // (multiples of 32 elements, the adaptive kernel's batch) make the items small enough that the
 // tail of the launch - at most one item per warp - stays around one percent.
-SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r = 4) {
+SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) {
   SplitPlan s;
   const int64_t warps = (int64_t)c->num_sms * kWarpsPerCta;
   const int64_t max_by_len = std::max<int64_t>(1, c->n / 64);
   s.R = 1;
+  // Largest R that still leaves enough items per warp.  A fixed rule only gains from a larger R
+  // (more chains per lane), so it may use many splits; in adaptive mode a larger tile of FEW field
+  // points is also a looser tile (more upgraded elements), so R grows only when tiles are plentiful
+  // (measured on 1.5e6 elements x 1e4 points: fixed rule +4 % with R = 4, adaptive -5 %).
+  const int64_t split_cap = adaptive ? 64 : 512, per_warp = adaptive ? 8 : 16;
   for (int R = max_r; R > 1; R >>= 1) {
     const int64_t nt = (m + 32 * R - 1) / (32 * R);
-    if (nt * std::min<int64_t>(max_by_len, 64) >= 8 * warps) {
+    if (nt * std::min<int64_t>(max_by_len, split_cap) >= per_warp * warps) {
       s.R = R;
       break;
     }
@@ -225,7 +230,7 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r = 4) {
   const int64_t target = warps * 64;
   int64_t ns = (target + s.ntiles - 1) / s.ntiles;
   const int64_t max_by_mem = std::max<int64_t>(1, (int64_t)(1ull << 31) / std::max<int64_t>(32 * m, 1));
-  ns = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(ns, max_by_len), std::min<int64_t>(max_by_mem, 4096)));
+  ns = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(ns, max_by_len), std::min<int64_t>(max_by_mem, 512)));
   int64_t eps = (c->n + ns - 1) / ns;
   eps = (eps + 31) / 32 * 32;
   if (eps < 32) eps = 32;
@@ -541,7 +546,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     if ((rc = expand_level<float>(c, rule_id, sigma, c->pts32[rule_id], sigma_v))) return rc;
   }
 
-  const SplitPlan sp = plan_splits(c, m, grad ? 2 : 4);  // R = 6 was measured: 2 % slower than R = 4 in the full kernel
+  const SplitPlan sp = plan_splits(c, m, grad ? 2 : 4, adaptive);  // R = 6 was measured: 2 % slower than R = 4 in the full kernel
   if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
   if (grad && (rc = ensure(c->partial_g, (size_t)sp.nsplit * (size_t)m * 48))) return rc;
   // a2: tiles of spatially close field points (adaptive mode; a fixed rule has nothing to choose)
