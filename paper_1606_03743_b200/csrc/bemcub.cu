@@ -49,6 +49,11 @@ struct bemcub_ctx {
   int stride[5] = {4, 7, 12, 19, 33};
   // scratch
   DevBuf partial, partial_g;
+  // charges of the last call that passed a sigma: which expanded levels still hold them, and the
+  // sigma itself (the analytic branch needs it) - reused by calls with sigma == NULL
+  bool charged64[5] = {false, false, false, false, false}, charged32[5] = {false, false, false, false, false};
+  DevBuf sigma_keep;
+  bool sigma_kept = false;
   DevBuf sort_key[2], sort_idx[2], sort_hist, sort_pts, sort_box;  // a2: Morton order of the field points
   const uint32_t* sort_perm = nullptr;  // result of the last sort, reusable by the solver for the same points
   const double* sort_src = nullptr;
@@ -413,7 +418,7 @@ int bemcub_destroy(bemcub_ctx* c) {
   if (!c) return BEMCUB_OK;
   DeviceGuard g(c->device);
   cudaStreamSynchronize(c->stream);
-  release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial); release(c->partial_g);
+  release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial); release(c->partial_g); release(c->sigma_keep);
   for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); }
   for (int i = 0; i < 2; ++i) { release(c->sort_key[i]); release(c->sort_idx[i]); }
   release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
@@ -432,6 +437,8 @@ int bemcub_set_elements(bemcub_ctx* c, int64_t n, const uint8_t* type, const dou
   c->has_mesh = false;
   c->n = 0;
   c->sort_perm = nullptr;
+  c->sigma_kept = false;
+  for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = false;
   int rc;
   const size_t nn = (size_t)std::max<int64_t>(n, 1);
   if ((rc = ensure(c->type, nn)) || (rc = ensure(c->verts, nn * 72)) || (rc = ensure(c->cenL, nn * sizeof(double4))) ||
@@ -485,6 +492,7 @@ int bemcub_expand_points(bemcub_ctx* c, const double* sigma, int rule_id, double
   if (rule_id < 0 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
   DeviceGuard g(c->device);
   if (out_stride) *out_stride = c->stride[rule_id];
+  c->charged64[rule_id] = false;
   int rc = expand_level<double>(c, rule_id, sigma, c->pts64[rule_id]);
   if (rc) return rc;
   if (c->n > 0)
@@ -506,7 +514,8 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   if (rule_id < -1 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
   if (precision != BEMCUB_F64 && precision != BEMCUB_F32) return BEMCUB_ERR_INVALID_ARG;
   if (m == 0) return BEMCUB_OK;
-  if (!field_pts || (!out_phi && !out_E && !out_G) || (c->n > 0 && !sigma && !sigma_v)) return BEMCUB_ERR_INVALID_ARG;
+  if (!field_pts || (!out_phi && !out_E && !out_G)) return BEMCUB_ERR_INVALID_ARG;
+  const bool reuse = !sigma && !sigma_v;  // sigma == NULL: the charges of the previous call
   const bool adaptive = rule_id == BEMCUB_RULE_ADAPTIVE;
   const bool grad = out_G != nullptr;
   if (grad && precision != BEMCUB_F64) return BEMCUB_ERR_INVALID_ARG;  // the gradient is FP64 only
@@ -533,17 +542,76 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
 
   c->timing_valid = false;
   mark(c, 0);
-  // a1: expand the levels this call needs, sigma folded in
+  // a1: expand the levels this call needs, sigma folded in - or, with sigma == NULL, check that the
+  // previous call left them there (tracking evaluates the same charges at point after point)
+  bool need[5] = {false, false, false, false, false};
   if (adaptive) {
-    for (int l = 0; l < 5; ++l) {
-      bool used = false;
-      for (int w = 0; w <= 5; ++w) used |= (pol.map[w] == l);
-      if (used && (rc = expand_level<double>(c, l, sigma, c->pts64[l], sigma_v))) return rc;
-    }
-  } else if (precision == BEMCUB_F64) {
-    if ((rc = expand_level<double>(c, rule_id, sigma, c->pts64[rule_id], sigma_v))) return rc;
+    for (int l = 0; l < 5; ++l)
+      for (int w = 0; w <= 5; ++w) need[l] |= (pol.map[w] == l);
   } else {
-    if ((rc = expand_level<float>(c, rule_id, sigma, c->pts32[rule_id], sigma_v))) return rc;
+    need[rule_id] = true;
+  }
+  bool* charged = precision == BEMCUB_F64 ? c->charged64 : c->charged32;
+  if (reuse) {
+    for (int l = 0; l < 5; ++l)
+      if (need[l] && !charged[l]) return BEMCUB_ERR_INVALID_ARG;
+    for (int w = 0; w <= 5 && adaptive; ++w)
+      if (pol.map[w] == 5 && !c->sigma_kept) return BEMCUB_ERR_INVALID_ARG;
+    sigma = c->sigma_kept ? (const double*)c->sigma_keep.ptr : nullptr;
+  } else {
+    for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = false;  // whatever was there held other charges
+    for (int l = 0; l < 5; ++l) {
+      if (!need[l]) continue;
+      if (precision == BEMCUB_F64) rc = expand_level<double>(c, l, sigma, c->pts64[l], sigma_v);
+      else rc = expand_level<float>(c, l, sigma, c->pts32[l], sigma_v);
+      if (rc) return rc;
+      charged[l] = true;
+    }
+    c->sigma_kept = false;
+    if (sigma) {
+      if ((rc = ensure(c->sigma_keep, (size_t)c->n * 8))) return rc;
+      CUDA_TRY(cudaMemcpyAsync(c->sigma_keep.ptr, sigma, (size_t)c->n * 8, cudaMemcpyDeviceToDevice, c->stream));
+      c->sigma_kept = true;
+    }
+  }
+
+  // Few field points (tracking-style calls): elements across the lanes, per-pair rule choice,
+  // warp-shuffle reduction (eval_few_kernel); no tiles, hence no sort.
+  if (!grad && precision == BEMCUB_F64 && m <= kFewMaxM) {
+    const int blocks = c->num_sms * 2;
+    if ((rc = ensure(c->partial, (size_t)blocks * (size_t)m * sizeof(double4)))) return rc;
+    FewParams fw;
+    for (int l = 0; l < 5; ++l) {
+      fw.lvl_pts[l] = (const double4*)c->pts64[l].ptr;
+      fw.stride[l] = c->stride[l];
+    }
+    fw.cenL = (const double4*)c->cenL.ptr;
+    fw.type = (const uint8_t*)c->type.ptr;
+    fw.verts = (const double*)c->verts.ptr;
+    fw.sigma = sigma;
+    fw.n = c->n;
+    if (adaptive) fw.pol = pol;
+    fw.rule = adaptive ? -1 : rule_id;
+    fw.field = field_pts;
+    fw.m = m;
+    fw.partial = (double4*)c->partial.ptr;
+    fw.counters = c->d_counters;
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    mark(c, 1);
+    const dim3 grid((unsigned)blocks, (unsigned)((m + kFewM - 1) / kFewM));
+    if (out_E) eval_few_kernel<kModePhiE><<<grid, kFewWarps * 32, 0, c->stream>>>(fw);
+    else eval_few_kernel<kModePhi><<<grid, kFewWarps * 32, 0, c->stream>>>(fw);
+    count_launch(c);
+    CUDA_TRY(cudaGetLastError());
+    mark(c, 2);
+    reduce_scale_kernel<<<1, 32, 0, c->stream>>>(m, blocks, m, (const double4*)c->partial.ptr, nullptr, coulomb_k(), nullptr,
+                                                 out_phi, out_E, nullptr);
+    count_launch(c);
+    CUDA_TRY(cudaGetLastError());
+    mark(c, 3);
+    c->timing_valid = c->timing;
+    c->counters_pending = true;
+    return BEMCUB_OK;
   }
 
   const SplitPlan sp = plan_splits(c, m, grad ? 2 : 4, adaptive);  // R = 6 was measured: 2 % slower than R = 4 in the full kernel
@@ -684,6 +752,7 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   for (int l = 0; l < 5; ++l) {
     bool used = false;
     for (int w = 0; w <= 5; ++w) used |= (pol.map[w] == l);
+    if (used) c->charged64[l] = false;
     if (used && (rc = expand_level<double>(c, l, nullptr, c->pts64[l]))) return rc;  // unit sigma
     ap.lvl_pts[l] = (const double4*)c->pts64[l].ptr;
     ap.stride[l] = c->stride[l];

@@ -647,6 +647,149 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
 }
 
 // ------------------------------------------------------------------------------------------------
+// Few field points (m <= kFewMaxM; particle tracking asks for the field at one point after the
+// other): the roles are swapped.  Every THREAD owns elements (grid-stride), the
+// kFewM field points of the pass are shared by all lanes, every (element, point) pair gets its
+// rule from its own distance ratio (the per-pair policy of L159, exactly), and the partial sums
+// of the lanes are combined with warp shuffles, then across the warps of the CTA; a6 adds the CTAs.
+// The pass is bound by reading every expanded point once (HBM), not by the FP64 pipe.
+constexpr int kFewM = 4;        // field points per pass (grid.y)
+constexpr int kFewMaxM = 32;    // above this the tiled kernels win (10^6 elements: 0.54 ms at m = 16 vs 1.4 ms tiled at m = 17)
+constexpr int kFewWarps = 8;
+
+struct FewParams {
+  const double4* lvl_pts[5];
+  int stride[5];
+  const double4* cenL;
+  const uint8_t* type;
+  const double* verts;
+  const double* sigma;
+  int64_t n;
+  PolicyDev pol;
+  int rule;  // fixed level 0..4, or -1: per pair by distance ratio
+  const double* field;
+  int64_t m;
+  double4* partial;  // [gridDim.x][m]
+  unsigned long long* counters;
+};
+
+__device__ __forceinline__ double warp_sum_f64(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFullMask, v, o);
+  return v;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(kFewWarps * 32) eval_few_kernel(const __grid_constant__ FewParams p) {
+  __shared__ double red[kFewWarps][kFewM][4];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t j0 = (int64_t)blockIdx.y * kFewM;
+  const int mj = (int)min((int64_t)kFewM, p.m - j0);
+  double px[kFewM], py[kFewM], pz[kFewM];
+#pragma unroll
+  for (int j = 0; j < kFewM; ++j) {
+    const int64_t jj = j0 + min(j, mj - 1);  // clamped duplicates are never stored
+    px[j] = p.field[3 * jj];
+    py[j] = p.field[3 * jj + 1];
+    pz[j] = p.field[3 * jj + 2];
+  }
+  Accum<double, kFewM, MODE> acc;
+  acc.zero();
+  unsigned long long n_inter = 0, n_ana = 0;
+
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < p.n; e += (int64_t)gridDim.x * blockDim.x) {
+    const double4 c = p.cenL[e];
+    const int t = p.type[e];
+    int lev[kFewM];
+    bool same = true;
+#pragma unroll
+    for (int j = 0; j < kFewM; ++j) {
+      if (p.rule >= 0) {
+        lev[j] = p.rule;
+      } else {
+        const double dx = __dsub_rn(px[j], c.x), dy = __dsub_rn(py[j], c.y), dz = __dsub_rn(pz[j], c.z);
+        const double D2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        lev[j] = p.pol.map[want_level(D2, c.w, p.pol.dr[t])];
+      }
+      same &= lev[j] == lev[0];
+    }
+    if (same && lev[0] != 5) {  // the usual case: one rule for all points of the pass
+      const int N = rule_npts(t, lev[0]);
+      const double4* src = p.lvl_pts[lev[0]] + e * p.stride[lev[0]];
+      for (int i = 0; i < N; ++i) interact<double, kFewM, MODE>(ldg4(src + i), px, py, pz, acc);
+      n_inter += (unsigned long long)N * mj;
+      continue;
+    }
+#pragma unroll
+    for (int j = 0; j < kFewM; ++j) {
+      if (j >= mj) continue;
+      if (lev[j] == 5) {
+        Vec3 V[4];
+        const int nv = load_polygon(p.type, p.verts, e, V);
+        const double sg = __ldg(p.sigma + e);
+        double ip;
+        Vec3 ie;
+        if constexpr (MODE == kModePhi) {
+          analytic_integrals<false>(V, nv, Vec3{px[j], py[j], pz[j]}, ip, ie);
+          acc.phi[j] += sg * ip;
+        } else {
+          analytic_integrals<true>(V, nv, Vec3{px[j], py[j], pz[j]}, ip, ie);
+          acc.phi[j] += sg * ip;
+          acc.ex[j] += sg * ie.x;
+          acc.ey[j] += sg * ie.y;
+          acc.ez[j] += sg * ie.z;
+        }
+        n_ana += 1;
+      } else {
+        const int N = rule_npts(t, lev[j]);
+        const double4* src = p.lvl_pts[lev[j]] + e * p.stride[lev[j]];
+        for (int i = 0; i < N; ++i) {
+          const double4 s = ldg4(src + i);
+          if constexpr (MODE == kModePhi) interact_one_phi(s.x, s.y, s.z, s.w, px[j], py[j], pz[j], acc.phi[j]);
+          else interact_one(s.x, s.y, s.z, s.w, px[j], py[j], pz[j], acc.phi[j], acc.ex[j], acc.ey[j], acc.ez[j]);
+        }
+        n_inter += N;
+      }
+    }
+  }
+
+  // lanes -> warp (shuffles) -> CTA (shared memory, fixed order) -> partial[blockIdx.x]
+#pragma unroll
+  for (int j = 0; j < kFewM; ++j) {
+    const double a = warp_sum_f64(acc.phi[j]);
+    double bx = 0.0, by = 0.0, bz = 0.0;
+    if constexpr (MODE != kModePhi) {
+      bx = warp_sum_f64(acc.ex[j]);
+      by = warp_sum_f64(acc.ey[j]);
+      bz = warp_sum_f64(acc.ez[j]);
+    }
+    if (lane == 0) {
+      red[warp][j][0] = a; red[warp][j][1] = bx; red[warp][j][2] = by; red[warp][j][3] = bz;
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < mj) {
+    double4 s = make_double4(0, 0, 0, 0);
+    for (int w = 0; w < kFewWarps; ++w) {
+      s.x += red[w][threadIdx.x][0]; s.y += red[w][threadIdx.x][1];
+      s.z += red[w][threadIdx.x][2]; s.w += red[w][threadIdx.x][3];
+    }
+    p.partial[(int64_t)blockIdx.x * p.m + j0 + threadIdx.x] = s;
+  }
+  if (p.counters) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      n_inter += __shfl_xor_sync(kFullMask, n_inter, o);
+      n_ana += __shfl_xor_sync(kFullMask, n_ana, o);
+    }
+    if (lane == 0) {
+      if (n_inter) atomicAdd(p.counters, n_inter);
+      if (n_ana) atomicAdd(p.counters + 1, n_ana);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Measurement helper (bemcub_inner_loop_rate): the very same consume() loop as the kernels above,
 // fed from a window that is filled once - no TMA, no classification, no work queue.  Its rate is
 // the ceiling the instruction mix of Eq. 4.1 allows on this GPU (register-file bandwidth and
