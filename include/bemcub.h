@@ -125,15 +125,15 @@ int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const d
  *   precision = BEMCUB_F64, or BEMCUB_F32: points, field points and the interaction arithmetic
  *   are FP32, sums of at most 128 terms are FP32 and those block sums are accumulated in FP64
  *   (the analytic branch stays FP64); buffers keep their double type.
- * sigma == NULL: evaluate with the charges of the previous call on this ctx that passed a sigma
- *   (same precision; every rule level this call needs must have been needed by that call too,
- *   e.g. the same policy or the same fixed rule; otherwise INVALID_ARG).  This skips the
- *   preprocessing pass a1 - what a particle tracker wants, which asks for the field of the same
- *   charges at one point after the other (L32).  bemcub_set_elements, bemcub_assemble* and
- *   bemcub_expand_points drop the kept charges.
+ * sigma == NULL: evaluate with the sigma of the previous call on this ctx that passed one (the ctx
+ *   keeps a copy; INVALID_ARG if there is none).  Rule levels already expanded for that sigma are
+ *   reused, so the preprocessing pass a1 is skipped - what a particle tracker wants, which asks
+ *   for the field of the same charges at one point after the other (L32).  bemcub_set_elements
+ *   drops the kept sigma; so does a bemcub_eval_linear call.
  * Calls with m <= 32 take a different route on the device: elements are spread over the lanes,
  *   every (element, point) pair gets its rule from its own distance ratio (allow_upgrade has no
- *   effect), and the lanes' partial sums are combined with warp shuffles.
+ *   effect), the lanes' partial sums are combined with warp shuffles, and the Gaussian points
+ *   are computed on the fly from the vertices (L218) - such a call has no preprocessing pass.
  * m = 0 is a no-op.  Asynchronous. */
 int bemcub_eval(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
                 int64_t m, const double* field_pts, double* out_phi, double* out_E, int precision);

@@ -72,6 +72,38 @@ __global__ void geometry_kernel(int64_t n, const uint8_t* __restrict__ type, con
   }
 }
 
+__device__ __forceinline__ int rule_npts_of(int type, int level) {
+  return type == 0 ? (c_tri_off[level + 1] - c_tri_off[level]) : (c_rect_off[level + 1] - c_rect_off[level]);
+}
+
+// Point i of rule `level` on one element: Q_i by Eq. 3.3 (triangle, L109) or Eq. 3.2 (rectangle,
+// L103) and q_i = w_i q sigma(Q_i)/sigma  (q = sigma A; sv != nullptr: linear density, L275).
+// The ONE place this arithmetic lives: the preprocessing kernel and the on-the-fly kernel call it,
+// so precomputed and on-the-fly points are bit-identical (L218 vs L246).
+__device__ __forceinline__ bool rule_point(int t, int level, int i, const double* __restrict__ v, const double4 c, double q,
+                                           const double* __restrict__ sv, double4& out) {
+  if (t == 0) {
+    const double* r = c_tri_tab + 4 * (c_tri_off[level] + i);
+    const double la = r[0], lb = r[1], lc = r[2];
+    // Eq. 3.3: Q = lambda_A A + lambda_B B + lambda_C C
+    out.x = fma(lc, v[6], fma(lb, v[3], la * v[0]));
+    out.y = fma(lc, v[7], fma(lb, v[4], la * v[1]));
+    out.z = fma(lc, v[8], fma(lb, v[5], la * v[2]));
+    const double sq = sv ? fma(lc, sv[2], fma(lb, sv[1], la * sv[0])) : 1.0;
+    out.w = r[3] * q * sq;
+  } else {
+    const double* r = c_rect_tab + 4 * (c_rect_off[level] + i);
+    const double xs = 0.5 * r[0], ys = 0.5 * r[1];
+    // Eq. 3.2: Q = Q_cen + (a/2) x u_x + (b/2) y u_y, with a u_x = P1 - P0 and b u_y = P3 - P0
+    out.x = fma(ys, v[6] - v[0], fma(xs, v[3] - v[0], c.x));
+    out.y = fma(ys, v[7] - v[1], fma(xs, v[4] - v[1], c.y));
+    out.z = fma(ys, v[8] - v[2], fma(xs, v[5] - v[2], c.z));
+    const double sq = sv ? fma(0.5 + ys, sv[2] - sv[0], fma(0.5 + xs, sv[1] - sv[0], sv[0])) : 1.0;
+    out.w = r[2] * q * sq;
+  }
+  return true;
+}
+
 template <typename T> struct Point4;
 template <> struct Point4<double> { typedef double4 type; };
 template <> struct Point4<float> { typedef float4 type; };
@@ -101,36 +133,10 @@ __global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* _
   const double* v = verts + 9 * e;
   const double q = (sigma ? sigma[e] : 1.0) * area[e];  // q = sigma A (L143); with sigma_v: q = A
   const double* sv = sigma_v ? sigma_v + 3 * e : nullptr;
-  if (t == 0) {
-    const int N = c_tri_off[level + 1] - c_tri_off[level];
-    if (i < N) {
-      const double* r = c_tri_tab + 4 * (c_tri_off[level] + i);
-      const double la = r[0], lb = r[1], lc = r[2];
-      // Eq. 3.3: Q = lambda_A A + lambda_B B + lambda_C C
-      const double x = fma(lc, v[6], fma(lb, v[3], la * v[0]));
-      const double y = fma(lc, v[7], fma(lb, v[4], la * v[1]));
-      const double z = fma(lc, v[8], fma(lb, v[5], la * v[2]));
-      const double sq = sv ? fma(lc, sv[2], fma(lb, sv[1], la * sv[0])) : 1.0;
-      store_point(out + idx, x, y, z, r[3] * q * sq);
-      return;
-    }
-  } else {
-    const int N = c_rect_off[level + 1] - c_rect_off[level];
-    if (i < N) {
-      const double* r = c_rect_tab + 4 * (c_rect_off[level] + i);
-      const double4 c = cenL[e];
-      const double xs = 0.5 * r[0], ys = 0.5 * r[1];
-      // Eq. 3.2: Q = Q_cen + (a/2) x u_x + (b/2) y u_y, with a u_x = P1 - P0 and b u_y = P3 - P0
-      const double x = fma(ys, v[6] - v[0], fma(xs, v[3] - v[0], c.x));
-      const double y = fma(ys, v[7] - v[1], fma(xs, v[4] - v[1], c.y));
-      const double z = fma(ys, v[8] - v[2], fma(xs, v[5] - v[2], c.z));
-      const double sq = sv ? fma(0.5 + ys, sv[2] - sv[0], fma(0.5 + xs, sv[1] - sv[0], sv[0])) : 1.0;
-      store_point(out + idx, x, y, z, r[2] * q * sq);
-      return;
-    }
-  }
   const double4 c = cenL[e];
-  store_point(out + idx, c.x, c.y, c.z, 0.0);
+  double4 pt;
+  if (i < rule_npts_of(t, level) && rule_point(t, level, i, v, c, q, sv, pt)) store_point(out + idx, pt.x, pt.y, pt.z, pt.w);
+  else store_point(out + idx, c.x, c.y, c.z, 0.0);
 }
 
 // Step a6: sum the per-split partial results in split order and apply k = 1/(4 pi eps0) once

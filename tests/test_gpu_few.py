@@ -88,10 +88,22 @@ def test_sigma_null_reuses_the_charges_of_the_previous_call():
         torch.cuda.synchronize()
         assert abs(p1.item() - ref["phi"][j]) <= TOL_F64 * ref["Sphi"][j]
         assert np.max(np.abs(e1.cpu().numpy()[0] - ref["E"][j])) <= TOL_F64 * ref["SE"][j]
-    # a fixed rule whose level was not expanded by that call: refused; after a new mesh: refused
-    b.bemcub_eval(h, d_sigma, 1, None, m, d_all, phi, E, b.F64)
-    with pytest.raises(Exception):
-        b.bemcub_eval(h, None, 3, None, m, d_all, phi, E, b.F64)
+    # another rule with the kept sigma: its level is expanded on demand
+    b.bemcub_eval(h, None, 3, None, m, d_all, phi, E, b.F64)
+    torch.cuda.synchronize()
+    ref3 = oracle.evaluate(c["etype"], c["verts"], c["sigma"], pts, 3)
+    err = parity_errors(phi.cpu().numpy(), E.cpu().numpy(), ref3)
+    assert err["phi"] <= TOL_F64 and err["E"] <= TOL_F64, err
+    # few points with the kept sigma: on the fly (nothing expanded for level 0) and from kept points (level 3) agree with the oracle
+    for level in (0, 3):
+        p4 = torch.empty(4, dtype=torch.float64, device="cuda")
+        e4 = torch.empty((4, 3), dtype=torch.float64, device="cuda")
+        b.bemcub_eval(h, None, level, None, 4, d_all[:4].contiguous(), p4, e4, b.F64)
+        torch.cuda.synchronize()
+        r4 = oracle.evaluate(c["etype"], c["verts"], c["sigma"], pts[:4], level)
+        e = parity_errors(p4.cpu().numpy(), e4.cpu().numpy(), r4)
+        assert e["phi"] <= TOL_F64 and e["E"] <= TOL_F64, (level, e)
+    # a new mesh drops the kept sigma
     b.bemcub_set_elements(h, g.n, g.d_type, g.d_verts)
     with pytest.raises(Exception):
         b.bemcub_eval(h, None, 1, None, m, d_all, phi, E, b.F64)
