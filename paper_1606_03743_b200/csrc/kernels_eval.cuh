@@ -683,7 +683,7 @@ __device__ __forceinline__ double warp_sum_f64(double v) {
 // Table 4 compares it with precomputed points): no preprocessing pass, 121 instead of 260 bytes
 // read per element (reading precomputed points was measured 20 % slower here).
 template <int MODE>
-__global__ void __launch_bounds__(kFewWarps * 32) eval_few_kernel(const __grid_constant__ FewParams p) {
+__global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __grid_constant__ FewParams p) {
   __shared__ double red[kFewWarps][kFewM][4];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t j0 = (int64_t)blockIdx.y * kFewM;
