@@ -130,7 +130,7 @@ int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const d
  *   reused, so the preprocessing pass a1 is skipped - what a particle tracker wants, which asks
  *   for the field of the same charges at one point after the other (L32).  bemcub_set_elements
  *   drops the kept sigma; so does a bemcub_eval_linear call.
- * Calls with m <= 32 take a different route on the device: elements are spread over the lanes,
+ * Calls with m <= 64 take a different route on the device: elements are spread over the lanes,
  *   every (element, point) pair gets its rule from its own distance ratio (allow_upgrade has no
  *   effect), the lanes' partial sums are combined with warp shuffles, and the Gaussian points
  *   are computed on the fly from the vertices (L218) - such a call has no preprocessing pass.

@@ -595,7 +595,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     count_launch(c);
     CUDA_TRY(cudaGetLastError());
     mark(c, 2);
-    reduce_scale_kernel<<<1, 32, 0, c->stream>>>(m, blocks, m, (const double4*)c->partial.ptr, nullptr, coulomb_k(), nullptr,
+    reduce_scale_kernel<<<(unsigned)((m + 31) / 32), 32, 0, c->stream>>>(m, blocks, m, (const double4*)c->partial.ptr, nullptr, coulomb_k(), nullptr,
                                                  out_phi, out_E, nullptr);
     count_launch(c);
     CUDA_TRY(cudaGetLastError());

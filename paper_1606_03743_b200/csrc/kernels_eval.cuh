@@ -654,7 +654,7 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
 // of the lanes are combined with warp shuffles, then across the warps of the CTA; a6 adds the CTAs.
 // The pass is bound by reading every expanded point once (HBM), not by the FP64 pipe.
 constexpr int kFewM = 4;        // field points per pass (grid.y)
-constexpr int kFewMaxM = 32;    // above this the tiled kernels win (10^6 elements: 0.54 ms at m = 16 vs 1.4 ms tiled at m = 17)
+constexpr int kFewMaxM = 64;    // above this the tiled kernels win (10^6 elements: 1.4 ms at m = 64 either way; 2.9 ms tiled with a new sigma)
 constexpr int kFewWarps = 8;
 
 struct FewParams {

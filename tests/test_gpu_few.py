@@ -1,4 +1,4 @@
-"""-m gpu: the few-field-point path (m <= 32: elements across the lanes, per-pair rule choice, partial sums
+"""-m gpu: the few-field-point path (m <= 64: elements across the lanes, per-pair rule choice, partial sums
 combined with warp shuffles).  Per-pair choice means the result must match the per-pair oracle whatever
 allow_upgrade says, and the interaction counters must match it exactly."""
 from __future__ import annotations
@@ -13,9 +13,9 @@ from gpu_common import TOL_F64, Gpu, parity_errors
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("m", [1, 2, 3, 4, 5, 13, 16, 32])
+@pytest.mark.parametrize("m", [1, 2, 3, 4, 5, 13, 16, 32, 63, 64])
 def test_adaptive_few_points_incl_near_field(m):
-    c = synth.config4(scale=0.003, ntracks=7, npts_per_track=9)
+    c = synth.config4(scale=0.003, ntracks=8, npts_per_track=9)
     rng = np.random.default_rng(100 + m)
     pts = c["pts"][rng.choice(len(c["pts"]), m, replace=False)].copy()
     # pull one point close to the wall so that the analytic branch and N = 33 / 19 are exercised
@@ -57,7 +57,7 @@ def test_fixed_rule_few_points_mixed_mesh(level):
 
 
 def test_sigma_null_reuses_the_charges_of_the_previous_call():
-    c = synth.config4(scale=0.003, ntracks=7, npts_per_track=9)
+    c = synth.config4(scale=0.003, ntracks=12, npts_per_track=9)       # 108 points: the tiled path
     g = Gpu(c["etype"], c["verts"])
     torch, b = g.torch, g.b
     h = g.ctx.handle
