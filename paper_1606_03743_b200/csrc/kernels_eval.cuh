@@ -485,30 +485,32 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     {  // bounding sphere of the tile (clamped duplicates lie inside it by construction).  Points
        // with a non-finite coordinate are left out: their own result is NaN whatever the rule, and
        // they must not spoil the rule choice of the other points of the tile.
-      double lox = CUDART_INF, hix = -CUDART_INF, loy = CUDART_INF, hiy = -CUDART_INF, loz = CUDART_INF, hiz = -CUDART_INF;
+      // (fmin / fmax / warp_min / warp_max return the other operand when one is NaN, so a point is
+      // left out by turning its coordinates into NaN for this computation only)
+      const double nan = CUDART_NAN;
+      double lox = nan, hix = nan, loy = nan, hiy = nan, loz = nan, hiz = nan;
       int cntok = 0;
-      bool fin[R];
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         cntok += w.ok(r, lane) ? 1 : 0;
-        fin[r] = isfinite(w.px[r]) && isfinite(w.py[r]) && isfinite(w.pz[r]);
-        if (fin[r]) {
-          lox = fmin(lox, w.px[r]); hix = fmax(hix, w.px[r]);
-          loy = fmin(loy, w.py[r]); hiy = fmax(hiy, w.py[r]);
-          loz = fmin(loz, w.pz[r]); hiz = fmax(hiz, w.pz[r]);
-        }
+        const bool fin = isfinite(w.px[r]) && isfinite(w.py[r]) && isfinite(w.pz[r]);
+        const double bx = fin ? w.px[r] : nan, by = fin ? w.py[r] : nan, bz = fin ? w.pz[r] : nan;
+        lox = fmin(lox, bx); hix = fmax(hix, bx);
+        loy = fmin(loy, by); hiy = fmax(hiy, by);
+        loz = fmin(loz, bz); hiz = fmax(hiz, bz);
       }
       lox = warp_min(lox); hix = warp_max(hix);
       loy = warp_min(loy); hiy = warp_max(hiy);
       loz = warp_min(loz); hiz = warp_max(hiz);
-      const bool any_fin = lox <= hix;
+      const bool any_fin = lox <= hix;  // false if every point of the tile is non-finite (NaN compares false)
       const double cx = any_fin ? 0.5 * (lox + hix) : 0.0, cy = any_fin ? 0.5 * (loy + hiy) : 0.0,
                    cz = any_fin ? 0.5 * (loz + hiz) : 0.0;
       double d2 = 0.0;
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         const double dx = w.px[r] - cx, dy = w.py[r] - cy, dz = w.pz[r] - cz;
-        if (fin[r]) d2 = fmax(d2, dx * dx + dy * dy + dz * dz);
+        const double t = dx * dx + dy * dy + dz * dz;
+        d2 = fmax(d2, t <= 1e300 ? t : 0.0);  // a non-finite point (t = NaN or inf) does not widen the sphere
       }
       const double rho = sqrt(warp_max(d2));
       cntok = warp_sum(cntok);
