@@ -384,6 +384,14 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         rate, cores, sample, dt, k = oracle_rate(c, args, target_seconds=15.0)
         cpu = {"value": rate, "unit": UNIT if not is_matrix else "matrix entries/s", "cores": cores, "kind": "oracle",
                "sample": sample, "seconds": dt}
+        if not is_matrix:   # the paper's CPU numbers are single-threaded (Table 2): one thread on a smaller sample
+            import oracle
+            k1 = max(4, int(k / max(cores, 1) / 4))
+            idx1 = np.sort(np.random.default_rng(160603753).choice(m, min(k1, m), replace=False))
+            t0 = time.perf_counter()
+            oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx1], c["rule"], dr=oracle.default_policy(True),
+                            precision="double", nthreads=1)
+            cpu["value_single_thread"] = n * len(idx1) / (time.perf_counter() - t0)
 
     if rank == 0:
         line = {
