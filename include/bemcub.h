@@ -18,11 +18,12 @@
  * General conventions
  *   - Unless a parameter is marked HOST, every pointer is a DEVICE pointer owned by the caller
  *     (e.g. a PyTorch allocation) on the device given to bemcub_create.  The library never frees
- *     or keeps caller buffers; bemcub_set_elements copies what it needs into ctx-owned memory.
+ *     or keeps caller buffers; bemcub_set_elements copies what it needs into ctx-owned memory,
+ *     and bemcub_eval copies sigma (see "sigma == NULL" there).
  *   - All work is enqueued on the CUDA stream given to bemcub_create (NULL = legacy default
  *     stream).  bemcub_eval / bemcub_assemble* are asynchronous: results are valid once the caller
- *     has synchronised that stream.  bemcub_set_elements, the *_host calls and bemcub_fp64_peak
- *     synchronise internally.  (A call that has to grow ctx-owned scratch calls cudaMalloc.)
+ *     has synchronised that stream.  bemcub_set_elements, bemcub_solve, the *_host calls,
+ *     bemcub_fp64_peak and bemcub_inner_loop_rate synchronise internally.  (A call that has to grow ctx-owned scratch calls cudaMalloc.)
  *   - Every function returns BEMCUB_OK (0) or a negative error code; nothing throws or longjmps
  *     across the ABI.  There is no CPU fallback: without a usable CUDA device bemcub_create fails.
  *   - SI units: lengths m, sigma C/m^2, Phi V, E V/m.  eps0 = 8.8541878128e-12 F/m (CODATA 2018;
