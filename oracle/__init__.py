@@ -26,7 +26,9 @@ def build(force: bool = False) -> Path:
     """Compile liboracle.so with g++ (no CUDA)."""
     if not force and _SO.exists() and all(_SO.stat().st_mtime >= s.stat().st_mtime for s in _SRC):
         return _SO
-    cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-shared", "-fPIC",
+    # -ffp-contract=off: the double-typed rule decision forms D^2 with separately rounded products
+    # (DESIGN.md reading 8) on every host, also where the compiler would otherwise contract to FMAs
+    cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
            str(_SRC[0]), "-o", str(_SO)]
     subprocess.run(cmd, check=True, cwd=_HERE)
     return _SO
@@ -43,6 +45,7 @@ def lib() -> C.CDLL:
         L.orc_coulomb_k.restype = C.c_double
         L.orc_rule_monomial_residual.restype = C.c_double
         L.orc_points.restype = C.c_int64
+        L.orc_duffy_monomial_residual.restype = C.c_double
         _lib = L
     return _lib
 
@@ -122,8 +125,9 @@ def evaluate(etype, verts, sigma, pts, level: int, dr=None, levels_mask: int = A
     """Eq. 4.1 summed over all elements at every field point.
 
     level 0..4 = fixed rule (N = 4, 7, 12, 19|17, 33); level -1 = per-pair rule by distance
-    ratio with limits dr[2][5].  Returns dict(phi[m], E[m][3], Sphi[m], SE[m][, npi[m]]) where
-    Sphi = k*sum|q_i|/r_i and SE = k*sum|q_i|/r_i^2 are the parity denominators.
+    ratio with limits dr[2][5].  Returns dict(phi[m], E[m][3], Sphi[m], SE[m][, npi[m], nana[m]]) where
+    Sphi = k*sum|q_i|/r_i and SE = k*sum|q_i|/r_i^2 are the parity denominators, npi the point-charge
+    interactions and nana the analytic pairs each field point used (want_counts).
     """
     etype = np.ascontiguousarray(etype, dtype=np.uint8)
     verts, sigma, pts = _f64(verts), _f64(sigma), _f64(pts)
@@ -131,15 +135,18 @@ def evaluate(etype, verts, sigma, pts, level: int, dr=None, levels_mask: int = A
     assert verts.shape == (n, 3, 3) and sigma.shape == (n,) and pts.shape == (m, 3)
     phi, E, Sphi, SE = np.zeros(m), np.zeros((m, 3)), np.zeros(m), np.zeros(m)
     npi = np.zeros(m, dtype=np.int64) if want_counts else None
+    nana = np.zeros(m, dtype=np.int64) if want_counts else None
     drp = None if dr is None else _f64(dr)
     rc = lib().orc_eval(C.c_int64(n), _p(etype, C.c_uint8), _p(verts), _p(sigma), level,
                         _p(drp), levels_mask, C.c_int64(m), _p(pts), _p(phi), _p(E), _p(Sphi),
-                        _p(SE), _p(npi, C.c_int64), 0 if precision == "long double" else 1, nthreads)
+                        _p(SE), _p(npi, C.c_int64), _p(nana, C.c_int64),
+                        0 if precision == "long double" else 1, nthreads)
     if rc:
         raise ValueError(f"orc_eval rc={rc}")
     out = dict(phi=phi, E=E, Sphi=Sphi, SE=SE)
     if want_counts:
         out["npi"] = npi
+        out["nana"] = nana
     return out
 
 
@@ -184,6 +191,45 @@ def evaluate_linear(etype, verts, sigma_v, pts, level: int, dr=None, levels_mask
     if rc:
         raise ValueError(f"orc_eval_linear rc={rc}")
     return dict(phi=phi, E=E, Sphi=Sphi, SE=SE)
+
+
+DUFFY = 8             # method code of the Duffy-mapped rectangle rule of level l: DUFFY + l
+
+
+def evaluate_pairs(etype, verts, pts, method: int, sigma=None, dr=None, levels_mask: int = ALL_LEVELS,
+                   precision: str = "long double"):
+    """Element k seen from field point k (no sum over elements; PAPER.md L193-196 item a, the unit of
+    the accuracy protocol of L68/L149).  method 0..4 = cubature level, 5 = analytic closed form,
+    -1 = by distance ratio (dr[2][5]), DUFFY + l = rectangle rule of level l (Duffy-mapped on
+    triangles, L163-169).  Returns dict(phi[K], E[K][3], Sphi[K], SE[K], used[K])."""
+    etype = np.ascontiguousarray(etype, dtype=np.uint8)
+    verts, pts = _f64(verts), _f64(pts)
+    K = len(etype)
+    assert verts.shape == (K, 3, 3) and pts.shape == (K, 3)
+    sg = None if sigma is None else _f64(sigma)
+    phi, E, Sphi, SE = np.zeros(K), np.zeros((K, 3)), np.zeros(K), np.zeros(K)
+    used = np.zeros(K, dtype=np.uint8)
+    drp = None if dr is None else _f64(dr)
+    rc = lib().orc_eval_pairs(C.c_int64(K), _p(etype, C.c_uint8), _p(verts), _p(sg), method, _p(drp), levels_mask,
+                              _p(pts), _p(phi), _p(E), _p(Sphi), _p(SE), _p(used, C.c_uint8),
+                              0 if precision == "long double" else 1)
+    if rc:
+        raise ValueError(f"orc_eval_pairs rc={rc}")
+    return dict(phi=phi, E=E, Sphi=Sphi, SE=SE, used=used)
+
+
+def duffy_nodes(level: int):
+    """Duffy-mapped rectangle rule on the reference triangle: (bary[N][3], w[N])."""
+    n, _ = rule_info(1, level)
+    bary, w = np.zeros((n, 3)), np.zeros(n)
+    rc = lib().orc_duffy_nodes(level, _p(bary), _p(w))
+    if rc:
+        raise ValueError(f"orc_duffy_nodes rc={rc}")
+    return bary, w
+
+
+def duffy_monomial_residual(level: int, a: int, b: int) -> float:
+    return lib().orc_duffy_monomial_residual(level, a, b)
 
 
 def _single(fn, etype, verts9, P, *extra):

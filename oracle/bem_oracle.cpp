@@ -13,8 +13,9 @@
 // Every function cites the passage of /root/reference/PAPER.md it follows.  Arithmetic is
 // long double (x87 80-bit) in the parity instantiation; a double instantiation of the very
 // same template is what bench.py times as the CPU baseline.  No blocking, fusion or
-// reordering beyond the paper's statement: per field point, elements in index order, the
-// rule's points in table order.
+// reordering beyond the paper's statement: geometry (centroid, area, L) once per element, then
+// one field point after the other, elements in index order, the rule's points in table order,
+// mapped onto the element for every (element, field point) pair anew (L218).
 //
 // Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`):
 //   tables      : sum w = 1, exact monomial integrals up to the stated degree, failure at d+1
@@ -24,9 +25,13 @@
 //                 E = -grad Phi by central differences
 //   analytic    : closed forms (square centre, equilateral centroid, on-axis rectangle),
 //                 GL2 16 vs 32, long-double adaptive quadrature on tiny inputs
+//   pairs       : the single-element integrator (element k seen from point k) against the summed
+//                 path on one-element meshes; Duffy-mapped rectangle rules: sum w' = 1, exact
+//                 triangle monomials up to (D-1)/2 and not beyond, the printed ~1e-8 at DR = 100 (L169)
+//   policy      : the shipped Phi+E distance-ratio limits by the paper's random-element protocol
 //   KATRIN Table 1 numbers: parity unpinned (meshes not available).
 //
-// Build: g++ -O2 -std=c++17 -fopenmp -shared -fPIC bem_oracle.cpp -o liboracle.so
+// Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC bem_oracle.cpp -o liboracle.so
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -138,6 +143,31 @@ void element_points(const Geom<T>& g, int level, std::vector<Pt<T>>& out) {
             out.push_back({g.cen.x + x * g.hx.x + y * g.hy.x, g.cen.y + x * g.hx.y + y * g.hy.y,
                            g.cen.z + x * g.hx.z + y * g.hy.z, (T)nd.w});
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// Duffy variant (Sec. 4): "a triangle can be mapped into a rectangle by the Duffy
+// transformation, therefore the numerical integration over a triangle by Gaussian cubature can also
+// be done by using the Duffy transformation in conjunction with the Gaussian cubature formulas for
+// rectangles of App. B".  The paper prints no formula (Refs. [64,69]); reading 20 takes
+// the classical map that collapses one edge of the square onto vertex A:
+//     Q(u,v) = A + u [ (B - A) + v (C - B) ],  (u,v) in [0,1]^2,   dS = 2 area u du dv,
+// with the collapsing coordinate along the rule's y axis: u = (1+y)/2, v = (1+x)/2 for a node
+// (x,y) of the rectangle rule.  (Tables B2, B4, B5 are not symmetric under x <-> y; of the two
+// assignments this one reproduces the error the paper prints for the 7-point rule at DR = 100,
+// "about 1e-8" (L169): 6e-9 against 7e-11 for the other.)  Relative to the triangle area the
+// node weight becomes w' = 2 u w = (1 + y) w  (sum w' = 1 because the rule integrates y exactly).
+// A triangle polynomial of degree d becomes a polynomial of degree up to 2d in (u,v), times the
+// Jacobian u: exactness is guaranteed for d <= (D - 1)/2 only, D the degree of the rectangle rule.
+template <class T>
+void element_points_duffy(const Geom<T>& g, int level, std::vector<Pt<T>>& out) {
+    out.clear();
+    const V3<T> AB = sub(g.v[1], g.v[0]), BC = sub(g.v[2], g.v[1]);
+    for (const RectNode& nd : rect_rule(level)) {
+        const T u = ((T)1 + (T)nd.y) / (T)2, v = ((T)1 + (T)nd.x) / (T)2;
+        out.push_back({g.v[0].x + u * (AB.x + v * BC.x), g.v[0].y + u * (AB.y + v * BC.y),
+                       g.v[0].z + u * (AB.z + v * BC.z), ((T)1 + (T)nd.y) * (T)nd.w});
     }
 }
 
@@ -361,75 +391,65 @@ static int choose_level(double D2, double L, const double* dr5, int levels_mask)
 template <class T>
 int eval_impl(int64_t n, const uint8_t* etype, const double* verts, const double* sigma, int level,
               const double* dr, int levels_mask, int64_t m, const double* pts, double* phi, double* E,
-              double* Sphi, double* SE, int64_t* npi, int nthreads) {
+              double* Sphi, double* SE, int64_t* npi, int64_t* nana, int nthreads) {
     if (n < 0 || m < 0) return ERR_INVALID;
     if (level < -1 || level > 4) return ERR_BAD_RULE;
     if (level == -1 && (!dr || (levels_mask & 63) == 0)) return ERR_INVALID;
-    // validate geometry once
+    // step 2 (geometry) once per element
+    std::vector<Geom<T>> G((size_t)n);
     for (int64_t e = 0; e < n; ++e) {
-        Geom<T> g;
-        int rc = make_geom<T>(etype[e], verts + 9 * e, g);
+        int rc = make_geom<T>(etype[e], verts + 9 * e, G[e]);
         if (rc) return rc;
     }
-    const int64_t BS = 32;
-    const int64_t nblocks = (m + BS - 1) / BS;
     const T k = (T)coulomb_k();
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
 #endif
+    // steps 3-5, one field point after the other: elements in index order, the rule's points in table order
 #pragma omp parallel for schedule(dynamic, 1)
-    for (int64_t b = 0; b < nblocks; ++b) {
-        const int64_t j0 = b * BS, j1 = std::min(m, j0 + BS);
-        T aphi[BS], aex[BS], aey[BS], aez[BS], asphi[BS], ase[BS];
-        int64_t cnt[BS];
-        for (int64_t j = 0; j < BS; ++j) { aphi[j] = aex[j] = aey[j] = aez[j] = asphi[j] = ase[j] = 0; cnt[j] = 0; }
-        std::vector<Pt<T>> cache[5];
+    for (int64_t j = 0; j < m; ++j) {
+        const V3<T> P{(T)pts[3 * j], (T)pts[3 * j + 1], (T)pts[3 * j + 2]};
+        T aphi = 0, aex = 0, aey = 0, aez = 0, asphi = 0, ase = 0;
+        int64_t cnt = 0, cana = 0;
+        std::vector<Pt<T>> pv;
         for (int64_t e = 0; e < n; ++e) {
-            Geom<T> g;
-            make_geom<T>(etype[e], verts + 9 * e, g);
-            bool have[5] = {false, false, false, false, false};
-            const T q = (T)sigma[e] * g.area;               // q = sigma * A (L143)
-            const double cx = (double)g.cen.x, cy = (double)g.cen.y, cz = (double)g.cen.z, Ld = (double)g.L;
-            for (int64_t j = j0; j < j1; ++j) {
-                const V3<T> P{(T)pts[3 * j], (T)pts[3 * j + 1], (T)pts[3 * j + 2]};
-                int lv = level;
-                if (level == -1) {
-                    double dx = pts[3 * j] - cx, dy = pts[3 * j + 1] - cy, dz = pts[3 * j + 2] - cz;
-                    lv = choose_level(dx * dx + dy * dy + dz * dz, Ld, dr + 5 * g.type, levels_mask);
-                }
-                const int jj = (int)(j - j0);
-                if (lv == 5) {
-                    T Ip; V3<T> Ie;
-                    analytic_integrals<T>(g, P, Ip, Ie);
-                    const T s = (T)sigma[e];
-                    aphi[jj] += s * Ip; aex[jj] += s * Ie.x; aey[jj] += s * Ie.y; aez[jj] += s * Ie.z;
-                    asphi[jj] += tabs(s * Ip);
-                    ase[jj] += tabs(s) * norm(Ie);
-                    continue;
-                }
-                if (!have[lv]) { element_points<T>(g, lv, cache[lv]); have[lv] = true; }
-                for (const Pt<T>& p : cache[lv]) {
-                    const T qi = p.w * q;                    // q_i = w_i q (L143)
-                    const T dx = P.x - p.x, dy = P.y - p.y, dz = P.z - p.z;
-                    const T r2 = dx * dx + dy * dy + dz * dz;
-                    const T inv = (T)1 / tsqrt<T>(r2);       // one square root, one division (L46)
-                    const T inv3 = inv * inv * inv;
-                    aphi[jj] += qi * inv;
-                    aex[jj] += qi * dx * inv3; aey[jj] += qi * dy * inv3; aez[jj] += qi * dz * inv3;
-                    asphi[jj] += tabs(qi) * inv;
-                    ase[jj] += tabs(qi) * inv * inv;
-                }
-                cnt[jj] += (int64_t)cache[lv].size();
+            const Geom<T>& g = G[e];
+            int lv = level;
+            if (level == -1) {
+                const double dx = pts[3 * j] - (double)g.cen.x, dy = pts[3 * j + 1] - (double)g.cen.y, dz = pts[3 * j + 2] - (double)g.cen.z;
+                lv = choose_level(dx * dx + dy * dy + dz * dz, (double)g.L, dr + 5 * g.type, levels_mask);
             }
+            if (lv == 5) {
+                T Ip; V3<T> Ie;
+                analytic_integrals<T>(g, P, Ip, Ie);
+                const T s = (T)sigma[e];
+                aphi += s * Ip; aex += s * Ie.x; aey += s * Ie.y; aez += s * Ie.z;
+                asphi += tabs(s * Ip);
+                ase += tabs(s) * norm(Ie);
+                ++cana;
+                continue;
+            }
+            element_points<T>(g, lv, pv);
+            const T q = (T)sigma[e] * g.area;               // q = sigma * A (L143)
+            for (const Pt<T>& p : pv) {
+                const T qi = p.w * q;                        // q_i = w_i q (L143)
+                const T dx = P.x - p.x, dy = P.y - p.y, dz = P.z - p.z;
+                const T r2 = dx * dx + dy * dy + dz * dz;
+                const T inv = (T)1 / tsqrt<T>(r2);           // one square root, one division (L46)
+                const T inv3 = inv * inv * inv;
+                aphi += qi * inv;
+                aex += qi * dx * inv3; aey += qi * dy * inv3; aez += qi * dz * inv3;
+                asphi += tabs(qi) * inv;
+                ase += tabs(qi) * inv * inv;
+            }
+            cnt += (int64_t)pv.size();
         }
-        for (int64_t j = j0; j < j1; ++j) {
-            const int jj = (int)(j - j0);
-            if (phi) phi[j] = (double)(k * aphi[jj]);
-            if (E) { E[3 * j] = (double)(k * aex[jj]); E[3 * j + 1] = (double)(k * aey[jj]); E[3 * j + 2] = (double)(k * aez[jj]); }
-            if (Sphi) Sphi[j] = (double)(k * asphi[jj]);
-            if (SE) SE[j] = (double)(k * ase[jj]);
-            if (npi) npi[j] = cnt[jj];
-        }
+        if (phi) phi[j] = (double)(k * aphi);
+        if (E) { E[3 * j] = (double)(k * aex); E[3 * j + 1] = (double)(k * aey); E[3 * j + 2] = (double)(k * aez); }
+        if (Sphi) Sphi[j] = (double)(k * asphi);
+        if (SE) SE[j] = (double)(k * ase);
+        if (npi) npi[j] = cnt;
+        if (nana) nana[j] = cana;
     }
     return ERR_OK;
 }
@@ -551,6 +571,69 @@ int linear_impl(int64_t n, const uint8_t* etype, const double* verts, const doub
     return ERR_OK;
 }
 
+// ---------------------------------------------------------------------------------------
+// The single-element boundary integrator (the paper's innermost layer, L193-196 item a): element k
+// seen from field point k, k < K, no sum over elements.  This is the unit of the paper's accuracy
+// protocol (L68, L149: 1000 random elements and directions per distance ratio).
+// method: 0..4 cubature level (Eq. 4.1 with the element's own rule); 5 the analytic closed form;
+//         -1 the distance-ratio choice (dr, levels_mask); 8+l (l = 0..4) the rectangle rule of
+//         level l - on a triangle through the Duffy map above, on a rectangle as it is.
+// used[k] (may be null) = what was evaluated: 0..4, 5 = analytic.
+template <class T>
+int pairs_impl(int64_t K, const uint8_t* etype, const double* verts, const double* sigma, int method,
+               const double* dr, int levels_mask, const double* pts, double* phi, double* E, double* Sphi,
+               double* SE, uint8_t* used) {
+    if (K < 0) return ERR_INVALID;
+    if (!(method >= -1 && method <= 5) && !(method >= 8 && method <= 12)) return ERR_BAD_RULE;
+    if (method == -1 && (!dr || (levels_mask & 63) == 0)) return ERR_INVALID;
+    for (int64_t e = 0; e < K; ++e) {
+        Geom<T> g;
+        int rc = make_geom<T>(etype[e], verts + 9 * e, g);
+        if (rc) return rc;
+    }
+    const T k = (T)coulomb_k();
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < K; ++e) {
+        Geom<T> g;
+        make_geom<T>(etype[e], verts + 9 * e, g);
+        const V3<T> P{(T)pts[3 * e], (T)pts[3 * e + 1], (T)pts[3 * e + 2]};
+        const T sg = sigma ? (T)sigma[e] : (T)1;
+        int lv = method;
+        if (method == -1) {
+            const double dx = pts[3 * e] - (double)g.cen.x, dy = pts[3 * e + 1] - (double)g.cen.y, dz = pts[3 * e + 2] - (double)g.cen.z;
+            lv = choose_level(dx * dx + dy * dy + dz * dz, (double)g.L, dr + 5 * g.type, levels_mask);
+        }
+        T aphi = 0, ax = 0, ay = 0, az = 0, sphi = 0, se = 0;
+        if (lv == 5) {
+            T Ip; V3<T> Ie;
+            analytic_integrals<T>(g, P, Ip, Ie);
+            aphi = sg * Ip; ax = sg * Ie.x; ay = sg * Ie.y; az = sg * Ie.z;
+            sphi = tabs(sg * Ip); se = tabs(sg) * norm(Ie);
+        } else {
+            std::vector<Pt<T>> pv;
+            if (lv >= 8 && g.type == TRI) element_points_duffy<T>(g, lv - 8, pv);
+            else element_points<T>(g, lv >= 8 ? lv - 8 : lv, pv);
+            const T q = sg * g.area;
+            for (const Pt<T>& p : pv) {
+                const T qi = p.w * q;
+                const T dx = P.x - p.x, dy = P.y - p.y, dz = P.z - p.z;
+                const T inv = (T)1 / tsqrt<T>(dx * dx + dy * dy + dz * dz);
+                const T inv3 = inv * inv * inv;
+                aphi += qi * inv;
+                ax += qi * dx * inv3; ay += qi * dy * inv3; az += qi * dz * inv3;
+                sphi += tabs(qi) * inv;
+                se += tabs(qi) * inv * inv;
+            }
+        }
+        if (phi) phi[e] = (double)(k * aphi);
+        if (E) { E[3 * e] = (double)(k * ax); E[3 * e + 1] = (double)(k * ay); E[3 * e + 2] = (double)(k * az); }
+        if (Sphi) Sphi[e] = (double)(k * sphi);
+        if (SE) SE[e] = (double)(k * se);
+        if (used) used[e] = (uint8_t)(lv >= 8 ? lv - 8 : lv);
+    }
+    return ERR_OK;
+}
+
 }  // namespace orc
 
 using namespace orc;
@@ -649,12 +732,13 @@ int orc_default_policy(double* dr, int want_field) {
 int orc_choose_level(double D2, double L, const double* dr5, int levels_mask) { return choose_level(D2, L, dr5, levels_mask); }
 
 // precision: 0 = long double (parity), 1 = double (timed CPU baseline).  level -1 = adaptive.
+// npi[m] / nana[m] (may be null): point-charge interactions / analytic pairs used per field point.
 int orc_eval(int64_t n, const uint8_t* etype, const double* verts, const double* sigma, int level,
              const double* dr, int levels_mask, int64_t m, const double* pts, double* phi, double* E,
-             double* Sphi, double* SE, int64_t* npi, int precision, int nthreads) {
+             double* Sphi, double* SE, int64_t* npi, int64_t* nana, int precision, int nthreads) {
     if (precision == 0)
-        return eval_impl<long double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
-    return eval_impl<double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nthreads);
+        return eval_impl<long double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nana, nthreads);
+    return eval_impl<double>(n, etype, verts, sigma, level, dr, levels_mask, m, pts, phi, E, Sphi, SE, npi, nana, nthreads);
 }
 
 // Linear sigma over each element (L275), long double, cubature levels only.
@@ -761,6 +845,46 @@ int orc_assemble_rows(int64_t n, const uint8_t* etype, const double* verts, cons
         }
     }
     return ERR_OK;
+}
+
+// Element k seen from field point k (no sum): see pairs_impl.  precision 0 = long double, 1 = double.
+int orc_eval_pairs(int64_t K, const uint8_t* etype, const double* verts, const double* sigma, int method,
+                   const double* dr, int levels_mask, const double* pts, double* phi, double* E, double* Sphi,
+                   double* SE, uint8_t* used, int precision) {
+    if (precision == 0) return pairs_impl<long double>(K, etype, verts, sigma, method, dr, levels_mask, pts, phi, E, Sphi, SE, used);
+    return pairs_impl<double>(K, etype, verts, sigma, method, dr, levels_mask, pts, phi, E, Sphi, SE, used);
+}
+
+// Duffy-mapped rectangle rule of `level` on the reference triangle A=(0,0), B=(1,0), C=(0,1):
+// bary[N][3] = (lambda_A, lambda_B, lambda_C) of each node, w[N] = its weight relative to the area.
+int orc_duffy_nodes(int level, double* bary, double* w) {
+    if (level < 0 || level > 4) return ERR_BAD_RULE;
+    const double ref[9] = {0, 0, 0, 1, 0, 0, 0, 1, 0};
+    Geom<long double> g;
+    make_geom<long double>(TRI, ref, g);
+    std::vector<Pt<long double>> p;
+    element_points_duffy<long double>(g, level, p);
+    for (size_t i = 0; i < p.size(); ++i) {
+        bary[3 * i] = (double)(1 - p[i].x - p[i].y); bary[3 * i + 1] = (double)p[i].x; bary[3 * i + 2] = (double)p[i].y;
+        w[i] = (double)p[i].w;
+    }
+    return ERR_OK;
+}
+
+// sum_i w'_i x_i^a y_i^b - a! b! 2/(a+b+2)!  for the Duffy-mapped rule on the reference triangle (long double).
+double orc_duffy_monomial_residual(int level, int a, int b) {
+    const double ref[9] = {0, 0, 0, 1, 0, 0, 0, 1, 0};
+    Geom<long double> g;
+    make_geom<long double>(TRI, ref, g);
+    std::vector<Pt<long double>> p;
+    element_points_duffy<long double>(g, level, p);
+    long double s = 0;
+    for (auto& q : p) s += q.w * powl(q.x, a) * powl(q.y, b);
+    long double num = 2, den = 1;
+    for (int i = 2; i <= a; ++i) num *= i;
+    for (int i = 2; i <= b; ++i) num *= i;
+    for (int i = 2; i <= a + b + 2; ++i) den *= i;
+    return (double)(s - num / den);
 }
 
 int orc_num_threads() {

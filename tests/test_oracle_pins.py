@@ -401,6 +401,45 @@ def test_dr_limits_reach_printed_accuracy_level():
         assert np.mean(errs_close) > 20 * np.mean(errs)
 
 
+@pytest.mark.parametrize("kind", [TRI, RECT])
+def test_field_dr_limits_by_the_papers_protocol(kind):
+    """Pin of the shipped Phi+E limits (reading 7; L159: for the field the limits are
+    'slightly higher', and 'if both the potential and the field has to be computed ... one should use
+    the limits defined by the field').  The paper's protocol (L68, L149): 1000 random elements with
+    corners in the unit cube, a random direction each, mean of err(Phi) = |dPhi/Phi| and err(E) =
+    sum_j |dE_j| / |E| (L80), double arithmetic for the rule, exact reference in long double (closed
+    form below DR = 12, the 33-point rule above).  At every shipped limit the rule that takes over
+    there is at the paper's 2e-15 level for the FIELD as well (<= 3e-15; potential <= 5e-16), and the
+    limits are not slack: 40 % nearer every rule is above that level, 20 % nearer all but the
+    rectangle N = 4 rule."""
+    fdr = oracle.default_policy(True)[kind]
+    n = 1000
+    et, verts = synth.random_elements(kind, n, seed=1234 + kind)
+    cen, _, L = oracle.geometry(et, verts)
+    dirs = synth.isotropic_directions(np.random.default_rng(77 + kind), n)
+
+    def mean_errors(level, ratio):
+        P = cen + dirs * (ratio * L)[:, None]
+        ref = oracle.evaluate_pairs(et, verts, P, 5 if ratio < 12.0 else 4)
+        r = oracle.evaluate_pairs(et, verts, P, level, precision="double")
+        e_phi = np.abs(r["phi"] - ref["phi"]) / np.abs(ref["phi"])
+        e_E = np.abs(r["E"] - ref["E"]).sum(axis=1) / np.linalg.norm(ref["E"], axis=1)
+        return float(e_phi.mean()), float(e_E.mean())
+
+    for band, level in ((4, 0), (3, 1), (2, 2), (1, 3), (0, 4)):       # dr[band] = lower end of `level`'s range
+        lim = float(fdr[band])
+        e_phi, e_E = mean_errors(level, lim)
+        assert e_phi <= 5e-16 and e_E <= 3e-15, (kind, level, lim, e_phi, e_E)
+        _, e_E_06 = mean_errors(level, 0.6 * lim)
+        assert e_E_06 > 3e-15, (kind, level, 0.6 * lim, e_E_06)
+        if not (kind == RECT and level == 0):
+            _, e_E_08 = mean_errors(level, 0.8 * lim)
+            assert e_E_08 > 3e-15, (kind, level, 0.8 * lim, e_E_08)
+    # and they are the same numbers the header of the C ABI promises
+    expect = {TRI: [4, 10, 25, 100, 2000], RECT: [6, 15, 40, 150, 3000]}[kind]
+    assert list(fdr) == expect
+
+
 def test_adaptive_sum_uses_per_pair_rule():
     """Adaptive evaluation = sum over elements of the fixed-rule value at the level the policy
     picks per pair; point-interaction counts follow; the analytic branch is taken below the
