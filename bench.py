@@ -1,15 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the bemcub hot path on B200 (driver contract: one JSON line on rank 0).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4|cfg2|cfg3]
-                    [--scale S]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfg4|cfg1|cfg2|cfg3|cfg5|solve|table3|accuracy] [--scale S] [--no-secondary]
 
 Metric (BASELINE.json): FP64 Phi+E element.point interactions/s.  One step = one pass of the whole
 hot path (a1 preprocessing, a2 rule binning, a3 point-charge sum, a4 analytic near field, a6
 reduction + scaling) over one batch of synthetic input.  Default workload =
 config 4 (`configs[3]`, "the 10^6-element config" the north_star target is quoted on): 8e5
-rectangles + 2e5 triangles, 10^6 helical-track field points, distance-ratio-adaptive rules.
-`--workload cfg2 / cfg3` and `--scale` exist for profiling smaller cases; they are not bench lines.
+rectangles + 2e5 triangles, 10^6 helical-track field points, distance-ratio-adaptive rules.  The
+default line also carries a `secondary` list: short device-timed runs of the other configs (matrix
+fill of config 3, configs 1, 2, 5), each with its own roofline, clocks and oracle timing.
+The other `--workload` values time one workload alone (profiling); `--workload accuracy` runs the
+paper's random-element accuracy study (Figs. 8-10) through bemcub_eval_pairs and writes its
+table to `--out`.
 
 Multi-GPU (torchrun): field points shard across ranks with no data-path collective; every rank
 holds the full mesh and its own 10^6 field points (weak scaling).
@@ -33,11 +37,14 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-FLOP_PER_INTERACTION = 26      # 8 DFMA + 6 DMUL + 4 DADD per point charge, Phi + E
-FLOP_PER_INTERACTION_PHI = 18  # 6 DFMA + 3 DMUL + 3 DADD, potential only (matrix fill)
+FLOP_PER_INTERACTION = 26       # 8 DFMA + 6 DMUL + 4 DADD per point charge, Phi + E
+FLOP_PER_INTERACTION_PHI = 18   # 6 DFMA + 3 DMUL + 3 DADD, potential only (matrix fill)
 FLOP_PER_INTERACTION_GRAD = 41  # + 5 DFMA + 4 DMUL + 1 DADD for the gradient sums (28 FP64 instructions)
+FP64_LANES_PER_SM = 64          # B200: one FP64 warp instruction per scheduler every 2 cycles (profiles/r2_issue_model.md)
 METRIC = "FP64 Phi+E element.point interactions/s"
 UNIT = "element.point interactions/s"
+# ncu counter of the committed capture of the bench's own launch configuration (not measured by this run)
+NCU_PIPE = {"cfg4": ("profiles/r2_cfg4_full_eval_adaptive_counters.csv", "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed")}
 
 
 def parse_args():
@@ -46,14 +53,17 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg4", "cfg2", "cfg3", "solve", "table3"])
+    ap.add_argument("--workload", default="cfg4",
+                    choices=["cfg4", "cfg1", "cfg2", "cfg3", "cfg5", "solve", "table3", "accuracy"])
     ap.add_argument("--scale", type=float, default=1.0, help="config-4 size factor (profiling only)")
-    ap.add_argument("--rule", type=int, default=1, help="fixed rule level of --workload cfg2")
-    ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="--workload cfg2 only")
+    ap.add_argument("--rule", type=int, default=1, help="fixed rule level of --workload cfg2 / cfg5 / table3 (-1 = adaptive)")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="fixed-rule workloads only")
     ap.add_argument("--gradient", action="store_true",
                     help="also compute the field gradient (bemcub_eval_gradient; cubature levels only) - not the bench line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="default workload only: skip the secondary block")
+    ap.add_argument("--out", default=None, help="--workload accuracy: text file for the tables")
     return ap.parse_args()
 
 
@@ -65,8 +75,9 @@ class ClockSampler:
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, gpu_index: int):
+    def __init__(self, gpu_index: int, period_ms: int = 200):
         self.gpu = gpu_index
+        self.period = period_ms
         self.proc = None
         self.lines = []
         self.thread = None
@@ -74,7 +85,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", str(self.period),
                  "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -115,10 +126,10 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------------------------
-def make_workload(args, rank: int):
+def make_workload(name: str, args, rank: int):
     """Seeded synthetic inputs.  Rank r > 0 draws its own field points."""
     from paper_1606_03743_b200 import synth
-    if args.workload == "cfg4":
+    if name == "cfg4":
         c = synth.config4(scale=args.scale)
         if rank > 0:  # weak scaling: same mesh, another 10^6 track points per rank
             c["pts"] = synth.helical_tracks(c["ntracks"], c["npts_per_track"], seed=synth.SEED_CFG4_TRACKS + 1000 * rank)
@@ -126,12 +137,21 @@ def make_workload(args, rank: int):
         c["desc"] = ("config 4: cylinder R=5 m L=20 m (%d rectangles) + two end cones (%d triangles), sigma = 8 "
                      "Fourier modes, %d helical-track field points, DR-adaptive rules, Phi+E"
                      % (int((c["etype"] == 1).sum()), int((c["etype"] == 0).sum()), len(c["pts"])))
-    elif args.workload == "cfg2":
+    elif name == "cfg1":
+        c = synth.config1()
+        c["rule"] = 1
+        c["desc"] = "config 1: level-3 icosphere (1280 triangles), 1000 field points, Table A2 (N = 7), Phi+E"
+    elif name == "cfg2":
         c = synth.config2()
         c["rule"] = args.rule
         c["desc"] = "config 2: unit-cube surface 6144 squares, 10^4 field points, fixed rule level %d, %s" % (
             args.rule, args.precision)
-    elif args.workload == "table3":
+    elif name == "cfg5":
+        c = synth.config5(synth.TRI)
+        c["rule"] = args.rule
+        c["desc"] = "config 5: single triangle, 10^6 field points at log-uniform distance ratios 1..1e6, rule level %d, %s" % (
+            args.rule, args.precision)
+    elif name == "table3":
         # the SHAPE of the paper's GPU timing (Table 3: 1.5 M rectangles, 10^4 field points) on a
         # synthetic cylinder; --rule 1 = the 7-point rule, --rule -1 = distance-ratio dependent
         et, vt = synth.cylinder_rects(5.0, -10.0, 10.0, 1500, 1000)
@@ -139,7 +159,7 @@ def make_workload(args, rank: int):
                  pts=synth.helical_tracks(100, 100), rule=args.rule)
         c["desc"] = ("Table-3 shape: cylinder of 1.5e6 rectangles, 1e4 helical-track field points, rule %s, Phi+E"
                      % ("adaptive" if args.rule == -1 else "level %d" % args.rule))
-    elif args.workload == "solve":
+    elif name == "solve":
         c = synth.config3()
         c["pts"] = np.zeros((len(c["etype"]), 3))
         c["rule"] = None
@@ -150,58 +170,76 @@ def make_workload(args, rank: int):
         c["pts"] = np.zeros((len(c["etype"]), 3))
         c["rule"] = None
         c["desc"] = "config 3: level-5 icosphere 20480 x 20480 collocation matrix, L159 limits"
+    c["workload"] = name
     return c
 
 
-def oracle_rate(c, args, target_seconds: float, min_pts: int = 8, max_pts: int = 65536):
-    """Times the CPU oracle (double-precision instantiation, OpenMP over field points, all host
-    cores, as it stands) on a bounded seeded sample of the workload's field points / matrix rows.
-    Returns (units per second, cores, sample description, seconds, sampled units)."""
+def oracle_rate(c, target_seconds: float, full: bool = False, min_units: int = 8, max_units: int = 65536):
+    """Times the CPU oracle (double-precision instantiation where it has one, OpenMP over field points /
+    rows, all host cores, as it stands) on a bounded seeded sample of the workload's field points /
+    matrix rows - or on all of them (`full`).  The sample is a multiple of the thread count, so every
+    thread is busy.  Returns dict(value, cores, threads_busy, sample, seconds, units[, points_per_pair])."""
     import oracle
     cores = oracle.num_threads()
     n = len(c["etype"])
+    is_matrix = c["workload"] == "cfg3"
     rng = np.random.default_rng(160603751)
-    if args.workload == "cfg3":
+    counts = {}
+    if is_matrix:
         dr = oracle.default_policy(False)
         run = lambda idx: oracle.assemble_rows(c["etype"], c["verts"], idx, dr)
         total = n
     else:
         dr = oracle.default_policy(True)
-        run = lambda idx: oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx], c["rule"], dr=dr,
-                                          precision="double")
+        def run(idx):
+            r = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx], c["rule"], dr=dr, precision="double",
+                                want_counts=True)
+            counts["npi"] = int(r["npi"].sum())
         total = len(c["pts"])
-    probe = min(total, max(min_pts, 4 * cores))
-    idx = np.sort(rng.choice(total, probe, replace=False))
-    t0 = time.perf_counter()
-    run(idx)
-    t_probe = time.perf_counter() - t0
-    k = int(min(max_pts, total, max(probe, probe * target_seconds / max(t_probe, 1e-6))))
-    k = max(cores, k // cores * cores)
-    idx = np.sort(rng.choice(total, min(k, total), replace=False))
+    if full:
+        k = total
+    else:
+        probe = min(total, max(min_units, cores))
+        idx = np.sort(rng.choice(total, probe, replace=False))
+        t0 = time.perf_counter()
+        run(idx)
+        t_probe = time.perf_counter() - t0
+        k = int(min(max_units, total, max(probe, probe * target_seconds / max(t_probe, 1e-6))))
+        k = min(total, max(cores, k // cores * cores))
+    idx = np.sort(rng.choice(total, k, replace=False)) if k < total else np.arange(total)
     t0 = time.perf_counter()
     run(idx)
     dt = time.perf_counter() - t0
-    what = "matrix rows" if args.workload == "cfg3" else "field points"
-    sample = f"all {n} elements x {len(idx)} seeded {what} of the workload, oracle double-precision path, {cores} OpenMP threads"
-    return n * len(idx) / dt, cores, sample, dt, len(idx)
+    what = "matrix rows" if is_matrix else "field points"
+    which = "long-double (its only matrix path)" if is_matrix else "double-precision"
+    out = {"value": n * len(idx) / dt, "unit": "matrix entries/s" if is_matrix else UNIT, "cores": cores,
+           "threads_busy": min(cores, len(idx)), "kind": "oracle",
+           "sample": f"all {n} elements x {len(idx)} {'(all) ' if k == total else 'seeded '}{what} of the workload, oracle "
+                     f"{which} path, {cores} OpenMP threads, one field point / row per task",
+           "seconds": dt, "units": len(idx)}
+    if "npi" in counts:
+        out["points_per_pair"] = counts["npi"] / (float(n) * len(idx))
+    return out
 
 
 def run_reference(args, rank: int):
     """--impl reference: the oracle as it stands on the host cores, rank 0 only."""
     if rank != 0:
         return
-    c = make_workload(args, 0)
+    name = args.workload if args.workload in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "table3") else "cfg4"
+    c = make_workload(name, args, 0)
     # each step a bounded sample (~4 s) so that warmup + steps end within a few minutes
-    rate0, cores, sample, dt, k = oracle_rate(c, args, target_seconds=4.0)
+    probe = oracle_rate(c, target_seconds=4.0)
     import oracle
-    n = len(c["etype"])
+    n, k = len(c["etype"]), probe["units"]
+    is_matrix = name == "cfg3"
     rng = np.random.default_rng(160603752)
-    total = n if args.workload == "cfg3" else len(c["pts"])
-    dr = oracle.default_policy(args.workload != "cfg3")
+    total = n if is_matrix else len(c["pts"])
+    dr = oracle.default_policy(not is_matrix)
 
     def step():
-        idx = np.sort(rng.choice(total, k, replace=False))
-        if args.workload == "cfg3":
+        idx = np.sort(rng.choice(total, k, replace=False)) if k < total else np.arange(total)
+        if is_matrix:
             oracle.assemble_rows(c["etype"], c["verts"], idx, dr)
         else:
             oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx], c["rule"], dr=dr, precision="double")
@@ -213,17 +251,188 @@ def run_reference(args, rank: int):
         step()
     dt = (time.perf_counter() - t0) / max(args.steps, 1)
     value = n * k / dt
-    unit = UNIT if args.workload != "cfg3" else "matrix entries/s"
+    unit = UNIT if not is_matrix else "matrix entries/s"
     line = {
-        "impl": "reference", "metric": METRIC if args.workload != "cfg3" else "FP64 collocation-matrix entries/s",
+        "impl": "reference", "metric": METRIC if not is_matrix else "FP64 collocation-matrix entries/s",
         "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": c["desc"], "elements": n, "sampled_units_per_step": k},
-        "cpu_baseline": {"value": value, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": unit, "cores": probe["cores"], "threads_busy": probe["threads_busy"],
+                         "kind": "oracle", "sample": probe["sample"]},
         "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------
+def measure_peak(b, h, num_sms: int, seconds: float = 2.4) -> dict:
+    """Roofline denominator: the FP64 issue-rate sweep (DFMA / DADD / DMUL / the Eq. 4.1 mix at 8, 16, 32
+    warps per SM, `seconds` / 12 each), its maximum, and the nominal rate beside it."""
+    rates, mhz = b.bemcub_fp64_issue_sweep(h, seconds / b.PEAK_VARIANTS)
+    best = int(np.argmax(rates))
+    table = [{"mix": b.PEAK_MIXES[i // 3], "warps_per_sm": b.PEAK_WARPS[i % 3], "fp64_inst_per_s": float(rates[i]),
+              "sm_mhz": float(mhz[i]), "of_nominal": float(rates[i] / (FP64_LANES_PER_SM * num_sms * mhz[i] * 1e6)) if mhz[i] else None}
+             for i in range(b.PEAK_VARIANTS)]
+    return {"fp64_inst_per_s": float(rates[best]), "tflops": 2.0 * float(rates[best]) / 1e12,
+            "best": f"{b.PEAK_MIXES[best // 3]}, {b.PEAK_WARPS[best % 3]} warps/SM", "sm_mhz": float(mhz[best]),
+            "sweep": table,
+            "source": "bemcub_fp64_issue_sweep in this run: max FP64 instruction issue rate over 4 mixes x 3 occupancies, "
+                      f"{seconds / b.PEAK_VARIANTS:.2f} s each (x2 flop per instruction); MEASURED_PEAKS.json has no FP64 entry"}
+
+
+def nominal_tflops(num_sms: int, sm_mhz: float) -> float:
+    return FP64_LANES_PER_SM * num_sms * 2.0 * sm_mhz * 1e6 / 1e12
+
+
+def roofline_block(kernel: str, k_ms: float, step_ms: float, inter: float, inter_own, fpi: int, ipi: int, peak: dict,
+                   num_sms: int, kernel_mhz, smi_mhz) -> dict:
+    """FLOP fractions of the dominant kernel four ways (executed / the method's own work, against the
+    measured peak / the nominal rate at the clock the kernel ran at) and the arithmetic pipe fraction."""
+    ach = inter * fpi / (k_ms * 1e-3) / 1e12
+    clock = kernel_mhz or smi_mhz or peak["sm_mhz"]
+    nom = nominal_tflops(num_sms, clock)
+    r = {"bound": "alu", "achieved": ach, "peak": peak["tflops"], "unit": "TFLOP/s", "frac": ach / peak["tflops"],
+         "traffic": None,
+         "traffic_source": "not measured by this run; dram__bytes of one launch are in the ncu captures under profiles/ (ALU-bound: "
+                           "the bytes do not set the time)",
+         "kernel": kernel, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / step_ms if step_ms else None,
+         "point_interactions_per_launch": inter, "flop_per_interaction": fpi, "fp64_inst_per_interaction": ipi,
+         "frac_nominal": ach / nom, "nominal_tflops": nom,
+         "nominal_def": f"{num_sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {clock:.0f} MHz "
+                        f"({'SM clock read inside the kernel: cycle counter / global timer' if kernel_mhz else 'nvidia-smi median'})",
+         "peak_over_nominal": peak["tflops"] / nom, "peak_source": peak["source"], "peak_best_variant": peak["best"],
+         "kernel_sm_mhz": kernel_mhz,
+         "fp64_issue_frac_arith": inter * ipi / (k_ms * 1e-3) / peak["fp64_inst_per_s"],
+         "fp64_issue_frac_arith_def": "FP64 instructions of the interactions executed (interactions x instructions per interaction) "
+                                      "/ kernel time / measured issue rate: arithmetic, not a hardware counter"}
+    if inter_own is not None:
+        own = inter_own * fpi / (k_ms * 1e-3) / 1e12
+        r.update({"frac_own_work": own / peak["tflops"], "frac_own_work_nominal": own / nom,
+                  "own_work_interactions_per_launch": inter_own,
+                  "own_work_def": "point-charge interactions of the per-pair distance-ratio policy (what the method asks for; "
+                                  "device counter of one untimed call with allow_upgrade = 0); the tiles execute a few per cent more"})
+    return r
+
+
+def kernel_clock_mhz(st: dict):
+    return 1e3 * st["kernel_cycles"] / st["kernel_ns"] if st.get("kernel_ns") else None
+
+
+class Runner:
+    """One bemcub ctx on this rank's GPU, device-resident inputs of one workload, a timed loop."""
+
+    def __init__(self, b, torch, dev_index: int, c: dict):
+        self.b, self.torch, self.c = b, torch, c
+        self.dev = torch.device("cuda", dev_index)
+        self.ctx = b.Context(dev_index)
+        self.h = self.ctx.handle
+        self.n, self.m = len(c["etype"]), len(c["pts"])
+        self.h_type = torch.as_tensor(c["etype"]).pin_memory()
+        self.h_verts = torch.as_tensor(c["verts"]).pin_memory()
+        self.h_sigma = torch.as_tensor(np.ascontiguousarray(c["sigma"])).pin_memory()
+        self.h_pts = torch.as_tensor(c["pts"]).pin_memory()
+        self.d_type, self.d_verts = self.h_type.to(self.dev), self.h_verts.to(self.dev)
+        self.d_sigma, self.d_pts = self.h_sigma.to(self.dev), self.h_pts.to(self.dev)
+        b.bemcub_set_elements(self.h, self.n, self.d_type, self.d_verts)
+        b.bemcub_set_timing(self.h, True)
+
+    def timed(self, step, steps: int, warmup: int, barrier, gpu_index: int, period_ms: int = 200):
+        """W untimed + K timed steps: CUDA events around the K steps, the dominant kernel's own event
+        time per step, nvidia-smi clocks sampled during the timed region."""
+        b, torch = self.b, self.torch
+        for _ in range(warmup):
+            step()
+        barrier()
+        b.bemcub_reset_stats(self.h)
+        sampler = ClockSampler(gpu_index, period_ms)
+        sampler.start()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        kernel_ms = []
+        ev0.record()
+        for _ in range(steps):
+            step()
+            kernel_ms.append(b.bemcub_get_timing(self.h)[1])   # waits for this step's events only
+        ev1.record()
+        barrier()
+        clocks = sampler.stop()
+        st = b.bemcub_get_stats(self.h)
+        return {"ms": ev0.elapsed_time(ev1) / max(steps, 1), "kernel_ms": sum(kernel_ms) / max(len(kernel_ms), 1),
+                "clocks": clocks, "stats": st}
+
+    def close(self):
+        self.ctx.close()
+
+
+def steps_for(ms_estimate: float, seconds: float = 1.5, lo: int = 20, hi: int = 5000) -> int:
+    return int(min(hi, max(lo, seconds * 1e3 / max(ms_estimate, 1e-3))))
+
+
+def secondary_block(args, b, torch, dev_index: int, peak: dict, num_sms: int, barrier):
+    """Short device-timed runs of the other configs: matrix fill of config 3,
+    configs 1, 2 (B2 and B5, FP64 and FP32) and 5, each with roofline, clocks and the oracle beside it."""
+    out = []
+
+    def fixed_rule_entry(name, rule, precision_name):
+        a2 = argparse.Namespace(**vars(args))
+        a2.rule, a2.precision, a2.scale = rule, precision_name, 1.0
+        c = make_workload(name, a2, 0)
+        r = Runner(b, torch, dev_index, c)
+        prec = b.F32 if precision_name == "f32" else b.F64
+        phi = torch.empty(r.m, dtype=torch.float64, device=r.dev)
+        E = torch.empty((r.m, 3), dtype=torch.float64, device=r.dev)
+        step = lambda: b.bemcub_eval(r.h, r.d_sigma, c["rule"], None, r.m, r.d_pts, phi, E, prec)
+        probe = r.timed(step, 5, 3, barrier, dev_index)
+        t = r.timed(step, steps_for(probe["ms"]), 3, barrier, dev_index, period_ms=100)
+        st = t["stats"]
+        inter = float(st["point_interactions"])
+        entry = {"workload": c["desc"], "dtype": precision_name, "ms_per_step": t["ms"], "kernel_ms": t["kernel_ms"],
+                 "value": float(r.n) * r.m / (t["ms"] * 1e-3), "unit": UNIT, "clocks": t["clocks"],
+                 "points_per_pair": inter / (float(r.n) * r.m)}
+        if prec == b.F64:
+            entry["roofline"] = roofline_block("eval_fixed_kernel", t["kernel_ms"], t["ms"], inter, inter, FLOP_PER_INTERACTION, 18,
+                                               peak, num_sms, kernel_clock_mhz(st), t["clocks"].get("sm_mhz"))
+        else:
+            entry["roofline"] = {"bound": "alu", "achieved": inter * FLOP_PER_INTERACTION / (t["kernel_ms"] * 1e-3) / 1e12,
+                                 "unit": "TFLOP/s", "peak": None, "frac": None, "traffic": None,
+                                 "note": "FP32 variant: reported, no FP32 peak measured (the FP32 pipe has twice the lanes)"}
+        if not args.no_cpu_baseline and prec == b.F64:
+            entry["cpu_baseline"] = oracle_rate(c, target_seconds=3.0, full=float(r.n) * r.m * 7 <= 3e9)
+        r.close()
+        return entry
+
+    # matrix fill, config 3
+    c3 = make_workload("cfg3", args, 0)
+    r = Runner(b, torch, dev_index, c3)
+    pol0 = b.bemcub_default_policy(False)
+    A = torch.empty((r.n, r.n), dtype=torch.float64, device=r.dev)
+    step = lambda: b.bemcub_assemble(r.h, pol0, A, r.n)
+    t = r.timed(step, 300, 5, barrier, dev_index, period_ms=100)
+    st = t["stats"]
+    inter = float(st["point_interactions"])
+    pol_pp = b.bemcub_default_policy(False)
+    pol_pp.allow_upgrade = 0
+    b.bemcub_assemble(r.h, pol_pp, A, r.n)             # untimed: the per-pair policy's own work
+    own = float(b.bemcub_get_stats(r.h)["point_interactions"])
+    roof = roofline_block("assemble_kernel", t["kernel_ms"], t["ms"], inter, own, FLOP_PER_INTERACTION_PHI, 12, peak, num_sms,
+                          kernel_clock_mhz(st), t["clocks"].get("sm_mhz"))
+    roof["store_stream_gb_s"] = float(r.n) * r.n * 8 / (t["kernel_ms"] * 1e-3) / 1e9
+    entry = {"workload": c3["desc"], "dtype": "f64", "ms_per_step": t["ms"], "kernel_ms": t["kernel_ms"],
+             "value": float(r.n) * r.n / (t["ms"] * 1e-3), "unit": "matrix entries/s", "steps": 300, "clocks": t["clocks"],
+             "points_per_entry": inter / (float(r.n) * r.n), "points_per_entry_own_work": own / (float(r.n) * r.n),
+             "analytic_entries_per_row": st["analytic_pairs"] / float(r.n), "roofline": roof}
+    if not args.no_cpu_baseline:
+        entry["cpu_baseline"] = oracle_rate(c3, target_seconds=6.0, min_units=64)
+    del A
+    r.close()
+    out.append(entry)
+
+    out.append(fixed_rule_entry("cfg1", 1, "f64"))
+    for rule in (1, 4):
+        for prec in ("f64", "f32"):
+            out.append(fixed_rule_entry("cfg2", rule, prec))
+    out.append(fixed_rule_entry("cfg5", 1, "f64"))
+    return out
 
 
 # --------------------------------------------------------------------------------------------
@@ -235,28 +444,23 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the bemcub path has no CPU fallback")
     torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    c = make_workload(args, rank)
-    n, m = len(c["etype"]), len(c["pts"])
-    is_matrix = args.workload in ("cfg3", "solve")
-    is_solve = args.workload == "solve"
-    precision = b.F32 if (args.workload == "cfg2" and args.precision == "f32") else b.F64
+    num_sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    ctx = b.Context(local_rank)
-    h = ctx.handle
-    # pinned host copies (the e2e leg reads them), device-resident copies (the kernel-only leg)
-    h_type = torch.as_tensor(c["etype"]).pin_memory()
-    h_verts = torch.as_tensor(c["verts"]).pin_memory()
-    h_sigma = torch.as_tensor(np.ascontiguousarray(c["sigma"])).pin_memory()
-    h_pts = torch.as_tensor(c["pts"]).pin_memory()
-    d_type, d_verts = h_type.to(dev), h_verts.to(dev)
-    d_sigma, d_pts = h_sigma.to(dev), h_pts.to(dev)
-    b.bemcub_set_elements(h, n, d_type, d_verts)
+    if args.workload == "accuracy":
+        return run_accuracy(args, b, torch, local_rank, barrier)
+
+    c = make_workload(args.workload, args, rank)
+    r = Runner(b, torch, local_rank, c)
+    h, dev, n, m = r.h, r.dev, r.n, r.m
+    is_matrix = args.workload in ("cfg3", "solve")
+    is_solve = args.workload == "solve"
+    precision = b.F32 if (args.workload in ("cfg2", "cfg5") and args.precision == "f32") else b.F64
+    adaptive = c["rule"] == -1
     solve_info = {}
     if is_solve:
         pol = b.bemcub_default_policy(False)
@@ -272,45 +476,28 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         out = torch.empty((n, n), dtype=torch.float64, device=dev)
         step = lambda: b.bemcub_assemble(h, pol, out, n)
     else:
-        pol = b.bemcub_default_policy(True) if c["rule"] == -1 else None
+        pol = b.bemcub_default_policy(True) if adaptive else None
         phi = torch.empty(m, dtype=torch.float64, device=dev)
         E = torch.empty((m, 3), dtype=torch.float64, device=dev)
         if args.gradient:
             if pol is not None:
                 pol.use_levels_mask = 0b011111          # derivatives exist for the point charges only (L273)
             G = torch.empty((m, 6), dtype=torch.float64, device=dev)
-            step = lambda: b.bemcub_eval_gradient(h, d_sigma, c["rule"], pol, m, d_pts, phi, E, G)
+            step = lambda: b.bemcub_eval_gradient(h, r.d_sigma, c["rule"], pol, m, r.d_pts, phi, E, G)
         else:
-            step = lambda: b.bemcub_eval(h, d_sigma, c["rule"], pol, m, d_pts, phi, E, precision)
+            step = lambda: b.bemcub_eval(h, r.d_sigma, c["rule"], pol, m, r.d_pts, phi, E, precision)
 
-    # roofline denominator: sustained DFMA rate of this GPU, measured in this run
-    dfma_per_s = b.bemcub_fp64_peak(h, 2.0)
-    peak_tflops = 2.0 * dfma_per_s / 1e12
+    # roofline denominator: FP64 issue rate of this GPU, measured in this run
+    peak = measure_peak(b, h, num_sms)
     # second reference: the kernels' own inner loop on resident data (what the 18-instruction mix allows)
     loop_rate = b.bemcub_inner_loop_rate(h, 1.0)
 
-    b.bemcub_set_timing(h, True)
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    b.bemcub_reset_stats(h)
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    kernel_ms = []
-    ev0.record()
-    for _ in range(args.steps):
-        step()
-        kernel_ms.append(b.bemcub_get_timing(h)[1])   # waits for this step's events only
-    ev1.record()
-    barrier()
-    clocks = sampler.stop()
-    st = b.bemcub_get_stats(h)
-    ms = ev0.elapsed_time(ev1) / max(args.steps, 1)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    t = r.timed(step, args.steps, args.warmup, barrier, local_rank)
+    st, clocks, ms, k_ms = t["stats"], t["clocks"], t["ms"], t["kernel_ms"]
+    tt = torch.tensor([ms], dtype=torch.float64, device=dev)
     if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms_max = float(tt.item())
     units_per_step = float(n) * float(n if is_matrix else m) * (solve_info.get("matvecs", 1) if is_solve else 1)
     if is_solve:
         areas = 0.5 * np.linalg.norm(np.cross(c["verts"][:, 1] - c["verts"][:, 0], c["verts"][:, 2] - c["verts"][:, 0]), axis=1)
@@ -319,33 +506,40 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     value = units_per_step * world / (ms_max * 1e-3)
 
     # dominant kernel against the FP64-ALU roofline
-    k_ms = sum(kernel_ms) / max(len(kernel_ms), 1)
     inter = float(st["point_interactions"])          # point-charge interactions of the last step
     fpi = FLOP_PER_INTERACTION_PHI if is_matrix else (FLOP_PER_INTERACTION_GRAD if args.gradient else FLOP_PER_INTERACTION)
     ipi = 12 if is_matrix else (28 if args.gradient else 18)   # FP64 instructions per interaction
-    flop = inter * fpi
+    inter_own = None
+    if (adaptive and not args.gradient) or args.workload == "cfg3":
+        # the method's own work: one untimed call with the exact per-pair policy, counted on the device
+        pol_pp = b.bemcub_default_policy(not is_matrix)
+        pol_pp.allow_upgrade = 0
+        if is_matrix:
+            b.bemcub_assemble(h, pol_pp, out, n)
+        else:
+            b.bemcub_eval(h, r.d_sigma, -1, pol_pp, m, r.d_pts, phi, E, precision)
+        inter_own = float(b.bemcub_get_stats(h)["point_interactions"])
+    elif not is_matrix and not adaptive:
+        inter_own = inter
+    kernel = ("eval_adaptive_kernel<kModePhi>" if is_solve else "assemble_kernel" if is_matrix else
+              ("eval_adaptive_kernel" if adaptive else "eval_fixed_kernel"))
     if precision == b.F32:
-        roof = {"bound": "alu", "achieved": flop / (k_ms * 1e-3) / 1e12, "peak": None, "unit": "TFLOP/s", "frac": None,
+        roof = {"bound": "alu", "achieved": inter * fpi / (k_ms * 1e-3) / 1e12, "peak": None, "unit": "TFLOP/s", "frac": None,
                 "traffic": None, "note": "FP32 variant: reported, no FP32 peak measured"}
     else:
-        ach = flop / (k_ms * 1e-3) / 1e12
-        # DRAM bytes of ONE launch of the dominant kernel from the committed ncu capture of this very
-        # workload (profiles/r1_cfg4_full_eval_adaptive_counters.csv: 3.28 GB read + 0.55 GB written)
-        traffic = 3277495040 + 549181696 if (args.workload == "cfg4" and args.scale == 1.0 and not args.gradient) else None
-        roof = {"bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
-                "traffic": traffic, "kernel": "eval_adaptive_kernel<kModePhi>" if is_solve else "assemble_kernel" if is_matrix else
-                ("eval_adaptive_kernel" if c["rule"] == -1 else "eval_fixed_kernel"),
-                "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms,
-                "point_interactions_per_launch": inter,
-                "flop_per_interaction": fpi,
-                "peak_source": "bemcub_fp64_peak: sustained all-SM DFMA-only loop (best of 16 / 32 warps per SM), 2 s, same run (x2 flop/FMA); "
-                               "MEASURED_PEAKS.json has no FP64 entry",
-                "fp64_pipe_frac": (inter * ipi / (k_ms * 1e-3)) / dfma_per_s,
-                "inner_loop_ceiling": {"interactions_per_s": loop_rate,
-                                       "frac_of_peak": loop_rate * FLOP_PER_INTERACTION / (2.0 * dfma_per_s),
-                                       "kernel_over_ceiling": None if is_matrix else (inter / (k_ms * 1e-3)) / loop_rate,
-                                       "source": "bemcub_inner_loop_rate: Eq. 4.1 loop (18 FP64 instr + MUFU, 8 of 18 "
-                                                 "are FMAs => at most 26/36 = 72.2% of the DFMA peak), resident data"}}
+        roof = roofline_block(kernel, k_ms, ms, inter, inter_own, fpi, ipi, peak, num_sms, kernel_clock_mhz(st), clocks.get("sm_mhz"))
+        roof["inner_loop_ceiling"] = {
+            "interactions_per_s": loop_rate,
+            "frac_of_peak": loop_rate * FLOP_PER_INTERACTION / peak["tflops"] / 1e12,
+            "kernel_over_ceiling": None if is_matrix else (inter / (k_ms * 1e-3)) / loop_rate,
+            "source": "bemcub_inner_loop_rate: Eq. 4.1 loop (18 FP64 instr + MUFU, 8 of 18 are FMAs => at most 26/36 = 72.2% "
+                      "of the FLOP peak), resident data"}
+        if is_matrix:
+            roof["store_stream_gb_s"] = float(n) * n * 8 / (k_ms * 1e-3) / 1e9
+        if args.workload in NCU_PIPE and args.scale == 1.0 and not args.gradient:
+            roof["ncu_fp64_pipe_counter"] = {"file": NCU_PIPE[args.workload][0], "metric": NCU_PIPE[args.workload][1],
+                                             "note": "hardware counter of a committed capture of this launch configuration, "
+                                                     "not of this run"}
 
     # end to end through the host-buffer C-ABI calls: H2D of the inputs, compute, D2H of Phi/E
     e2e = None
@@ -355,43 +549,50 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         ctx2 = b.Context(local_rank)
 
         def step_host():
-            b.bemcub_set_elements_host(ctx2.handle, n, h_type, h_verts)
-            b.bemcub_eval_host(ctx2.handle, h_sigma, c["rule"], pol, m, h_pts, o_phi, o_E, precision)
+            b.bemcub_set_elements_host(ctx2.handle, n, r.h_type, r.h_verts)
+            b.bemcub_eval_host(ctx2.handle, r.h_sigma, c["rule"], pol, m, r.h_pts, o_phi, o_E, precision)
 
         step_host()
         barrier()
-        t0 = time.perf_counter()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record()
         for _ in range(args.steps):
             step_host()
         ev1.record()
         barrier()
         ms_e = ev0.elapsed_time(ev1) / max(args.steps, 1)
-        t = torch.tensor([ms_e], dtype=torch.float64, device=dev)
+        tt = torch.tensor([ms_e], dtype=torch.float64, device=dev)
         if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": units_per_step * world / (float(t.item()) * 1e-3), "unit": UNIT,
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e = {"value": units_per_step * world / (float(tt.item()) * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": int(n * 1 + n * 72 + n * 8 + m * 24), "d2h_bytes_per_step": int(m * 32),
-               "ms_per_step": float(t.item()), "api": "bemcub_set_elements_host + bemcub_eval_host (pinned host buffers)"}
+               "ms_per_step": float(tt.item()), "api": "bemcub_set_elements_host + bemcub_eval_host (pinned host buffers)"}
         assert bool(torch.isfinite(o_phi).all())
         ctx2.close()
     elif is_matrix:
         e2e = {"value": None, "unit": "matrix entries/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
                "note": "matrix stays on the device (3.36 GB); no host leg"}
+    launches = int(st["kernel_launches"])
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not is_solve:
-        rate, cores, sample, dt, k = oracle_rate(c, args, target_seconds=15.0)
-        cpu = {"value": rate, "unit": UNIT if not is_matrix else "matrix entries/s", "cores": cores, "kind": "oracle",
-               "sample": sample, "seconds": dt}
+        cpu = oracle_rate(c, target_seconds=15.0)
         if not is_matrix:   # the paper's CPU numbers are single-threaded (Table 2): one thread on a smaller sample
             import oracle
-            k1 = max(4, int(k / max(cores, 1) / 4))
+            k1 = max(4, int(cpu["units"] / max(cpu["cores"], 1) / 4))
             idx1 = np.sort(np.random.default_rng(160603753).choice(m, min(k1, m), replace=False))
             t0 = time.perf_counter()
             oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx1], c["rule"], dr=oracle.default_policy(True),
                             precision="double", nthreads=1)
             cpu["value_single_thread"] = n * len(idx1) / (time.perf_counter() - t0)
+
+    secondary = None
+    if rank == 0 and world == 1 and args.workload == "cfg4" and args.scale == 1.0 and not args.no_secondary and not args.gradient:
+        r.close()
+        r = None
+        del phi, E
+        torch.cuda.empty_cache()
+        secondary = secondary_block(args, b, torch, local_rank, peak, num_sms, barrier)
 
     if rank == 0:
         line = {
@@ -404,18 +605,138 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                        "parallelism": f"field points sharded over {world} GPU(s), no collective",
                        "l2": "inputs larger than L2 (expanded point arrays %.0f MB; compute-bound kernel)"
                              % (n * (7 + 12 + 19 + 33) * 32 / 1e6) if args.workload == "cfg4" else "compute-bound; not flushed",
-                       "points_per_pair": inter / units_per_step if units_per_step else None},
+                       "points_per_pair": inter / units_per_step if units_per_step else None,
+                       "points_per_pair_own_work": inter_own / units_per_step if (inter_own and units_per_step) else None},
             "pct_fp64_peak": 100.0 * roof["frac"] if roof.get("frac") else None,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(st["kernel_launches"]),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
             "roofline": roof, "cpu_baseline": cpu,
         }
+        if secondary is not None:
+            line["secondary"] = secondary
         if is_solve:
             line["metric"] = "FP64 potential-only element.point interactions/s inside bemcub_solve"
             line["unit"] = "element.point interactions/s"
             line["solve"] = solve_info
             line["roofline"]["note"] = "kernel_ms / interactions are those of the LAST mat-vec of the solve"
         print(json.dumps(line), flush=True)
+    if r is not None:
+        r.close()
+
+
+# --------------------------------------------------------------------------------------------
+def run_accuracy(args, b, torch, dev_index: int, barrier):
+    """The paper's accuracy study on the GPU (Sec. 2 and 4: L68, L80, L149; Figs. 8-10; L163-169): random
+    triangles / rectangles with corners in the unit cube, a field point in a random direction at each of
+    500 distance ratios from 2 to 1e4, 2000 elements per ratio (10^6 pairs per element type), every rule
+    of App. A/B, the Duffy-mapped rectangle rules on triangles and the closed form, FP64 and FP32, all
+    through bemcub_eval_pairs.  The exact reference is this run's cpu_baseline leg: the oracle in long
+    double (closed form below DR = 12, 33-point rule above), timed.  Tables go to --out."""
+    import oracle
+    from paper_1606_03743_b200 import synth
+    dev = torch.device("cuda", dev_index)
+    ctx = b.Context(dev_index)
+    h = ctx.handle
+    n_ratio, per_ratio = 500, 2000
+    grid = np.geomspace(2.0, 1.0e4, n_ratio)
+    ratio = np.repeat(grid, per_ratio)
+    K = len(ratio)
+    lines, gpu_ms, gpu_pairs, cpu_s, cpu_pairs, launches = [], 0.0, 0, 0.0, 0, 0
+    sampler = ClockSampler(dev_index)
+    sampler.start()
+    summary = {}
+    for kind, kname in ((synth.TRI, "triangles"), (synth.RECT, "rectangles")):
+        et, verts, pts = synth.random_pairs(kind, K, ratio, 160603790 + kind)
+        t0 = time.perf_counter()
+        lo = oracle.evaluate_pairs(et, verts, pts, 5)
+        hi = oracle.evaluate_pairs(et, verts, pts, 4)
+        cpu_s += time.perf_counter() - t0
+        cpu_pairs += 2 * K
+        near = ratio < 12.0
+        phi_x = np.where(near, lo["phi"], hi["phi"])
+        E_x = np.where(near[:, None], lo["E"], hi["E"])
+        d = lambda a: torch.as_tensor(np.ascontiguousarray(a)).to(dev)
+        d_et, d_verts, d_pts = d(et), d(verts), d(pts)
+        phi = torch.empty(K, dtype=torch.float64, device=dev)
+        E = torch.empty((K, 3), dtype=torch.float64, device=dev)
+        methods = [(f"N={oracle.rule_info(kind, l)[0]}", l, b.F64) for l in range(5)]
+        methods += [(f"N={oracle.rule_info(kind, l)[0]} f32", l, b.F32) for l in range(5)]
+        if kind == synth.TRI:
+            methods += [(f"Duffy N={oracle.rule_info(1, l)[0]}", b.METHOD_DUFFY_L0 + l, b.F64) for l in range(5)]
+        methods += [("closed form", b.METHOD_ANALYTIC, b.F64)]
+        cols = {}
+        for name, method, prec in methods:
+            for rep in range(2):     # first call warms up
+                ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                ev0.record()
+                b.bemcub_eval_pairs(h, K, d_et, d_verts, None, method, None, d_pts, phi, E, prec)
+                ev1.record()
+                torch.cuda.synchronize()
+            gpu_ms += ev0.elapsed_time(ev1)
+            gpu_pairs += K
+            launches += 1
+            e_phi = np.abs(phi.cpu().numpy() - phi_x) / np.abs(phi_x)
+            e_E = np.abs(E.cpu().numpy() - E_x).sum(axis=1) / np.linalg.norm(E_x, axis=1)
+            cols[name] = (e_phi.reshape(n_ratio, per_ratio).mean(axis=1), e_E.reshape(n_ratio, per_ratio).mean(axis=1))
+        # first distance ratio from which a rule's mean error stays at the paper's level (L159)
+        for name in [m_[0] for m_ in methods[:5]]:
+            ok_phi = cols[name][0] <= 2e-15
+            ok_E = cols[name][1] <= 3e-15
+            def first_from(ok):
+                bad = np.flatnonzero(~ok)
+                return float(grid[0]) if len(bad) == 0 else (None if bad[-1] == len(ok) - 1 else float(grid[bad[-1] + 1]))
+            summary[f"{kname} {name}"] = {"phi_2e-15_from_dr": first_from(ok_phi), "field_3e-15_from_dr": first_from(ok_E)}
+        lines.append(f"## {kname}: mean relative error over {per_ratio} random elements per distance ratio (every 10th of {n_ratio} ratios)")
+        lines.append("# err(Phi) = |dPhi/Phi|, err(E) = sum_j |dE_j| / |E| (PAPER.md L80); columns: Phi / E per method")
+        lines.append("DR        " + "  ".join(f"{name:>19s}" for name in cols))
+        for i in range(0, n_ratio, 10):
+            lines.append(f"{grid[i]:9.3f} " + "  ".join(f"{cols[nm][0][i]:9.2e}/{cols[nm][1][i]:9.2e}" for nm in cols))
+        lines.append("")
+    # Fig. 10: aspect-ratio dependence of the 7-point rule at DR = 300
+    lines.append("## Fig. 10: 7-point rule at DR = 300, mean field / potential error per aspect-ratio bin (4e5 random elements per type)")
+    edges = [1, 1.5, 2, 3, 5, 10, 20, 50, 100, 1e9]
+    for kind, kname in ((synth.TRI, "triangles"), (synth.RECT, "rectangles")):
+        Kar = 400_000
+        et, verts, pts = synth.random_pairs(kind, Kar, 300.0, 160603795 + kind)
+        ar = synth.aspect_ratio(et, verts)
+        t0 = time.perf_counter()
+        ref = oracle.evaluate_pairs(et, verts, pts, 4)
+        cpu_s += time.perf_counter() - t0
+        cpu_pairs += Kar
+        d = lambda a: torch.as_tensor(np.ascontiguousarray(a)).to(dev)
+        phi = torch.empty(Kar, dtype=torch.float64, device=dev)
+        E = torch.empty((Kar, 3), dtype=torch.float64, device=dev)
+        b.bemcub_eval_pairs(h, Kar, d(et), d(verts), None, 1, None, d(pts), phi, E, b.F64)
+        torch.cuda.synchronize()
+        launches += 1
+        e_phi = np.abs(phi.cpu().numpy() - ref["phi"]) / np.abs(ref["phi"])
+        e_E = np.abs(E.cpu().numpy() - ref["E"]).sum(axis=1) / np.linalg.norm(ref["E"], axis=1)
+        for lo_, hi_ in zip(edges[:-1], edges[1:]):
+            sel = (ar >= lo_) & (ar < hi_)
+            if sel.any():
+                lines.append(f"{kname:10s} AR [{lo_:5g},{hi_:7g})  n={int(sel.sum()):7d}  Phi {e_phi[sel].mean():9.2e}  E {e_E[sel].mean():9.2e}")
+    clocks = sampler.stop()
+    if args.out:
+        os.makedirs(os.path.dirname(os.path.abspath(args.out)) or ".", exist_ok=True)
+        with open(args.out, "w") as f:
+            f.write("# bench.py --workload accuracy: the accuracy study of arXiv 1606.03743 (Figs. 8-10, L163-169) on one B200,\n"
+                    "# GPU results of bemcub_eval_pairs against the long-double oracle (closed form below DR = 12, N = 33 above).\n")
+            f.write("\n".join(lines) + "\n")
     ctx.close()
+    value = gpu_pairs / (gpu_ms * 1e-3)
+    line = {"metric": "single-element (element, point) pairs/s, all methods of the accuracy study", "value": value,
+            "unit": "element.point pairs/s", "n_gpus": 1, "steps": 1, "warmup": 1, "ms_per_step": gpu_ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64+f32", "data": "synthetic",
+            "config": {"workload": f"accuracy study: {n_ratio} distance ratios 2..1e4 x {per_ratio} random elements, triangles and "
+                                   "rectangles, 5 rules x FP64/FP32 + Duffy + closed form; Fig. 10 at DR = 300"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": None, "unit": "element.point pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                    "note": "study mode; errors are reduced on the host"},
+            "roofline": {"bound": "alu", "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None, "traffic": None,
+                         "note": "one thread per pair with on-the-fly geometry: a study tool, not a throughput kernel"},
+            "cpu_baseline": {"value": cpu_pairs / cpu_s, "unit": "element.point pairs/s", "cores": oracle.num_threads(),
+                             "kind": "oracle", "sample": "the exact references of the whole study (long double)", "seconds": cpu_s},
+            "limits": summary, "table": args.out}
+    print(json.dumps(line), flush=True)
 
 
 def main():
@@ -430,6 +751,7 @@ def main():
         import torch
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")      # the communicator log shows the ranks (and NVLS) of the barrier
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     try:

@@ -62,6 +62,13 @@ enum {
   BEMCUB_LEVEL_ANALYTIC = 5  /* bit index of the analytic branch in use_levels_mask        */
 };
 
+/* methods of bemcub_eval_pairs besides the rule levels and BEMCUB_RULE_ADAPTIVE */
+enum {
+  BEMCUB_METHOD_ANALYTIC = 5,  /* the closed form of Eq. 2.1 at any distance                  */
+  BEMCUB_METHOD_DUFFY_L0 = 8   /* + l (l = 0..4): rectangle rule of level l; on a triangle    */
+                               /* through the Duffy map (L163-169), on a rectangle as it is    */
+};
+
 enum { BEMCUB_F64 = 0, BEMCUB_F32 = 1 };
 
 enum {
@@ -102,6 +109,10 @@ typedef struct {
                                /* the stream is synchronised and bemcub_get_stats is called)*/
   int64_t analytic_pairs;      /* (element, point) pairs sent to the analytic branch, ditto */
   int64_t last_eval_launches;  /* kernels launched by the most recent eval/assemble call    */
+  int64_t kernel_cycles;       /* SM cycles and nanoseconds of the dominant kernel of the   */
+  int64_t kernel_ns;           /* last eval/assemble call, read on the device (clock64 and  */
+                               /* %globaltimer of one persistent CTA): cycles/ns = the SM   */
+                               /* clock the kernel really ran at; 0 for calls with m <= 64  */
 } bemcub_stats;
 
 /* device: CUDA device ordinal.  cuda_stream: a cudaStream_t cast to void* (NULL = default).    */
@@ -138,6 +149,25 @@ int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const d
  * m = 0 is a no-op.  Asynchronous. */
 int bemcub_eval(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
                 int64_t m, const double* field_pts, double* out_phi, double* out_E, int precision);
+
+/* The single-element integrator (the paper's innermost layer, L193-196 item a; the unit of its
+ * accuracy protocol, L68 and L149, Figs. 8-10): element k seen from field point k, k < npairs, NO
+ * sum over elements.  Independent of the ctx mesh (bemcub_set_elements is not needed).
+ *   type[npairs], verts[npairs][3][3] as in bemcub_set_elements; sigma[npairs] or NULL (unit density);
+ *   field_pts[npairs][3]; out_phi[npairs]; out_E[npairs][3] or NULL.
+ *   method = BEMCUB_RULE_L0..L4: Eq. 4.1 with the element's own rule of that level;
+ *            BEMCUB_RULE_ADAPTIVE: rule or closed form by the pair's distance ratio (host_policy, HOST);
+ *            BEMCUB_METHOD_ANALYTIC: the closed form (step a4) whatever the distance;
+ *            BEMCUB_METHOD_DUFFY_L0 + l: the RECTANGLE rule of level l - on a triangle through the
+ *            Duffy transformation Q = A + u[(B-A) + v(C-B)], u = (1+y)/2, v = (1+x)/2, weights (1+y) w
+ *            (Sec. 4: "much larger errors": the mapped rule is exact for triangle polynomials
+ *            of degree (D-1)/2 only), on a rectangle unchanged.
+ *   precision = BEMCUB_F32: points and the interaction arithmetic in FP32 (closed form stays FP64).
+ * A degenerate or non-rectangular element gives NaN in its own outputs (no error code: the call is
+ * asynchronous and does not validate).  npairs = 0 is a no-op. */
+int bemcub_eval_pairs(bemcub_ctx* ctx, int64_t npairs, const uint8_t* type, const double* verts, const double* sigma,
+                      int method, const bemcub_policy* host_policy, const double* field_pts, double* out_phi,
+                      double* out_E, int precision);
 
 /* Field gradient from the same point charges (L273: derivatives of the field "can be easily
  * computed from the point charges"): out_G[m][6] = G_xx, G_yy, G_zz, G_xy, G_xz, G_yz with
@@ -201,10 +231,19 @@ int bemcub_expand_points(bemcub_ctx* ctx, const double* sigma, int rule_id, doub
 /* Centroid [n][3], area [n], L [n] of the current mesh (any pointer may be NULL).  Asynchronous. */
 int bemcub_get_geometry(bemcub_ctx* ctx, double* out_cen, double* out_area, double* out_L);
 
-/* Roofline denominator: runs a DFMA-only kernel (16 independent chains per thread; at 16 and at 32
- * warps per SM, the better of the two counts) on all SMs for about `seconds` and returns the
- * sustained rate in FP64 FMA/s (flop/s = 2x).  Synchronises. */
-int bemcub_fp64_peak(bemcub_ctx* ctx, double seconds, double* host_dfma_per_s);
+/* Roofline denominator: the issue rate of the plain FP64 pipe.  bemcub_fp64_issue_sweep runs, for
+ * about `seconds_per_variant` each, kernels that issue nothing but independent chains of one FP64
+ * instruction kind - mix 0: DFMA, 1: DADD, 2: DMUL, 3: the 8 DFMA : 6 DMUL : 4 DADD mix of Eq. 4.1 -
+ * at 8, 16 and 32 warps per SM, every instruction reading at most two vector registers (the second
+ * source is a uniform register: an FP64 instruction with three distinct vector-register sources
+ * issues at 2/3 of the rate).  HOST outputs, index = mix * 3 + occupancy:
+ * host_rates[12] in FP64 lane-instructions per second (warp instructions x 32), host_sm_mhz[12]
+ * (may be NULL) the SM clock during that launch (cycle counter / global timer).
+ * bemcub_fp64_peak = the maximum of such a sweep lasting about `seconds` in total; flop/s = 2x (every
+ * instruction counted as an FMA).  Both synchronise. */
+#define BEMCUB_PEAK_VARIANTS 12
+int bemcub_fp64_issue_sweep(bemcub_ctx* ctx, double seconds_per_variant, double* host_rates, double* host_sm_mhz);
+int bemcub_fp64_peak(bemcub_ctx* ctx, double seconds, double* host_fp64_inst_per_s);
 
 /* Second roofline reference: the evaluation kernels' own inner loop (Eq. 4.1: 18 FP64
  * instructions + one MUFU per point-charge interaction, 4 field points per lane, 12 warps per SM)

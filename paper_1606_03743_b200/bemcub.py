@@ -17,6 +17,7 @@ from . import build as _build
 TRI, RECT = 0, 1
 RULE_ADAPTIVE = -1
 LEVEL_ANALYTIC = 5
+METHOD_ANALYTIC, METHOD_DUFFY_L0 = 5, 8
 F64, F32 = 0, 1
 ALL_LEVELS = 63
 
@@ -31,7 +32,8 @@ class bemcub_policy(C.Structure):
 
 class bemcub_stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_int64), ("point_interactions", C.c_int64),
-                ("analytic_pairs", C.c_int64), ("last_eval_launches", C.c_int64)]
+                ("analytic_pairs", C.c_int64), ("last_eval_launches", C.c_int64),
+                ("kernel_cycles", C.c_int64), ("kernel_ns", C.c_int64)]
 
 
 class BemcubError(RuntimeError):
@@ -58,6 +60,7 @@ def _load() -> C.CDLL:
         "bemcub_set_elements": [vp, i64, vp, vp],
         "bemcub_eval": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
         "bemcub_eval_gradient": [vp, vp, C.c_int, PP, i64, vp, vp, vp, vp],
+        "bemcub_eval_pairs": [vp, i64, vp, vp, vp, C.c_int, PP, vp, vp, vp, C.c_int],
         "bemcub_eval_linear": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
         "bemcub_solve": [vp, PP, vp, vp, dbl, C.c_int, C.POINTER(C.c_int), C.POINTER(dbl)],
         "bemcub_assemble": [vp, PP, vp, i64],
@@ -69,6 +72,7 @@ def _load() -> C.CDLL:
         "bemcub_expand_points": [vp, vp, C.c_int, vp, C.POINTER(C.c_int)],
         "bemcub_get_geometry": [vp, vp, vp, vp],
         "bemcub_fp64_peak": [vp, dbl, C.POINTER(dbl)],
+        "bemcub_fp64_issue_sweep": [vp, dbl, vp, vp],
         "bemcub_inner_loop_rate": [vp, dbl, C.POINTER(dbl)],
         "bemcub_get_stats": [vp, C.POINTER(bemcub_stats)],
         "bemcub_reset_stats": [vp],
@@ -86,10 +90,10 @@ def _load() -> C.CDLL:
 
 _lib = _load()
 EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval",
-            "bemcub_eval_gradient", "bemcub_eval_linear", "bemcub_solve",
+            "bemcub_eval_gradient", "bemcub_eval_linear", "bemcub_eval_pairs", "bemcub_solve",
             "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
             "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
-            "bemcub_fp64_peak", "bemcub_inner_loop_rate", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
+            "bemcub_fp64_peak", "bemcub_fp64_issue_sweep", "bemcub_inner_loop_rate", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
             "bemcub_get_timing", "bemcub_strerror"]
 
 
@@ -180,6 +184,12 @@ def bemcub_eval_gradient(ctx, sigma, rule_id: int, policy, m: int, field_pts, ou
                                      _dptr(out_phi), _dptr(out_E), _dptr(out_G)), "bemcub_eval_gradient")
 
 
+def bemcub_eval_pairs(ctx, npairs: int, etype, verts, sigma, method: int, policy, field_pts, out_phi, out_E,
+                      precision: int = F64) -> None:
+    _check(_lib.bemcub_eval_pairs(ctx, npairs, _dptr(etype), _dptr(verts), _dptr(sigma), method, _policy_ptr(policy),
+                                  _dptr(field_pts), _dptr(out_phi), _dptr(out_E), precision), "bemcub_eval_pairs")
+
+
 def bemcub_eval_linear(ctx, sigma_vertex, rule_id: int, policy, m: int, field_pts, out_phi, out_E,
                        precision: int = F64) -> None:
     _check(_lib.bemcub_eval_linear(ctx, _dptr(sigma_vertex), rule_id, _policy_ptr(policy), m, _dptr(field_pts),
@@ -247,6 +257,18 @@ def bemcub_fp64_peak(ctx, seconds: float) -> float:
     v = C.c_double()
     _check(_lib.bemcub_fp64_peak(ctx, seconds, C.byref(v)), "bemcub_fp64_peak")
     return v.value
+
+
+PEAK_VARIANTS = 12
+PEAK_MIXES = ("DFMA", "DADD", "DMUL", "mix 8 DFMA : 6 DMUL : 4 DADD")
+PEAK_WARPS = (8, 16, 32)
+
+
+def bemcub_fp64_issue_sweep(ctx, seconds_per_variant: float):
+    """(rates[12] FP64 lane-instructions/s, sm_mhz[12]); index = mix * 3 + occupancy."""
+    rates, mhz = np.zeros(PEAK_VARIANTS), np.zeros(PEAK_VARIANTS)
+    _check(_lib.bemcub_fp64_issue_sweep(ctx, seconds_per_variant, _hptr(rates), _hptr(mhz)), "bemcub_fp64_issue_sweep")
+    return rates, mhz
 
 
 def bemcub_inner_loop_rate(ctx, seconds: float) -> float:

@@ -14,7 +14,8 @@ from pathlib import Path
 
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
-LIB = PKG / "libbemcub.so"
+# BEMCUB_LIB: load another build of the same library (A/B timing of kernel variants); never rebuilt
+LIB = Path(os.environ["BEMCUB_LIB"]) if os.environ.get("BEMCUB_LIB") else PKG / "libbemcub.so"
 SOURCES = [CSRC / "bemcub.cu"]
 DEPS = sorted(CSRC.glob("*.cu*")) + sorted(CSRC.glob("*.h")) + sorted(CSRC.glob("*.inl")) + [PKG.parent / "include" / "bemcub.h"]
 
@@ -32,6 +33,8 @@ def nvcc_path() -> str:
 
 
 def is_stale() -> bool:
+    if os.environ.get("BEMCUB_LIB"):
+        return False
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime

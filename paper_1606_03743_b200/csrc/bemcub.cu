@@ -12,6 +12,7 @@
 #include "../../include/bemcub.h"
 #include "kernels_assemble.cuh"
 #include "kernels_eval.cuh"
+#include "kernels_pairs.cuh"
 #include "kernels_pre.cuh"
 #include "kernels_solve.cuh"
 #include "kernels_sort.cuh"
@@ -63,6 +64,7 @@ struct bemcub_ctx {
   unsigned long long* d_counters = nullptr;
   bemcub_stats stats{};
   bool counters_pending = false;
+  bool counters_counted = true;  // false: the interaction count is known on the host (fixed rule); only the clock is read back
   // optional per-call timing of the dominant kernel (bemcub_set_timing)
   bool timing = false;
   bool timing_valid = false;
@@ -184,17 +186,19 @@ int build_policy(const bemcub_policy* hp, PolicyDev* out) {
 
 // Expanded points of one level, FP64 or FP32, into ctx-owned memory.
 template <typename T>
-int expand_level(bemcub_ctx* c, int level, const double* sigma, DevBuf& dst, const double* sigma_v = nullptr) {
+int expand_level(bemcub_ctx* c, int level, const double* sigma, DevBuf& dst, const double* sigma_v = nullptr, int stride = 0,
+                 double scale = 1.0) {
   typedef typename Point4<T>::type P4;
-  const int64_t total = c->n * c->stride[level];
+  if (stride == 0) stride = c->stride[level];
+  const int64_t total = c->n * stride;
   int rc = ensure(dst, (size_t)std::max<int64_t>(total, 1) * sizeof(P4));
   if (rc) return rc;
   if (total == 0) return BEMCUB_OK;
   const int threads = 256;
   const int64_t blocks = (total + threads - 1) / threads;
   expand_kernel<T><<<(unsigned)blocks, threads, 0, c->stream>>>(
-      c->n, level, c->stride[level], (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr,
-      (const double4*)c->cenL.ptr, (const double*)c->area.ptr, sigma, sigma_v, (P4*)dst.ptr);
+      c->n, level, stride, (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr,
+      (const double4*)c->cenL.ptr, (const double*)c->area.ptr, sigma, sigma_v, scale, (P4*)dst.ptr);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
@@ -312,11 +316,15 @@ void mark(bemcub_ctx* c, int i) {
 
 void refresh_counters(bemcub_ctx* c) {
   if (!c->counters_pending) return;
-  unsigned long long h[2] = {0, 0};
+  unsigned long long h[6] = {0, 0, 0, 0, 0, 0};
   cudaStreamSynchronize(c->stream);
   if (cudaMemcpy(h, c->d_counters, sizeof(h), cudaMemcpyDeviceToHost) == cudaSuccess) {
-    c->stats.point_interactions = (int64_t)h[0];
-    c->stats.analytic_pairs = (int64_t)h[1];
+    if (c->counters_counted) {
+      c->stats.point_interactions = (int64_t)h[0];
+      c->stats.analytic_pairs = (int64_t)h[1];
+    }
+    c->stats.kernel_cycles = (int64_t)h[4];
+    c->stats.kernel_ns = (int64_t)h[5];
   }
   c->counters_pending = false;
 }
@@ -405,7 +413,7 @@ int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream) {
   c->num_sms = prop.multiProcessorCount;
   int rc = upload_tables();
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_status, sizeof(GeomStatus)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
-  if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, 4 * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
+  if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
   if (rc != BEMCUB_OK) {
     bemcub_destroy(c);
     return rc;
@@ -585,7 +593,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     fw.counters = c->d_counters;
     fw.area = (const double*)c->area.ptr;
     fw.sigma_v = sigma_v;
-    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
     mark(c, 1);
     const dim3 grid((unsigned)blocks, (unsigned)((m + kFewM - 1) / kFewM));
     // points on the fly from the vertices (measured faster than reading kept points: 121 instead of
@@ -602,6 +610,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     mark(c, 3);
     c->timing_valid = c->timing;
     c->counters_pending = true;
+    c->counters_counted = true;
     return BEMCUB_OK;
   }
 
@@ -647,7 +656,8 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     fp.ntiles = sp.ntiles;
     fp.nitems = sp.nitems;
     fp.queue = c->d_counters + 2;
-    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    fp.counters = c->d_counters;
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
     const bool phi_only = !grad && !out_E;
     if (grad)
       rc = sp.R == 2 ? launch_fixed<double, 2, kModeGrad>(c, fp, sp) : launch_fixed<double, 1, kModeGrad>(c, fp, sp);
@@ -664,7 +674,8 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     c->stats.point_interactions =
         (c->n_tri * bemcub_rules::kTriN[rule_id] + c->n_rect * bemcub_rules::kRectN[rule_id]) * m;
     c->stats.analytic_pairs = 0;
-    c->counters_pending = false;
+    c->counters_pending = true;
+    c->counters_counted = false;
   } else {
     AdaptiveParams ap;
     for (int l = 0; l < 5; ++l) {
@@ -687,12 +698,13 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     ap.nitems = sp.nitems;
     ap.queue = c->d_counters + 2;
     ap.counters = c->d_counters;
-    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
     if (grad) rc = sp.R == 2 ? launch_adaptive<2, kModeGrad>(c, ap, sp) : launch_adaptive<1, kModeGrad>(c, ap, sp);
     else if (!out_E) rc = sp.R == 4 ? launch_adaptive<4, kModePhi>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2, kModePhi>(c, ap, sp) : launch_adaptive<1, kModePhi>(c, ap, sp);
     else rc = sp.R == 4 ? launch_adaptive<4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
     if (rc) return rc;
     c->counters_pending = true;
+    c->counters_counted = true;
   }
 
   mark(c, 2);
@@ -722,6 +734,39 @@ int bemcub_eval_linear(bemcub_ctx* c, const double* sigma_vertex, int rule_id, c
   return eval_common(c, nullptr, rule_id, host_policy, m, field_pts, out_phi, out_E, nullptr, precision, false, sigma_vertex);
 }
 
+int bemcub_eval_pairs(bemcub_ctx* c, int64_t npairs, const uint8_t* type, const double* verts, const double* sigma, int method,
+                      const bemcub_policy* host_policy, const double* field_pts, double* out_phi, double* out_E, int precision) {
+  if (!c || npairs < 0) return BEMCUB_ERR_INVALID_ARG;
+  if (!((method >= -1 && method <= BEMCUB_METHOD_ANALYTIC) || (method >= BEMCUB_METHOD_DUFFY_L0 && method <= BEMCUB_METHOD_DUFFY_L0 + 4)))
+    return BEMCUB_ERR_BAD_RULE;
+  if (precision != BEMCUB_F64 && precision != BEMCUB_F32) return BEMCUB_ERR_INVALID_ARG;
+  PairsParams pp;
+  if (method == BEMCUB_RULE_ADAPTIVE) {
+    int rc = build_policy(host_policy, &pp.pol);
+    if (rc) return rc;
+  }
+  if (npairs == 0) return BEMCUB_OK;
+  if (!type || !verts || !field_pts || !out_phi) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  pp.K = npairs;
+  pp.type = type;
+  pp.verts = verts;
+  pp.sigma = sigma;
+  pp.method = method;
+  pp.field = field_pts;
+  pp.phi = out_phi;
+  pp.E = out_E;
+  pp.k = coulomb_k();
+  const int threads = 128;
+  const unsigned blocks = (unsigned)((npairs + threads - 1) / threads);
+  if (precision == BEMCUB_F64) eval_pairs_kernel<double><<<blocks, threads, 0, c->stream>>>(pp);
+  else eval_pairs_kernel<float><<<blocks, threads, 0, c->stream>>>(pp);
+  c->stats.kernel_launches += 1;
+  c->stats.last_eval_launches = 1;
+  CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
+
 int bemcub_eval_gradient(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy, int64_t m,
                          const double* field_pts, double* out_phi, double* out_E, double* out_G) {
   if (!out_G) return BEMCUB_ERR_INVALID_ARG;
@@ -738,7 +783,7 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
                          int64_t ld) {
   if (!c) return BEMCUB_ERR_INVALID_ARG;
   if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
-  if (row0 < 0 || nrows < 0 || row0 + nrows > c->n || ld < c->n) return BEMCUB_ERR_INVALID_ARG;
+  if (row0 < 0 || nrows < 0 || row0 + nrows > c->n || ld < c->n || c->n > kAsmMaxN) return BEMCUB_ERR_INVALID_ARG;
   PolicyDev pol;
   int rc = build_policy(host_policy, &pol);
   if (rc) return rc;
@@ -753,9 +798,11 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
     bool used = false;
     for (int w = 0; w <= 5; ++w) used |= (pol.map[w] == l);
     if (used) c->charged64[l] = false;
-    if (used && (rc = expand_level<double>(c, l, nullptr, c->pts64[l]))) return rc;  // unit sigma
+    // unit sigma; every element padded to a multiple of kAsmU points (zero charges): the fill kernel
+    // takes kAsmU points per trip and has no remainder loop
+    ap.stride[l] = (c->stride[l] + kAsmU - 1) / kAsmU * kAsmU;
+    if (used && (rc = expand_level<double>(c, l, nullptr, c->pts64[l], nullptr, ap.stride[l], coulomb_k()))) return rc;
     ap.lvl_pts[l] = (const double4*)c->pts64[l].ptr;
-    ap.stride[l] = c->stride[l];
   }
   ap.cenL = (const double4*)c->cenL.ptr;
   ap.type = (const uint8_t*)c->type.ptr;
@@ -769,7 +816,7 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   ap.k = coulomb_k();
   ap.counters = c->d_counters;
   ap.queue = c->d_counters + 2;
-  CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+  CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
   CUDA_TRY(cudaFuncSetAttribute(assemble_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)assemble_smem_bytes()));
   // items = (64-row tile) x (split of the columns, a multiple of 32): about 32 per warp
   const int64_t warps = (int64_t)c->num_sms * kAsmWarps;
@@ -788,6 +835,7 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   mark(c, 3);
   c->timing_valid = c->timing;
   c->counters_pending = true;
+  c->counters_counted = true;
   return BEMCUB_OK;
 }
 
@@ -836,18 +884,25 @@ int bemcub_eval_host(bemcub_ctx* c, const double* host_sigma, int rule_id, const
   return BEMCUB_OK;
 }
 
-int bemcub_fp64_peak(bemcub_ctx* c, double seconds, double* host_dfma_per_s) {
-  if (!c || !host_dfma_per_s || !(seconds > 0.0) || seconds > 30.0) return BEMCUB_ERR_INVALID_ARG;
+int bemcub_fp64_issue_sweep(bemcub_ctx* c, double seconds_per_variant, double* host_rates, double* host_sm_mhz) {
+  if (!c || !host_rates || !(seconds_per_variant > 0.0) || seconds_per_variant > 10.0) return BEMCUB_ERR_INVALID_ARG;
   DeviceGuard g(c->device);
   const int threads = 256;
-  int rc = ensure(c->partial, (size_t)threads * c->num_sms * 8 * 8);
+  int rc = ensure(c->partial, (size_t)threads * c->num_sms * 4 * 8);
   if (rc) return rc;
   cudaEvent_t e0, e1;
   CUDA_TRY(cudaEventCreate(&e0));
   CUDA_TRY(cudaEventCreate(&e1));
-  auto run = [&](int blocks, int iters, float* ms) -> int {
+  unsigned long long* clk = c->d_counters + 6;
+  auto run = [&](int mix, int blocks, int iters, float* ms) -> int {
     CUDA_TRY(cudaEventRecord(e0, c->stream));
-    dfma_peak_kernel<<<blocks, threads, 0, c->stream>>>((double*)c->partial.ptr, iters, 0.999999, 1e-9);
+    double* out = (double*)c->partial.ptr;
+    switch (mix) {
+      case 0: fp64_issue_kernel<0><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
+      case 1: fp64_issue_kernel<1><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
+      case 2: fp64_issue_kernel<2><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
+      default: fp64_issue_kernel<3><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
+    }
     c->stats.kernel_launches += 1;
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaEventRecord(e1, c->stream));
@@ -855,28 +910,38 @@ int bemcub_fp64_peak(bemcub_ctx* c, double seconds, double* host_dfma_per_s) {
     CUDA_TRY(cudaEventElapsedTime(ms, e0, e1));
     return BEMCUB_OK;
   };
-  // two occupancies (16 and 32 warps per SM); the better sustained rate is the peak
-  double best = 0.0;
-  for (int per_sm = 2; per_sm <= 4; per_sm += 2) {
-    const int blocks = c->num_sms * per_sm;
-    const double per_iter = 64.0 * threads * blocks;  // DFMAs per loop iteration of the whole grid
-    float ms = 0.f;
-    if ((rc = run(blocks, 2000, &ms))) return rc;     // warm-up + calibration
-    if ((rc = run(blocks, 20000, &ms))) return rc;
-    const double rate0 = per_iter * 20000 / (ms * 1e-3);
-    // timed: launches of ~0.25 s each until seconds/2 have elapsed; total work / total time
-    const int iters = (int)std::min(2.0e9, std::max(1000.0, 0.25 * rate0 / per_iter));
-    double total_ms = 0.0, total_fma = 0.0;
-    while (total_ms < 0.5 * seconds * 1e3) {
-      if ((rc = run(blocks, iters, &ms))) return rc;
-      total_ms += ms;
-      total_fma += per_iter * iters;
+  for (int mix = 0; mix < 4; ++mix) {
+    const int chains = mix == 3 ? 18 : 16;
+    for (int occ = 0; occ < 3; ++occ) {
+      const int per_sm = 1 << occ;  // CTAs of 8 warps per SM: 8, 16, 32 warps
+      const int blocks = c->num_sms * per_sm;
+      const double per_iter = 4.0 * chains * threads * blocks;  // FP64 lane-instructions per loop iteration of the grid
+      float ms = 0.f;
+      if ((rc = run(mix, blocks, 2000, &ms))) return rc;  // warm-up
+      if ((rc = run(mix, blocks, 20000, &ms))) return rc;  // calibration
+      const double rate0 = per_iter * 20000 / (ms * 1e-3);
+      // one launch of the requested length: the sustained rate, with the clock it was sustained at
+      const int iters = (int)std::min(2.0e9, std::max(1000.0, seconds_per_variant * rate0 / per_iter));
+      if ((rc = run(mix, blocks, iters, &ms))) return rc;
+      host_rates[mix * 3 + occ] = per_iter * iters / (ms * 1e-3);
+      if (host_sm_mhz) {
+        unsigned long long h[2] = {0, 0};
+        CUDA_TRY(cudaMemcpy(h, clk, sizeof(h), cudaMemcpyDeviceToHost));
+        host_sm_mhz[mix * 3 + occ] = h[1] ? 1e3 * (double)h[0] / (double)h[1] : 0.0;
+      }
     }
-    best = std::max(best, total_fma / (total_ms * 1e-3));
   }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
-  *host_dfma_per_s = best;
+  return BEMCUB_OK;
+}
+
+int bemcub_fp64_peak(bemcub_ctx* c, double seconds, double* host_fp64_inst_per_s) {
+  if (!c || !host_fp64_inst_per_s || !(seconds > 0.0) || seconds > 30.0) return BEMCUB_ERR_INVALID_ARG;
+  double rates[BEMCUB_PEAK_VARIANTS];
+  int rc = bemcub_fp64_issue_sweep(c, seconds / BEMCUB_PEAK_VARIANTS, rates, nullptr);
+  if (rc) return rc;
+  *host_fp64_inst_per_s = *std::max_element(rates, rates + BEMCUB_PEAK_VARIANTS);
   return BEMCUB_OK;
 }
 

@@ -48,22 +48,39 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst_smem, const void* src_g
 }
 
 // ---- reciprocal square root ------------------------------------------------------------------
-// MUFU.RSQ64H seed (reads only the high word of x, ~2^-20 relative error) ...
+// What bounds the hot loops is the ISSUE port, not latency (profiles/r2_issue_model.md):
+// an FP64 instruction holds a scheduler's dispatch for 2 cycles, 3 if it reads three distinct vector
+// registers that are not in the operand-reuse cache, and every other instruction (MUFU, MOV, LDS,
+// loop bookkeeping) takes a cycle of its own.  The refinement below is written for that model.
+//
+// MUFU.RSQ64H seed: reads only the high word of x and writes only the HIGH word of its result
+// (~2^-20 relative error).  The PTX instruction returns the seed with a zero low word, which costs
+// a MOV per call.  rsqrt_f64 instead takes the low word from `dead`, a value the caller does not
+// need any more (an intermediate of x): ptxas then lets MUFU write into the high half of that
+// value's register pair and the MOV disappears.  Any low word will do - it moves the seed by
+// < 2^-20 of its value, which the correction below absorbs - and this one is a function of the
+// interaction's own data, so results stay bit-reproducible.
 __device__ __forceinline__ double rsqrt_seed(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   return y;
 }
+// 0.375 of the correction polynomial.  DFMA takes one immediate only (the 0.5), so this constant
+// lives in a register; read from constant memory it cannot be re-materialised inside the loop
+// (two MOVs per trip when written as a literal).
+__constant__ double c_three_eighths = 0.375;
+
 // ... and one third-order correction y = y0 (1 + e/2 + 3e^2/8), e = 1 - x y0^2 : 5 FP64 instructions,
-// residual (5/16) e^3 ~ 2^-60.  (A second-order step would leave ~4e-12: not enough for the
-// 1e-12 parity bar nor for the paper's 1e-15 accuracy level.)
-__device__ __forceinline__ double rsqrt_f64(double x) {
-  const double y0 = rsqrt_seed(x);
+// residual (5/16) e^3 < 2^-57 for |e| < 2^-18.  (A second-order step would leave ~4e-12: not enough
+// for the 1e-12 parity bar nor for the paper's 1e-15 accuracy level.)  Written as
+// y = fma(y0, e p, y0): two distinct registers, where fma(y0 e, p, y0) reads three.
+__device__ __forceinline__ double rsqrt_f64(double x, double dead, double c375) {
+  const double y0 = __hiloint2double(__double2hiint(rsqrt_seed(x)), __double2loint(dead));
   const double t = __dmul_rn(x, y0);
   const double e = __fma_rn(-t, y0, 1.0);
-  const double p = __fma_rn(0.375, e, 0.5);
-  const double ye = __dmul_rn(y0, e);
-  return __fma_rn(ye, p, y0);
+  const double p = __fma_rn(c375, e, 0.5);
+  const double u = __dmul_rn(e, p);
+  return __fma_rn(y0, u, y0);
 }
 __device__ __forceinline__ float rsqrt_f32(float x) {
   float y;
@@ -79,6 +96,32 @@ __device__ __forceinline__ double4 ldg4(const double4* p) {
   const double2 b = __ldg(reinterpret_cast<const double2*>(p) + 1);
   return make_double4(a.x, a.y, b.x, b.y);
 }
+
+// ---- SM clock actually seen by a kernel ---------------------------------------------------------
+// Thread 0 of CTA 0 (a persistent CTA lives as long as the launch) reads the SM cycle counter and the
+// global nanosecond timer at both ends; counters[4] = cycles, counters[5] = ns.  cycles / ns is the
+// clock the kernel really ran at - the denominator of the per-cycle roofline (bench.py).
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+struct KernelClock {
+  long long c0;
+  unsigned long long t0;
+  __device__ __forceinline__ void begin() {
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
+      c0 = clock64();
+      t0 = global_timer_ns();
+    }
+  }
+  __device__ __forceinline__ void end(unsigned long long* counters) {
+    if (counters && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
+      counters[4] = (unsigned long long)(clock64() - c0);
+      counters[5] = global_timer_ns() - t0;
+    }
+  }
+};
 
 // ---- warp helpers ----------------------------------------------------------------------------
 __device__ __forceinline__ double warp_min(double v) {

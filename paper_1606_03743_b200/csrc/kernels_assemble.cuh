@@ -5,22 +5,31 @@
 //
 // Same execution model as the evaluation kernels (kernels_eval.cuh): persistent CTAs, every warp
 // pulls items from an atomic queue (16 warps per SM here).  One item = (tile of 64 rows) x (split of
-// the columns).  A lane owns rows i0 + lane and i0 + 32 + lane (their centroids sit in registers).  Columns are taken 32 at a
-// time: lane l classifies column j0+l against the bounding sphere of the row centroids, so the
-// rule of a column is warp-uniform unless the tile straddles a band limit (then: the more accurate
-// rule, or the exact per-pair choice with masks).  The point records of the batch's columns are
-// streamed through the warp's double-buffered shared-memory window by bulk TMA, whole elements per
-// stage, with a small segment table (column, first point, number of points) beside each stage.
-// Results of 8 consecutive columns go through a padded 64 x 8 shared-memory tile and leave as
-// 64-byte row segments (two full 32-byte sectors each, four rows per store instruction); the
-// rare analytic / pair-by-pair entries are stored directly while the first TMA copies fly.
+// the columns).  A lane owns rows i0 + lane and i0 + 32 + lane (their centroids sit in registers).
+// Columns are taken 32 at a time: lane l classifies column j0+l against the bounding sphere of the
+// row centroids, so the rule of a column is warp-uniform unless the tile straddles a band limit
+// (then: the more accurate rule, or the exact per-pair choice with masks).  The point records of the
+// batch's columns are streamed through the warp's double-buffered shared-memory window by bulk TMA,
+// whole elements per stage, with a small segment table (column, first point, number of points)
+// beside each stage.
+//
+// The kernel is bound by the issue port, so everything around the 12 FP64
+// instructions of an interaction is kept short:
+//  * the elements are expanded with k folded into the charges and padded with zero charges to a
+//    multiple of kAsmU points, so a column is whole trips of kAsmU points and its sum needs neither a
+//    remainder loop nor a final scaling;
+//  * results of 8 consecutive columns go through a 64 x 8 shared-memory tile and leave as 64-byte row
+//    segments, each lane storing its own rows with four 16-byte stores;
+//  * entries below the analytic limit are not evaluated where they are met (a warp-wide call for a
+//    handful of rows): their (row, column) pairs are queued in shared memory and evaluated 32 at a
+//    time, one pair per lane.
 #pragma once
 #include "kernels_eval.cuh"
 
 namespace bemcub {
 
 struct AssembleParams {
-  const double4* lvl_pts[5];  // unit-sigma points per level
+  const double4* lvl_pts[5];  // unit-sigma points per level, charges times k, padded (see above)
   int stride[5];
   const double4* cenL;
   const uint8_t* type;
@@ -39,66 +48,60 @@ struct AssembleParams {
 
 constexpr int kAsmWarps = 16;
 constexpr int kAsmThreads = kAsmWarps * 32;
-constexpr int kAsmR = 2;              // rows per lane
-constexpr int kAsmRows = 32 * kAsmR;  // rows per tile
+constexpr int kAsmR = 2;               // rows per lane
+constexpr int kAsmU = 4;               // points per trip; the expanded elements are padded to a multiple of it
+constexpr int kAsmRows = 32 * kAsmR;   // rows per tile
 constexpr int kGroupCols = 8;          // columns per output group: 64-byte row segments = two full sectors
-constexpr int kTilePad = kGroupCols + 1;
+constexpr int kTilePad = kGroupCols + 2;  // row stride of the output tile: 16-byte aligned rows
+constexpr int kAqCap = 128;            // analytic pair queue (ring), entries = row << 26 | column
+constexpr int64_t kAsmMaxN = (int64_t)1 << 26;  // ... hence this many elements at most (a 2^26-square matrix is out of reach anyway)
 
-// per-warp shared memory: window | output tile | segment tables | mbarriers | scratch
+// per-warp shared memory: window | output tile | segment tables | analytic queue | mbarriers | tallies
 struct AsmWarpSmem {
   double4 win[kStages][kBuf];
   double tile[kAsmRows * kTilePad];
   uint32_t seg[kStages][32];  // col | npts << 8 | first << 16
+  uint32_t aq[kAqCap];
   uint64_t bar[kStages];
-  WarpScratch scr;
+  unsigned long long n_inter, n_ana;
 };
 constexpr size_t assemble_smem_bytes() { return (size_t)kAsmWarps * sizeof(AsmWarpSmem); }
 
 // Potential-only term of Eq. 4.1: 12 FP64-pipe instructions (3 DADD + 3 DMUL + 6 DFMA).
-__device__ __forceinline__ double phi_one(const double4 s, double q, double px, double py, double pz, double acc) {
+__device__ __forceinline__ double phi_one(const double4 s, double q, double px, double py, double pz, double acc, double c375) {
   const double dx = __dsub_rn(px, s.x), dy = __dsub_rn(py, s.y), dz = __dsub_rn(pz, s.z);
   const double r2 = __fma_rn(dx, dx, __fma_rn(dy, dy, __dmul_rn(dz, dz)));
-  return __fma_rn(q, rsqrt_f64(r2), acc);
+  return __fma_rn(q, rsqrt_f64(r2, dz, c375), acc);
 }
 
-// One element's points (already in shared memory) against the lane's kAsmR rows, U points per
-// trip with their own partial sums: 8 independent chains per lane (measured: 64-row tiles x 4
-// points, 16 warps/SM, beat 128-row tiles x 2 points, 12 warps/SM, by 2 % and 5 % fewer points).
+// One element's points (already in shared memory; npts a multiple of kAsmU thanks to the zero-charge
+// padding) against the lane's kAsmR rows, kAsmU points per trip with their own partial sums:
+// kAsmU * kAsmR = 8 independent chains per lane.
 __device__ __forceinline__ void phi_segment(const double4* __restrict__ pts, int npts, const double (&px)[kAsmR],
-                                            const double (&py)[kAsmR], const double (&pz)[kAsmR], double (&acc)[kAsmR]) {
-  constexpr int U = 8 / kAsmR;  // points per trip: U * kAsmR = 8 independent chains
+                                            const double (&py)[kAsmR], const double (&pz)[kAsmR], double (&acc)[kAsmR],
+                                            double c375) {
+  constexpr int U = kAsmU;
   double part[U][kAsmR];
 #pragma unroll
   for (int u = 0; u < U; ++u)
 #pragma unroll
     for (int r = 0; r < kAsmR; ++r) part[u][r] = 0.0;
-  int i = 0;
 #pragma unroll 1
-  for (; i + U <= npts; i += U) {
+  for (int i = 0; i < npts; i += U) {
     double4 s[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) s[u] = pts[i + u];
 #pragma unroll
     for (int u = 0; u < U; ++u)
 #pragma unroll
-      for (int r = 0; r < kAsmR; ++r) part[u][r] = phi_one(s[u], s[u].w, px[r], py[r], pz[r], part[u][r]);
-  }
-#pragma unroll 1
-  for (; i < npts; ++i) {
-    const double4 s = pts[i];
-#pragma unroll
-    for (int r = 0; r < kAsmR; ++r) part[0][r] = phi_one(s, s.w, px[r], py[r], pz[r], part[0][r]);
+      for (int r = 0; r < kAsmR; ++r) part[u][r] = phi_one(s[u], s[u].w, px[r], py[r], pz[r], part[u][r], c375);
   }
 #pragma unroll
-  for (int r = 0; r < kAsmR; ++r) {
-    double t = part[0][r];
-#pragma unroll
-    for (int u = 1; u < U; ++u) t += part[u][r];
-    acc[r] = t;
-  }
+  for (int r = 0; r < kAsmR; ++r) acc[r] = (part[0][r] + part[1][r]) + (part[2][r] + part[3][r]);
 }
 
 __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_constant__ AssembleParams p) {
+  static_assert(kAsmU == 4, "phi_segment adds four partial sums");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   AsmWarpSmem& sm = reinterpret_cast<AsmWarpSmem*>(smem_raw)[warp];
@@ -107,12 +110,17 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
     mbar_init(bar0, 1);
     mbar_init(bar0 + 8, 1);
     mbar_fence_init();
-    sm.scr.n_inter = 0;
-    sm.scr.n_ana = 0;
+    sm.n_inter = 0;
+    sm.n_ana = 0;
   }
   __syncwarp();
   uint32_t phases = 0;
   const unsigned lt_mask = (1u << lane) - 1u;
+  const double c375 = c_three_eighths;
+  // 16-byte stores of whole 8-column groups need even ld and an aligned base
+  const bool vec_ok = ((p.ld & 1) == 0) && ((reinterpret_cast<uintptr_t>(p.out) & 15u) == 0);
+  KernelClock clk;
+  clk.begin();
 
   for (;;) {
     const int64_t item = next_item(p.queue, lane);
@@ -148,13 +156,35 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
     const double rho = sqrt(warp_max(d2));
     const double mag = fmax(fmax(fabs(cx), fabs(cy)), fabs(cz)) + rho;
 
+    // analytic pair queue of this item: [aq_head, aq_tail) in the ring sm.aq
+    int aq_head = 0, aq_tail = 0;
+    // Evaluates `take` (<= 32) queued pairs, one per lane: entry = row << 26 | column.
+    auto drain = [&](int take) {
+      __syncwarp();
+      if (lane < take) {
+        const uint32_t ent = sm.aq[(aq_head + lane) & (kAqCap - 1)];
+        const int row = (int)(ent >> 26);
+        const int64_t col = (int64_t)(ent & 0x3ffffffu);
+        const double4 ci = ldg4(p.cenL + p.row0 + r0 + row);
+        Vec3 V[4];
+        const int nv = load_polygon(p.type, p.verts, col, V);
+        double ip;
+        Vec3 ie;
+        analytic_integrals<false>(V, nv, Vec3{ci.x, ci.y, ci.z}, ip, ie);
+        p.out[(r0 + row) * p.ld + col] = p.k * ip;
+      }
+      aq_head += take;
+      __syncwarp();
+    };
+
     const int64_t col_begin = split * p.cols_per_split;
     const int64_t col_end = min(p.n, col_begin + p.cols_per_split);
     for (int64_t j0 = col_begin; j0 < col_end; j0 += 32) {
       const int ncol = (int)min((int64_t)32, col_end - j0);
       // ---- classify column j0 + lane against the row tile's bounding sphere
       const int64_t e = j0 + lane;
-      int cnt = 0, lvl = -1;
+      int cnt = 0, lvl = -1;  // cnt: the column's points in the stream, zero-charge padding included
+      int real = 0;           // ... and without it
       bool is_ana = false, is_mixed = false, is_fix = false;
       const double4* src = nullptr;
       if (lane < ncol) {
@@ -173,20 +203,21 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
           // cubature rule, and the rows below the limit are overwritten analytically afterwards
           is_fix = true;
           lvl = p.pol.map[4];
-          cnt = rule_npts(t, lvl);
-          src = p.lvl_pts[lvl] + e * p.stride[lvl];
         } else if (lnear != lfar && (!p.pol.allow_upgrade || lnear == 5)) {
           is_mixed = true;
         } else {
           lvl = lnear;
-          if (lvl == 5) {
-            is_ana = true;
-          } else {
-            cnt = rule_npts(t, lvl);
-            src = p.lvl_pts[lvl] + e * p.stride[lvl];
-          }
+          is_ana = lvl == 5;
+        }
+        if (lvl >= 0 && lvl < 5) {
+          real = rule_npts(t, lvl);
+          cnt = (real + kAsmU - 1) / kAsmU * kAsmU;
+          src = p.lvl_pts[lvl] + e * p.stride[lvl];
         }
       }
+      // point-charge interactions of the batch's streamed columns (padding not counted)
+      const int real_pts = warp_sum(real);
+      if (lane == 0) sm.n_inter += (unsigned long long)real_pts * nrow_here;
       int total;
       const int pre = warp_excl_scan(cnt, lane, &total);
       int cursor = 0;
@@ -215,10 +246,7 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
           cursor = next;
           if (nstage == 0) continue;
           if (inc) sm.seg[stage][__popc(incmask & lt_mask)] = (uint32_t)lane | ((uint32_t)cnt << 8) | ((uint32_t)(pre - base) << 16);
-          if (lane == 0) {
-            mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
-            sm.scr.n_inter += (unsigned long long)nstage * nrow_here;
-          }
+          if (lane == 0) mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
           __syncwarp();
           if (inc && !cont)
             tma_load_1d(win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
@@ -232,11 +260,26 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
       auto flush_group = [&]() {
         __syncwarp();
         if (cur_group >= 0) {
-          const int c = lane & (kGroupCols - 1);
-          const int64_t j = j0 + cur_group * kGroupCols + c;
-          if ((gmask >> c) & 1u) {
-#pragma unroll 4
-            for (int row = lane >> 3; row < nrow_here; row += 4) p.out[(r0 + row) * p.ld + j] = sm.tile[row * kTilePad + c];
+          const int64_t jg = j0 + cur_group * kGroupCols;
+          if (gmask == 0xffu && vec_ok) {
+            // all 8 columns present: every lane stores the 64 bytes of each of its rows
+#pragma unroll
+            for (int r = 0; r < kAsmR; ++r) {
+              const int row = r * 32 + lane;
+              if (row < nrow_here) {
+                const double2* t = reinterpret_cast<const double2*>(&sm.tile[row * kTilePad]);
+                double2* o = reinterpret_cast<double2*>(p.out + (r0 + row) * p.ld + jg);
+                const double2 a = t[0], b = t[1], c = t[2], d = t[3];
+                o[0] = a; o[1] = b; o[2] = c; o[3] = d;
+              }
+            }
+          } else {
+            const int c = lane & (kGroupCols - 1);
+            if ((gmask >> c) & 1u) {
+              double* o = p.out + (r0 + (lane >> 3)) * p.ld + jg + c;
+              const double* t = &sm.tile[(lane >> 3) * kTilePad + c];
+              for (int row = lane >> 3; row < nrow_here; row += 4, o += 4 * p.ld, t += 4 * kTilePad) *o = *t;
+            }
           }
         }
         __syncwarp();
@@ -253,9 +296,9 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
             gmask = 0;
           }
           double acc[kAsmR];
-          phi_segment(&sm.win[stage][d >> 16], (int)((d >> 8) & 255u), px, py, pz, acc);
+          phi_segment(&sm.win[stage][d >> 16], (int)((d >> 8) & 255u), px, py, pz, acc, c375);
 #pragma unroll
-          for (int r = 0; r < kAsmR; ++r) sm.tile[(r * 32 + lane) * kTilePad + (col & (kGroupCols - 1))] = p.k * acc[r];
+          for (int r = 0; r < kAsmR; ++r) sm.tile[(r * 32 + lane) * kTilePad + (col & (kGroupCols - 1))] = acc[r];
           gmask |= 1u << (col & (kGroupCols - 1));
         }
         __syncwarp();
@@ -263,23 +306,9 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
 
       int na = fill(0);
       int nb = na ? fill(1) : 0;
-      // while the first copies fly: this batch's special columns, stored directly
-      unsigned amask = __ballot_sync(kFullMask, is_ana), xmask = __ballot_sync(kFullMask, is_mixed);
-      if (amask && lane == 0) sm.scr.n_ana += (unsigned long long)__popc(amask) * nrow_here;
-      while (amask) {
-        const int l = __ffs(amask) - 1;
-        amask &= amask - 1;
-        Vec3 V[4];
-        const int nv = load_polygon(p.type, p.verts, j0 + l, V);
-#pragma unroll
-        for (int r = 0; r < kAsmR; ++r) {
-          double ip;
-          Vec3 ie;
-          analytic_integrals<false>(V, nv, Vec3{px[r], py[r], pz[r]}, ip, ie);
-          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j0 + l] = p.k * ip;
-        }
-      }
-      while (xmask) {  // exact per-pair choice
+      // while the first copies fly: the rare columns that need the exact per-pair choice, stored directly
+      unsigned xmask = __ballot_sync(kFullMask, is_mixed);
+      while (xmask) {
         const int l = __ffs(xmask) - 1;
         xmask &= xmask - 1;
         const int64_t j = j0 + l;
@@ -315,32 +344,25 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
               double ip;
               Vec3 ie;
               analytic_integrals<false>(V, nv, Vec3{px[r], py[r], pz[r]}, ip, ie);
-              val[r] = ip;
+              val[r] = p.k * ip;
             }
-            if (lane == 0) sm.scr.n_ana += (unsigned long long)all;
+            if (lane == 0) sm.n_ana += (unsigned long long)all;
           } else {
+            // the same arithmetic, in the same order, as the streamed columns (phi_segment on the
+            // padded record list, read from global memory here): an entry does not depend on the
+            // tile it was computed in
             const int N = rule_npts(t, lv);
-            const double4* sp = p.lvl_pts[lv] + j * p.stride[lv];
             double acc[kAsmR];
-#pragma unroll
-            for (int r = 0; r < kAsmR; ++r) acc[r] = 0.0;
-            double4 s = ldg4(sp);
-#pragma unroll 1
-            for (int i = 0; i < N; ++i) {
-              const double4 nxt = ldg4(sp + min(i + 1, N - 1));
-#pragma unroll
-              for (int r = 0; r < kAsmR; ++r) acc[r] = phi_one(s, s.w, px[r], py[r], pz[r], acc[r]);
-              s = nxt;
-            }
+            phi_segment(p.lvl_pts[lv] + j * p.stride[lv], (N + kAsmU - 1) / kAsmU * kAsmU, px, py, pz, acc, c375);
 #pragma unroll
             for (int r = 0; r < kAsmR; ++r)
               if (take[r]) val[r] = acc[r];
-            if (lane == 0) sm.scr.n_inter += (unsigned long long)all * N;
+            if (lane == 0) sm.n_inter += (unsigned long long)all * N;
           }
         }
 #pragma unroll
         for (int r = 0; r < kAsmR; ++r)
-          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j] = p.k * val[r];
+          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j] = val[r];
       }
       // ---- streamed columns
       for (;;) {
@@ -352,47 +374,39 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
         nb = fill(1);
       }
       flush_group();
-      // ---- rows of the straddling columns that lie below the analytic limit (exact per-pair test)
-      unsigned fmask = __ballot_sync(kFullMask, is_fix);
-      while (fmask) {
-        const int l = __ffs(fmask) - 1;
-        fmask &= fmask - 1;
+      // ---- entries below the analytic limit: every row of a column the whole tile sees that near,
+      // and - by the exact per-pair test - the rows of the straddling columns streamed above (their
+      // cubature values are overwritten: flush_group has synchronised the warp).  Queued, then
+      // evaluated one pair per lane.
+      unsigned qmask = __ballot_sync(kFullMask, is_ana || is_fix);
+      while (qmask) {
+        const int l = __ffs(qmask) - 1;
+        qmask &= qmask - 1;
         const int64_t j = j0 + l;
         const double4 c = ldg4(p.cenL + j);
         const int t = __ldg(p.type + j);
-        bool take[kAsmR];
-        bool any = false;
-        int mine = 0;
 #pragma unroll
         for (int r = 0; r < kAsmR; ++r) {
           const double dx = __dsub_rn(px[r], c.x), dy = __dsub_rn(py[r], c.y), dz = __dsub_rn(pz[r], c.z);
           const double D2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-          take[r] = p.pol.map[want_level(D2, c.w, p.pol.dr[t])] == 5;
-          any |= take[r];
-          mine += (take[r] && ok[r]) ? 1 : 0;
+          const bool take = ok[r] && p.pol.map[want_level(D2, c.w, p.pol.dr[t])] == 5;
+          const unsigned bal = __ballot_sync(kFullMask, take);
+          if (take) sm.aq[(aq_tail + __popc(bal & lt_mask)) & (kAqCap - 1)] = ((uint32_t)(r * 32 + lane) << 26) | (uint32_t)j;
+          aq_tail += __popc(bal);
         }
-        if (!__any_sync(kFullMask, any)) continue;
-        const int all = warp_sum(mine);
-        if (lane == 0) sm.scr.n_ana += (unsigned long long)all;
-        Vec3 V[4];
-        const int nv = load_polygon(p.type, p.verts, j, V);
-#pragma unroll
-        for (int r = 0; r < kAsmR; ++r) {
-          if (!take[r]) continue;
-          double ip;
-          Vec3 ie;
-          analytic_integrals<false>(V, nv, Vec3{px[r], py[r], pz[r]}, ip, ie);
-          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j] = p.k * ip;
-        }
+        while (aq_tail - aq_head >= 32) drain(32);
       }
     }
+    if (lane == 0) sm.n_ana += (unsigned long long)aq_tail;
+    if (aq_tail > aq_head) drain(aq_tail - aq_head);
   }
 
   __syncwarp();
   if (p.counters && lane == 0) {
-    if (sm.scr.n_inter) atomicAdd(p.counters, sm.scr.n_inter);
-    if (sm.scr.n_ana) atomicAdd(p.counters + 1, sm.scr.n_ana);
+    if (sm.n_inter) atomicAdd(p.counters, sm.n_inter);
+    if (sm.n_ana) atomicAdd(p.counters + 1, sm.n_ana);
   }
+  clk.end(p.counters);
 }
 
 }  // namespace bemcub

@@ -35,6 +35,10 @@ constexpr int kWarpsPerCta = 12;  // 1 CTA per SM, 3 warps per scheduler, <= 168
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kBuf = 128;  // points per stage of a warp's window
 constexpr int kStages = 2;
+#ifndef BEMCUB_UNROLL_R4
+#define BEMCUB_UNROLL_R4 1
+#endif
+constexpr int kUnrollR4 = BEMCUB_UNROLL_R4;  // source points per trip of the R = 4 loops
 
 // Per-warp bookkeeping kept in shared memory (not registers): bounding sphere of the current tile
 // and the interaction tallies.
@@ -42,6 +46,12 @@ struct WarpScratch {
   double cx, cy, cz, rho, mag;
   unsigned long long n_inter, n_ana;
   int nvalid, pad;
+  // state of the adaptive kernel's current 32-element batch (lane l = element batch0 + l), parked here
+  // between two produce() calls so that the consume loop has the registers to itself
+  const double4* src[32];
+  int cnt[32], pre[32], lvl[32];
+  int64_t batch_next;
+  int total, cursor;
 };
 
 // shared memory of one CTA: [warps][stages][kBuf] points | [warps][stages] mbarriers | [warps] scratch
@@ -79,10 +89,11 @@ struct Accum {
 
 // One point charge (sx,sy,sz,q) seen from one field point: Eq. 4.1 term.
 __device__ __forceinline__ void interact_one(double sx, double sy, double sz, double q, double px, double py, double pz,
-                                             double& phi, double& ex, double& ey, double& ez) {
+                                             double& phi, double& ex, double& ey, double& ez, double c375) {
   const double dx = __dsub_rn(px, sx), dy = __dsub_rn(py, sy), dz = __dsub_rn(pz, sz);
-  const double r2 = __fma_rn(dx, dx, __fma_rn(dy, dy, __dmul_rn(dz, dz)));
-  const double y = rsqrt_f64(r2);  // 1/|P-Q_i|: "one square root and one division" (L46)
+  const double yz = __fma_rn(dy, dy, __dmul_rn(dz, dz));
+  const double r2 = __fma_rn(dx, dx, yz);
+  const double y = rsqrt_f64(r2, yz, c375);  // 1/|P-Q_i|: "one square root and one division" (L46)
   const double qy = __dmul_rn(q, y);
   phi = __dadd_rn(phi, qy);
   const double y2 = __dmul_rn(y, y);
@@ -93,12 +104,13 @@ __device__ __forceinline__ void interact_one(double sx, double sy, double sz, do
 }
 // Potential only: 12 FP64-pipe instructions (3 DADD + 3 DMUL + 6 DFMA).
 __device__ __forceinline__ void interact_one_phi(double sx, double sy, double sz, double q, double px, double py, double pz,
-                                                 double& phi) {
+                                                 double& phi, double c375) {
   const double dx = __dsub_rn(px, sx), dy = __dsub_rn(py, sy), dz = __dsub_rn(pz, sz);
   const double r2 = __fma_rn(dx, dx, __fma_rn(dy, dy, __dmul_rn(dz, dz)));
-  phi = __fma_rn(q, rsqrt_f64(r2), phi);
+  phi = __fma_rn(q, rsqrt_f64(r2, dz, c375), phi);
 }
-__device__ __forceinline__ void interact_one_phi(float sx, float sy, float sz, float q, float px, float py, float pz, float& phi) {
+__device__ __forceinline__ void interact_one_phi(float sx, float sy, float sz, float q, float px, float py, float pz, float& phi,
+                                                 double) {
   const float dx = px - sx, dy = py - sy, dz = pz - sz;
   phi = fmaf(q, rsqrt_f32(fmaf(dx, dx, fmaf(dy, dy, dz * dz))), phi);
 }
@@ -106,10 +118,11 @@ __device__ __forceinline__ void interact_one_phi(float sx, float sy, float sz, f
 // s_zz is never formed: h r^2 = 3 g makes the gradient traceless, G_zz = -(G_xx + G_yy).
 __device__ __forceinline__ void interact_one_grad(double sx, double sy, double sz, double q, double px, double py, double pz,
                                                   double& phi, double& ex, double& ey, double& ez, double& sg, double& sxx,
-                                                  double& syy, double& sxy, double& sxz, double& syz) {
+                                                  double& syy, double& sxy, double& sxz, double& syz, double c375) {
   const double dx = __dsub_rn(px, sx), dy = __dsub_rn(py, sy), dz = __dsub_rn(pz, sz);
-  const double r2 = __fma_rn(dx, dx, __fma_rn(dy, dy, __dmul_rn(dz, dz)));
-  const double y = rsqrt_f64(r2);
+  const double yz = __fma_rn(dy, dy, __dmul_rn(dz, dz));
+  const double r2 = __fma_rn(dx, dx, yz);
+  const double y = rsqrt_f64(r2, yz, c375);
   const double qy = __dmul_rn(q, y);
   phi = __dadd_rn(phi, qy);
   const double y2 = __dmul_rn(y, y);
@@ -127,7 +140,7 @@ __device__ __forceinline__ void interact_one_grad(double sx, double sy, double s
   syz = __fma_rn(hy, dz, syz);
 }
 __device__ __forceinline__ void interact_one(float sx, float sy, float sz, float q, float px, float py, float pz,
-                                             float& phi, float& ex, float& ey, float& ez) {
+                                             float& phi, float& ex, float& ey, float& ez, double) {
   const float dx = px - sx, dy = py - sy, dz = pz - sz;
   const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
   const float y = rsqrt_f32(r2);
@@ -141,16 +154,16 @@ __device__ __forceinline__ void interact_one(float sx, float sy, float sz, float
 
 template <typename T, int R, int MODE, typename P4>
 __device__ __forceinline__ void interact(const P4 s, const T (&px)[R], const T (&py)[R], const T (&pz)[R],
-                                         Accum<T, R, MODE>& a) {
+                                         Accum<T, R, MODE>& a, double c375) {
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     if constexpr (MODE == kModeGrad)
       interact_one_grad(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], a.ex[r], a.ey[r], a.ez[r], a.sg[r], a.sxx[r],
-                        a.syy[r], a.sxy[r], a.sxz[r], a.syz[r]);
+                        a.syy[r], a.sxy[r], a.sxz[r], a.syz[r], c375);
     else if constexpr (MODE == kModePhi)
-      interact_one_phi(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r]);
+      interact_one_phi(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], c375);
     else
-      interact_one(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], a.ex[r], a.ey[r], a.ez[r]);
+      interact_one(s.x, s.y, s.z, s.w, px[r], py[r], pz[r], a.phi[r], a.ex[r], a.ey[r], a.ez[r], c375);
   }
 }
 
@@ -159,7 +172,8 @@ __device__ __forceinline__ void interact(const P4 s, const T (&px)[R], const T (
 template <typename T, int R, int MODE, typename P4>
 __device__ __forceinline__ void consume(const P4* __restrict__ buf, int cnt, const T (&px)[R], const T (&py)[R],
                                         const T (&pz)[R], Accum<T, R, MODE>& a) {
-  constexpr int U = R >= 4 ? 1 : (R >= 2 ? 2 : 4);
+  constexpr int U = R >= 4 ? kUnrollR4 : (R >= 2 ? 2 : 4);
+  const double c375 = c_three_eighths;
   int i = 0;
 #pragma unroll 1
   for (; i + U <= cnt; i += U) {
@@ -167,10 +181,10 @@ __device__ __forceinline__ void consume(const P4* __restrict__ buf, int cnt, con
 #pragma unroll
     for (int u = 0; u < U; ++u) s[u] = buf[i + u];
 #pragma unroll
-    for (int u = 0; u < U; ++u) interact<T, R, MODE>(s[u], px, py, pz, a);
+    for (int u = 0; u < U; ++u) interact<T, R, MODE>(s[u], px, py, pz, a, c375);
   }
 #pragma unroll 1
-  for (; i < cnt; ++i) interact<T, R, MODE>(buf[i], px, py, pz, a);
+  for (; i < cnt; ++i) interact<T, R, MODE>(buf[i], px, py, pz, a, c375);
 }
 
 // FP64: the window's sum goes straight into the running totals.  FP32: the window (<= kBuf
@@ -269,6 +283,7 @@ struct FixedParams {
   int64_t ntiles;           // ceil(m / (32 R))
   int64_t nitems;           // ntiles * nsplit; item = split * ntiles + tile
   unsigned long long* queue;  // work-item counter, zeroed before the launch
+  unsigned long long* counters;  // [4], [5]: cycles and nanoseconds of the launch (KernelClock)
 };
 
 template <typename T, int R, int MODE = kModePhiE>
@@ -279,6 +294,8 @@ __global__ void __launch_bounds__(kThreads, 1) eval_fixed_kernel(const __grid_co
   const WarpSmem<P4> ws = warp_smem<P4>(smem_raw, warp, lane);
   const P4* src = reinterpret_cast<const P4*>(p.pts);
   uint32_t phases = 0;  // parity of each stage's mbarrier, carried across items
+  KernelClock clk;
+  clk.begin();
 
   for (;;) {
     const int64_t item = next_item(p.queue, lane);
@@ -314,6 +331,7 @@ __global__ void __launch_bounds__(kThreads, 1) eval_fixed_kernel(const __grid_co
     store_partial<R, MODE>(p.partial + split * p.split_stride, (MODE == kModeGrad) ? p.partial_g + split * p.split_stride * 6 : nullptr, p.m,
                            tile, lane, tot);
   }
+  clk.end(p.counters);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -436,10 +454,11 @@ __device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e
       Accum<double, R, MODE> part;
       part.zero();
       double4 s = ldg4(src);
+      const double c375 = c_three_eighths;
 #pragma unroll 1
       for (int i = 0; i < N; ++i) {
         const double4 nxt = ldg4(src + min(i + 1, N - 1));  // prefetch: hides the global-load latency
-        interact<double, R, MODE>(s, w.px, w.py, w.pz, part);
+        interact<double, R, MODE>(s, w.px, w.py, w.pz, part, c375);
         s = nxt;
       }
 #pragma unroll
@@ -472,6 +491,8 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
   const WarpSmem<double4> ws = warp_smem<double4>(smem_raw, warp, lane);
   WarpScratch* const scr = ws.scr;
   uint32_t phases = 0;
+  KernelClock clk;
+  clk.begin();
 
   for (;;) {
     const int64_t item = next_item(p.queue, lane);
@@ -529,13 +550,24 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     Accum<double, R, MODE> tot;
     tot.zero();
 
-    // state of the current 32-element batch: lane l holds element batch0 + l
-    int64_t batch_next = e_begin;
-    int cnt = 0, pre = 0, total = 0, lvl = 0, cursor = 32;
-    const double4* src = nullptr;
+    // state of the current 32-element batch (lane l holds element batch0 + l) lives in the warp's
+    // scratch between two produce() calls: see WarpScratch
+    if (lane == 0) {
+      scr->batch_next = e_begin;
+      scr->total = 0;
+      scr->cursor = 32;
+    }
+    scr->cnt[lane] = 0;
+    scr->pre[lane] = 0;
+    scr->lvl[lane] = 0;
+    __syncwarp();
 
     // Fills `stage` with the next round of whole elements; returns the number of points (0 = done).
     auto produce = [&](int stage) -> int {
+      int64_t batch_next = scr->batch_next;
+      int cursor = scr->cursor, total = scr->total;
+      int cnt = scr->cnt[lane], pre = scr->pre[lane], lvl = scr->lvl[lane];
+      const double4* src = scr->src[lane];
       for (;;) {
         if (cursor < 32) {
           const int base = __shfl_sync(kFullMask, pre, cursor);
@@ -562,10 +594,16 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
           if (inc && !cont)
             tma_load_1d(ws.win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
                         (uint32_t)((run_end - pre) * sizeof(double4)), ws.bar0 + 8 * stage);
-          if (lane == 0) scr->n_inter += (unsigned long long)nstage * scr->nvalid;
+          if (lane == 0) {
+            scr->n_inter += (unsigned long long)nstage * scr->nvalid;
+            scr->cursor = cursor;
+          }
           return nstage;
         }
-        if (batch_next >= e_end) return 0;
+        if (batch_next >= e_end) {
+          if (lane == 0) scr->cursor = cursor;
+          return 0;
+        }
         // ---- a2: classify 32 elements, one per lane, against the tile's bounding sphere
         const int64_t batch0 = batch_next;
         const int64_t e = batch0 + lane;
@@ -603,6 +641,14 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
         }
         pre = warp_excl_scan(cnt, lane, &total);
         cursor = 0;
+        scr->cnt[lane] = cnt;
+        scr->pre[lane] = pre;
+        scr->lvl[lane] = lvl;
+        scr->src[lane] = src;
+        if (lane == 0) {
+          scr->batch_next = batch_next;
+          scr->total = total;
+        }
         unsigned amask = __ballot_sync(kFullMask, is_ana), xmask = __ballot_sync(kFullMask, is_mixed);
         if (amask) {
           bool all_ok[R];
@@ -646,6 +692,7 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     if (scr->n_inter) atomicAdd(p.counters, scr->n_inter);
     if (scr->n_ana) atomicAdd(p.counters + 1, scr->n_ana);
   }
+  clk.end(p.counters);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -700,6 +747,7 @@ __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __gri
   }
   Accum<double, kFewM, MODE> acc;
   acc.zero();
+  const double c375 = c_three_eighths;
   unsigned long long n_inter = 0, n_ana = 0;
 
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < p.n; e += (int64_t)gridDim.x * blockDim.x) {
@@ -730,7 +778,7 @@ __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __gri
     }
     if (same && lev[0] != 5) {  // the usual case: one rule for all points of the pass
       const int N = rule_npts(t, lev[0]);
-      for (int i = 0; i < N; ++i) interact<double, kFewM, MODE>(point(lev[0], i), px, py, pz, acc);
+      for (int i = 0; i < N; ++i) interact<double, kFewM, MODE>(point(lev[0], i), px, py, pz, acc, c375);
       n_inter += (unsigned long long)N * mj;
       continue;
     }
@@ -758,8 +806,8 @@ __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __gri
         const int N = rule_npts(t, lev[j]);
         for (int i = 0; i < N; ++i) {
           const double4 s = point(lev[j], i);
-          if constexpr (MODE == kModePhi) interact_one_phi(s.x, s.y, s.z, s.w, px[j], py[j], pz[j], acc.phi[j]);
-          else interact_one(s.x, s.y, s.z, s.w, px[j], py[j], pz[j], acc.phi[j], acc.ex[j], acc.ey[j], acc.ez[j]);
+          if constexpr (MODE == kModePhi) interact_one_phi(s.x, s.y, s.z, s.w, px[j], py[j], pz[j], acc.phi[j], c375);
+          else interact_one(s.x, s.y, s.z, s.w, px[j], py[j], pz[j], acc.phi[j], acc.ex[j], acc.ey[j], acc.ez[j], c375);
         }
         n_inter += N;
       }

@@ -21,18 +21,12 @@ struct GeomStatus {
   unsigned long long n_tri, n_rect;
 };
 
-// cenL[e] = (Q_cen.x, Q_cen.y, Q_cen.z, L); area[e] = A.
-__global__ void geometry_kernel(int64_t n, const uint8_t* __restrict__ type, const double* __restrict__ verts,
-                                double4* __restrict__ cenL, double* __restrict__ area, GeomStatus* status) {
-  const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (e >= n) return;
-  const double* v = verts + 9 * e;
+// Centroid, mean side L (in c.w) and area of one element from its nine stored coordinates; returns
+// 0 or the (negative) error code of include/bemcub.h.
+__device__ __forceinline__ int element_geometry(int t, const double* __restrict__ v, double4& c, double& A) {
   const double ax = v[0], ay = v[1], az = v[2];
   const double e1x = v[3] - ax, e1y = v[4] - ay, e1z = v[5] - az;
   const double e2x = v[6] - ax, e2y = v[7] - ay, e2z = v[8] - az;
-  const int t = type[e];
-  double4 c;
-  double A;
   int code = 0;
   if (t == 0) {
     // triangle A,B,C: area = |AB x AC|/2, centroid = (A+B+C)/3, L = (|AB|+|BC|+|CA|)/3
@@ -60,6 +54,18 @@ __global__ void geometry_kernel(int64_t n, const uint8_t* __restrict__ type, con
     c = make_double4(0, 0, 0, 0);
     code = -1;
   }
+  return code;
+}
+
+// cenL[e] = (Q_cen.x, Q_cen.y, Q_cen.z, L); area[e] = A.
+__global__ void geometry_kernel(int64_t n, const uint8_t* __restrict__ type, const double* __restrict__ verts,
+                                double4* __restrict__ cenL, double* __restrict__ area, GeomStatus* status) {
+  const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  const int t = type[e];
+  double4 c;
+  double A;
+  const int code = element_geometry(t, verts + 9 * e, c, A);
   cenL[e] = c;
   area[e] = A;
   if (code) atomicMin(&status->code, code);
@@ -116,7 +122,9 @@ __device__ __forceinline__ void store_point(float4* dst, double x, double y, dou
 }
 
 // One thread per (element, slot); slot < stride.  Slots beyond the element's own N are padding:
-// zero charge at the centroid.  sigma == nullptr means unit sigma (matrix assembly, L34).
+// zero charge at the position of the element's FIRST Gaussian point (a zero charge adds exactly
+// nothing wherever a real charge of the same place gives a finite term; the centroid would not do:
+// it is a field point of the matrix fill).  sigma == nullptr means unit sigma (matrix assembly, L34).
 // sigma_v != nullptr: the density varies linearly over the element (L275), sigma_v[e][3] = its
 // values at the three stored vertices, q_i = w_i A sigma(Q_i) with sigma(Q_i) from the rule's
 // reference coordinates (triangle: sum lambda_v sigma_v; rectangle: corner value + the two slopes).
@@ -124,19 +132,21 @@ template <typename T>
 __global__ void expand_kernel(int64_t n, int level, int stride, const uint8_t* __restrict__ type,
                               const double* __restrict__ verts, const double4* __restrict__ cenL,
                               const double* __restrict__ area, const double* __restrict__ sigma,
-                              const double* __restrict__ sigma_v, typename Point4<T>::type* __restrict__ out) {
+                              const double* __restrict__ sigma_v, double scale, typename Point4<T>::type* __restrict__ out) {
   const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (idx >= n * stride) return;
   const int64_t e = idx / stride;
   const int i = (int)(idx - e * stride);
   const int t = type[e];
   const double* v = verts + 9 * e;
-  const double q = (sigma ? sigma[e] : 1.0) * area[e];  // q = sigma A (L143); with sigma_v: q = A
+  // q = sigma A (L143); with sigma_v: q = A.  scale = 1 except for the matrix fill, which folds k in.
+  const double q = (sigma ? sigma[e] : 1.0) * area[e] * scale;
   const double* sv = sigma_v ? sigma_v + 3 * e : nullptr;
   const double4 c = cenL[e];
   double4 pt;
-  if (i < rule_npts_of(t, level) && rule_point(t, level, i, v, c, q, sv, pt)) store_point(out + idx, pt.x, pt.y, pt.z, pt.w);
-  else store_point(out + idx, c.x, c.y, c.z, 0.0);
+  const bool real = i < rule_npts_of(t, level);
+  rule_point(t, level, real ? i : 0, v, c, q, sv, pt);
+  store_point(out + idx, pt.x, pt.y, pt.z, real ? pt.w : 0.0);
 }
 
 // Step a6: sum the per-split partial results in split order and apply k = 1/(4 pi eps0) once
@@ -179,21 +189,37 @@ __global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride,
   }
 }
 
-// Roofline denominator: 16 independent DFMA chains per thread, nothing else in the loop.
-__global__ void dfma_peak_kernel(double* out, int iters, double a, double b) {
-  double x[16];
+// Roofline denominator (bemcub_fp64_issue_sweep): 16 (18 for the mix) independent chains per thread of
+// one FP64 instruction kind, the second operand in a uniform register so that an instruction reads at
+// most two vector registers - the form in which the pipe issues one warp instruction per two cycles
+// per scheduler.  MIX 0: DFMA, 1: DADD, 2: DMUL, 3: the 8 DFMA : 6 DMUL : 4 DADD mix of Eq. 4.1.
+// clk[0] = SM cycles, clk[1] = nanoseconds of the launch as thread 0 of CTA 0 saw them.
+template <int MIX>
+__global__ void fp64_issue_kernel(double* out, unsigned long long* clk, int iters, double a, double b) {
+  constexpr int C = (MIX == 3) ? 18 : 16;
+  double x[C];
 #pragma unroll
-  for (int k = 0; k < 16; ++k) x[k] = (double)(threadIdx.x + k) * 1e-3;
+  for (int k = 0; k < C; ++k) x[k] = 1.0 + (double)(threadIdx.x + k) * 1e-3;
+  KernelClock kc;
+  kc.begin();
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
 #pragma unroll
-      for (int k = 0; k < 16; ++k) x[k] = __fma_rn(x[k], a, b);
+      for (int k = 0; k < C; ++k) {
+        if (MIX == 0 || (MIX == 3 && k < 8)) x[k] = __fma_rn(x[k], a, b);
+        else if (MIX == 1 || (MIX == 3 && k >= 14)) x[k] = __dadd_rn(x[k], b);
+        else x[k] = __dmul_rn(x[k], a);
+      }
     }
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    clk[0] = (unsigned long long)(clock64() - kc.c0);
+    clk[1] = global_timer_ns() - kc.t0;
   }
   double s = 0.0;
 #pragma unroll
-  for (int k = 0; k < 16; ++k) s += x[k];
+  for (int k = 0; k < C; ++k) s += x[k];
   out[blockIdx.x * (int64_t)blockDim.x + threadIdx.x] = s;
 }
 

@@ -306,6 +306,42 @@ def random_elements(kind: int, n: int, seed: int):
     return np.full(n, kind, dtype=np.uint8), np.ascontiguousarray(verts)
 
 
+def mean_side_and_centre(etype: np.ndarray, verts: np.ndarray):
+    """(centre[n][3], mean side length[n]) of each element - used only to PLACE field points at a
+    wanted distance ratio; the libraries compute their own."""
+    cen = element_centroids(etype, verts)
+    a = np.linalg.norm(verts[:, 1] - verts[:, 0], axis=1)
+    b = np.linalg.norm(verts[:, 2] - verts[:, 1], axis=1)
+    c = np.linalg.norm(verts[:, 0] - verts[:, 2], axis=1)
+    tri = (a + b + c) / 3.0
+    rect = 0.5 * (a + c)                      # P0->P1 and P0->P3 are the two sides
+    return cen, np.where(etype == RECT, rect, tri)
+
+
+def aspect_ratio(etype: np.ndarray, verts: np.ndarray) -> np.ndarray:
+    """Triangle: longest side divided by the corresponding height; rectangle: longer side divided by
+    the shorter one."""
+    a = np.linalg.norm(verts[:, 1] - verts[:, 0], axis=1)
+    b = np.linalg.norm(verts[:, 2] - verts[:, 1], axis=1)
+    c = np.linalg.norm(verts[:, 0] - verts[:, 2], axis=1)
+    longest = np.maximum(np.maximum(a, b), c)
+    area = 0.5 * np.linalg.norm(np.cross(verts[:, 1] - verts[:, 0], verts[:, 2] - verts[:, 0]), axis=1)
+    tri = longest / (2.0 * area / longest)
+    rect = np.maximum(a, c) / np.minimum(a, c)
+    return np.where(etype == RECT, rect, tri)
+
+
+def random_pairs(kind: int, n: int, ratio, seed: int):
+    """The paper's accuracy protocol: n random elements (corners in the unit
+    cube), one field point each in a random direction from the element's centre at `ratio` (scalar or
+    [n]) mean side lengths.  Returns (etype, verts, pts)."""
+    etype, verts = random_elements(kind, n, seed)
+    cen, side = mean_side_and_centre(etype, verts)
+    dirs = isotropic_directions(_rng(seed + 7919), n)
+    pts = cen + dirs * (np.broadcast_to(np.asarray(ratio, dtype=np.float64), (n,)) * side)[:, None]
+    return etype, verts, np.ascontiguousarray(pts)
+
+
 def shard_range(total: int, rank: int, world: int) -> tuple[int, int]:
     """Contiguous [lo, hi) slice of `total` units owned by `rank` of `world` (sizes differ by
     at most one).  Used to shard field points / matrix rows across GPUs (no collective)."""

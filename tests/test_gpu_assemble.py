@@ -77,14 +77,17 @@ def test_mixed_mesh_rows_api_and_ragged_tiles():
 
 def test_cfg3_level5_full_size_sampled_rows():
     """Config 3 at full size (20480 x 20480, 3.36 GB) in the launch configuration bench.py uses;
-    the oracle recomputes 24 seeded rows."""
+    the oracle recomputes 72 rows: row 0, row n-1, the two rows at four 64-row tile boundaries, and
+    62 seeded ones."""
     c = synth.config3()
     n = len(c["etype"])
     assert n == 20480
     g = Gpu(c["etype"], c["verts"])
     pol = g.b.bemcub_default_policy(False)
     A = _assemble(g, pol, n)
-    rows = np.sort(np.random.default_rng(160603750).choice(n, 24, replace=False))
+    edges = np.array([0, 63, 64, 127, 128, 10239, 10240, n - 65, n - 64, n - 1])
+    rows = np.unique(np.concatenate([edges, np.random.default_rng(160603750).choice(n, 62, replace=False)]))
+    assert len(rows) >= 64
     got = A[g.torch.as_tensor(rows).cuda()].cpu().numpy()
     ref, code = oracle.assemble_rows(c["etype"], c["verts"], rows, oracle.default_policy(False))
     cub, ana = _check_rows(got, ref, code, "cfg3 sampled rows")

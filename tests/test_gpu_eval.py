@@ -171,6 +171,15 @@ def test_host_entry_points_match_device_path():
 
 
 # ------------------------------------------------------------------ a2 + a4: adaptive mode
+def _assert_parity_split(phi, E, ref, what):
+    """1e-12 on the field points whose oracle sum used no analytic pair, 1e-10 on the others."""
+    ana = ref["nana"] > 0
+    for sel, tol in ((~ana, TOL_F64), (ana, 1e-10)):
+        if sel.any():
+            sub = {k: v[sel] for k, v in ref.items()}
+            assert_parity(phi[sel], None if E is None else E[sel], sub, tol, f"{what} analytic={tol == 1e-10}")
+
+
 def _policy(b, want_field, allow_upgrade, mask=63, dr=None):
     p = b.bemcub_default_policy(want_field)
     if dr is not None:
@@ -230,26 +239,49 @@ def test_adaptive_policy_potential_limits_and_custom():
             pol = _policy(g.b, want_field, up, dr=dr)
             odr = oracle.default_policy(want_field) if dr is None else dr
             phi, E = g.eval(sigma, pts, -1, policy=pol)
-            ref = oracle.evaluate(etype, verts, sigma, pts, -1, dr=odr)
-            # points may fall inside the element cloud; the analytic branch handles them
-            err = parity_errors(phi, E, ref)
-            assert err["phi"] <= 1e-10 and err["E"] <= 1e-10, (err, up, want_field)
+            ref = oracle.evaluate(etype, verts, sigma, pts, -1, dr=odr, want_counts=True)
+            # points may fall inside the element cloud; the analytic branch handles them: 1e-10 where a
+            # point used it, 1e-12 on all the others
+            _assert_parity_split(phi, E, ref, (up, want_field))
     g.close()
 
 
 # ------------------------------------------------------------------ full-size config 4 (bench launch config)
 def test_cfg4_full_size_sampled():
-    """10^6 elements x 10^6 field points, adaptive, the exact call bench.py times; the oracle
-    recomputes 48 sampled field points one by one."""
+    """10^6 elements x 10^6 field points, adaptive, the exact call bench.py times; the oracle recomputes
+    1024 field points one by one: 768 drawn from a seed plus the first and the last 128 points of the
+    evaluation (Morton) order, i.e. the first tile and the ragged last one."""
     c = synth.config4()
-    assert len(c["etype"]) == 1_000_000 and len(c["pts"]) == 1_000_000
+    n, m = len(c["etype"]), len(c["pts"])
+    assert n == 1_000_000 and m == 1_000_000
     g = Gpu(c["etype"], c["verts"])
     pol = _policy(g.b, True, 1)
     phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
     assert np.all(np.isfinite(phi)) and np.all(np.isfinite(E))
-    idx = np.random.default_rng(160603749).choice(len(phi), 48, replace=False)
-    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx], -1, dr=oracle.default_policy(True))
+    ppp_upgrade = g.stats()["point_interactions"] / (float(n) * m)
+    # Morton order of the field points, recomputed here (30-bit keys on the bounding box, as DESIGN.md
+    # section 2 describes) only to pick the sample: points of the first and of the last tile
+    lo, hi = c["pts"].min(axis=0), c["pts"].max(axis=0)
+    q = np.minimum(((c["pts"] - lo) / (hi - lo) * 1024.0).astype(np.int64), 1023)
+    key = np.zeros(m, dtype=np.int64)
+    for bit in range(10):
+        for k in range(3):
+            key |= ((q[:, k] >> bit) & 1) << (3 * bit + k)
+    order = np.argsort(key, kind="stable")
+    idx = np.unique(np.concatenate([order[:128], order[-128:],
+                                    np.random.default_rng(160603749).choice(m, 768, replace=False)]))
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"][idx], -1, dr=oracle.default_policy(True),
+                          want_counts=True)
+    assert int(ref["nana"].sum()) == 0                                  # config 4 has no near-field pair (DR_min = 18)
     assert_parity(phi[idx], E[idx], ref, TOL_F64, "cfg4 full")
+    # the method's own work (per-pair policy) on the sample, and what the tiles execute beside it
+    ppp_own = ref["npi"].sum() / (float(n) * len(idx))
+    assert 7.2 < ppp_own < 7.6 and ppp_own <= ppp_upgrade < 1.05 * ppp_own, (ppp_own, ppp_upgrade)
+    # allow_upgrade = 0 on the sampled points: the device counter equals the oracle's count exactly
+    pol0 = _policy(g.b, True, 0)
+    phi0, E0 = g.eval(c["sigma"], c["pts"][idx], -1, policy=pol0)
+    assert g.stats()["point_interactions"] == int(ref["npi"].sum())
+    assert_parity(phi0, E0, ref, TOL_F64, "cfg4 sample, per-pair policy")
     g.close()
 
 
@@ -278,7 +310,7 @@ def test_potential_only_adaptive_with_analytic_branch(allow_upgrade, level):
     phi, _ = g.eval(sigma, cen, -1, policy=pol, want_E=False)
     ref = oracle.evaluate(c["etype"], c["verts"], sigma, cen, -1, dr=oracle.default_policy(False))
     err = parity_errors(phi, None, ref)
-    assert err["phi"] <= 1e-10, err          # analytic entries: BASELINE.json's 1e-10
+    assert err["phi"] <= 1e-10, err          # analytic entries: BASELINE.json's 1e-10 (every centroid has its self term)
     # with E as well: same potential; E itself is not compared - on the element's own surface the
     # normal field jumps by sigma/eps0 and its sign hangs on the rounding of h = n.(P - V0) ~ 1e-17
     phi2, E2 = g.eval(sigma, cen, -1, policy=pol)
@@ -319,4 +351,43 @@ def test_non_finite_field_points_do_not_spoil_their_tile():
     assert not np.any(np.isfinite(phi[bad]))
     ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], pts[good], -1, dr=oracle.default_policy(True))
     assert_parity(phi[good], E[good], ref, TOL_F64, "tile mates of non-finite points")
+    g.close()
+
+
+# ------------------------------------------------------------------ sharding by contiguous ranges
+@pytest.mark.parametrize("world", [2, 3, 8])
+def test_sub_ranges_reproduce_the_full_call(world):
+    """What every rank of a multi-GPU job does (bench.py --gpus N, multi.my_range): bemcub_eval on its
+    contiguous range of the field points, bemcub_assemble_rows on its range of the rows.  Fixed rule:
+    the concatenation is bit-identical to the single full call (a field point's sum does not depend on
+    its tile mates).  Adaptive: tiles differ, so the pieces agree with the oracle at the parity bar."""
+    c = synth.config4(scale=0.004, ntracks=30, npts_per_track=41)
+    m = len(c["pts"])
+    g = Gpu(c["etype"], c["verts"])
+    full_phi, full_E = g.eval(c["sigma"], c["pts"], 1)
+    pol = _policy(g.b, True, 1)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=oracle.default_policy(True), want_counts=True)
+    parts_phi, parts_E = [], []
+    for r in range(world):
+        lo, hi = synth.shard_range(m, r, world)
+        p1, e1 = g.eval(c["sigma"], c["pts"][lo:hi], 1)
+        parts_phi.append(p1)
+        parts_E.append(e1)
+        pa, ea = g.eval(c["sigma"], c["pts"][lo:hi], -1, policy=pol)
+        _assert_parity_split(pa, ea, {k: v[lo:hi] for k, v in ref.items()}, f"rank {r}/{world}")
+    assert np.array_equal(np.concatenate(parts_phi), full_phi) and np.array_equal(np.concatenate(parts_E), full_E)
+    # matrix rows
+    n = g.n
+    pol0 = _policy(g.b, False, 0)
+    torch = g.torch
+    A = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    g.b.bemcub_assemble(g.ctx.handle, pol0, A, n)
+    pieces = []
+    for r in range(world):
+        lo, hi = synth.shard_range(n, r, world)
+        rows = torch.empty((hi - lo, n), dtype=torch.float64, device="cuda")
+        g.b.bemcub_assemble_rows(g.ctx.handle, pol0, lo, hi - lo, rows, n)
+        pieces.append(rows)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.cat(pieces, dim=0), A)                      # per-pair policy: bit-identical
     g.close()

@@ -64,3 +64,29 @@ def test_adaptive_cfg4_small(allow_upgrade):
     with pytest.raises(Exception):
         run_linear(g, sv, c["pts"], -1, policy=bad)
     g.close()
+
+
+@pytest.mark.parametrize("m", [1, 4, 5, 64])
+def test_few_field_points_take_the_shuffle_path(m):
+    """m <= 64 dispatches bemcub_eval_linear to eval_few_kernel (elements across the lanes, points on the
+    fly with the linear density, per-pair rule): fixed rule and the distance-ratio choice."""
+    c = synth.config4(scale=0.003, ntracks=8, npts_per_track=9)
+    n = len(c["etype"])
+    rng = np.random.default_rng(60 + m)
+    sv = c["sigma"][:, None] * (1.0 + 0.3 * rng.uniform(-1.0, 1.0, (n, 3)))
+    pts = c["pts"][rng.choice(len(c["pts"]), m, replace=False)].copy()
+    g = Gpu(c["etype"], c["verts"])
+    for level in (1, 4):
+        phi, E = run_linear(g, sv, pts, level)
+        assert g.stats()["last_eval_launches"] == 2                       # eval_few_kernel + reduce_scale_kernel
+        err = parity_errors(phi, E, oracle.evaluate_linear(c["etype"], c["verts"], sv, pts, level))
+        assert err["phi"] <= TOL_F64 and err["E"] <= TOL_F64, (m, level, err)
+    pol = g.b.bemcub_default_policy(True)
+    pol.use_levels_mask = 0b011111
+    for up in (0, 1):                                                      # no effect on this path: per-pair rule
+        pol.allow_upgrade = up
+        phi, E = run_linear(g, sv, pts, -1, policy=pol)
+        ref = oracle.evaluate_linear(c["etype"], c["verts"], sv, pts, -1, dr=oracle.default_policy(True), levels_mask=0b011111)
+        err = parity_errors(phi, E, ref)
+        assert err["phi"] <= TOL_F64 and err["E"] <= TOL_F64, (m, up, err)
+    g.close()
