@@ -587,7 +587,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             cpu["value_single_thread"] = n * len(idx1) / (time.perf_counter() - t0)
 
     secondary = None
-    if rank == 0 and world == 1 and args.workload == "cfg4" and args.scale == 1.0 and not args.no_secondary and not args.gradient:
+    if rank == 0 and world == 1 and args.workload == "cfg4" and not args.no_secondary and not args.gradient:
         r.close()
         r = None
         del phi, E

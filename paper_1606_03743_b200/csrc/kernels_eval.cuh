@@ -35,10 +35,8 @@ constexpr int kWarpsPerCta = 12;  // 1 CTA per SM, 3 warps per scheduler, <= 168
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kBuf = 128;  // points per stage of a warp's window
 constexpr int kStages = 2;
-#ifndef BEMCUB_UNROLL_R4
-#define BEMCUB_UNROLL_R4 1
-#endif
-constexpr int kUnrollR4 = BEMCUB_UNROLL_R4;  // source points per trip of the R = 4 loops
+// source points per trip of the R = 4 loops (two per trip was measured on config 4 at full size: 0.3 % slower)
+constexpr int kUnrollR4 = 1;
 
 // Per-warp bookkeeping kept in shared memory (not registers): bounding sphere of the current tile
 // and the interaction tallies.
@@ -46,12 +44,6 @@ struct WarpScratch {
   double cx, cy, cz, rho, mag;
   unsigned long long n_inter, n_ana;
   int nvalid, pad;
-  // state of the adaptive kernel's current 32-element batch (lane l = element batch0 + l), parked here
-  // between two produce() calls so that the consume loop has the registers to itself
-  const double4* src[32];
-  int cnt[32], pre[32], lvl[32];
-  int64_t batch_next;
-  int total, cursor;
 };
 
 // shared memory of one CTA: [warps][stages][kBuf] points | [warps][stages] mbarriers | [warps] scratch
@@ -550,24 +542,14 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     Accum<double, R, MODE> tot;
     tot.zero();
 
-    // state of the current 32-element batch (lane l holds element batch0 + l) lives in the warp's
-    // scratch between two produce() calls: see WarpScratch
-    if (lane == 0) {
-      scr->batch_next = e_begin;
-      scr->total = 0;
-      scr->cursor = 32;
-    }
-    scr->cnt[lane] = 0;
-    scr->pre[lane] = 0;
-    scr->lvl[lane] = 0;
-    __syncwarp();
+    // state of the current 32-element batch: lane l holds element batch0 + l.  (Parking it in shared
+    // memory between two produce() calls was measured: no gain at scale 0.25, 3 % slower at full size.)
+    int64_t batch_next = e_begin;
+    int cnt = 0, pre = 0, total = 0, lvl = 0, cursor = 32;
+    const double4* src = nullptr;
 
     // Fills `stage` with the next round of whole elements; returns the number of points (0 = done).
     auto produce = [&](int stage) -> int {
-      int64_t batch_next = scr->batch_next;
-      int cursor = scr->cursor, total = scr->total;
-      int cnt = scr->cnt[lane], pre = scr->pre[lane], lvl = scr->lvl[lane];
-      const double4* src = scr->src[lane];
       for (;;) {
         if (cursor < 32) {
           const int base = __shfl_sync(kFullMask, pre, cursor);
@@ -594,16 +576,10 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
           if (inc && !cont)
             tma_load_1d(ws.win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
                         (uint32_t)((run_end - pre) * sizeof(double4)), ws.bar0 + 8 * stage);
-          if (lane == 0) {
-            scr->n_inter += (unsigned long long)nstage * scr->nvalid;
-            scr->cursor = cursor;
-          }
+          if (lane == 0) scr->n_inter += (unsigned long long)nstage * scr->nvalid;
           return nstage;
         }
-        if (batch_next >= e_end) {
-          if (lane == 0) scr->cursor = cursor;
-          return 0;
-        }
+        if (batch_next >= e_end) return 0;
         // ---- a2: classify 32 elements, one per lane, against the tile's bounding sphere
         const int64_t batch0 = batch_next;
         const int64_t e = batch0 + lane;
@@ -641,14 +617,6 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
         }
         pre = warp_excl_scan(cnt, lane, &total);
         cursor = 0;
-        scr->cnt[lane] = cnt;
-        scr->pre[lane] = pre;
-        scr->lvl[lane] = lvl;
-        scr->src[lane] = src;
-        if (lane == 0) {
-          scr->batch_next = batch_next;
-          scr->total = total;
-        }
         unsigned amask = __ballot_sync(kFullMask, is_ana), xmask = __ballot_sync(kFullMask, is_mixed);
         if (amask) {
           bool all_ok[R];
