@@ -23,7 +23,9 @@
  *   - All work is enqueued on the CUDA stream given to bemcub_create (NULL = legacy default
  *     stream).  bemcub_eval / bemcub_assemble* are asynchronous: results are valid once the caller
  *     has synchronised that stream.  bemcub_set_elements, bemcub_solve, the *_host calls,
- *     bemcub_fp64_peak and bemcub_inner_loop_rate synchronise internally.  (A call that has to grow ctx-owned scratch calls cudaMalloc.)
+ *     bemcub_fp64_peak / bemcub_fp64_issue_sweep, bemcub_inner_loop_rate and bemcub_get_stats synchronise
+ *     internally.  A call that has to grow ctx-owned scratch calls cudaFree / cudaMalloc (which
+ *     synchronise the device); repeated calls of the same shapes do not.
  *   - Every function returns BEMCUB_OK (0) or a negative error code; nothing throws or longjmps
  *     across the ABI.  There is no CPU fallback: without a usable CUDA device bemcub_create fails.
  *   - SI units: lengths m, sigma C/m^2, Phi V, E V/m.  eps0 = 8.8541878128e-12 F/m (CODATA 2018;
@@ -134,9 +136,10 @@ int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const d
  *   sigma[n]; rule_id = BEMCUB_RULE_L0..L4 (fixed rule for every pair; no near-field switching: a
  *   field point that coincides with a Gaussian point gives IEEE inf/nan) or BEMCUB_RULE_ADAPTIVE
  *   (policy must be non-NULL; HOST pointer); field_pts[m][3]; out_phi[m]; out_E[m][3] or NULL.
- *   precision = BEMCUB_F64, or BEMCUB_F32: points, field points and the interaction arithmetic
- *   are FP32, sums of at most 128 terms are FP32 and those block sums are accumulated in FP64
- *   (the analytic branch stays FP64); buffers keep their double type.
+ *   precision = BEMCUB_F64, or BEMCUB_F32 (fixed rules only: BEMCUB_RULE_ADAPTIVE with BEMCUB_F32 returns
+ *   INVALID_ARG - the distance-ratio limits are accuracy limits of FP64 arithmetic): points, field
+ *   points and the interaction arithmetic are FP32, sums of at most 128 terms are FP32 and those
+ *   block sums are accumulated in FP64; buffers keep their double type.
  * sigma == NULL: evaluate with the sigma of the previous call on this ctx that passed one (the ctx
  *   keeps a copy; INVALID_ARG if there is none).  Rule levels already expanded for that sigma are
  *   reused, so the preprocessing pass a1 is skipped - what a particle tracker wants, which asks
@@ -205,8 +208,9 @@ int bemcub_assemble_rows(bemcub_ctx* ctx, const bemcub_policy* host_policy, int6
  * one potential-only adaptive evaluation at the n element centroids under `host_policy` (use
  * bemcub_default_policy(.., 0): the potential limits).  sigma[n]: initial guess on entry (zeros
  * are fine), solution on exit.  Stops when |rhs - A sigma|_2 <= rel_tol |rhs|_2 or after
- * max_matvecs mat-vecs (then BEMCUB_ERR_NOT_CONVERGED, with the best iterate in sigma).
- * host_matvecs / host_rel_residual (HOST, may be NULL): mat-vecs used, final true relative residual.
+ * max_matvecs mat-vecs - never more: the last one of the budget is kept for the residual of the
+ * iterate returned (then BEMCUB_ERR_NOT_CONVERGED, with that iterate in sigma).
+ * host_matvecs / host_rel_residual (HOST, may be NULL): mat-vecs used, true relative residual of sigma.
  * Synchronous.  The policy's allow_upgrade changes the operator only at the rules' truncation level. */
 int bemcub_solve(bemcub_ctx* ctx, const bemcub_policy* host_policy, const double* rhs_potential, double* sigma,
                  double rel_tol, int max_matvecs, int* host_matvecs, double* host_rel_residual);
@@ -260,7 +264,8 @@ int bemcub_inner_loop_rate(bemcub_ctx* ctx, double seconds, double* host_interac
 int bemcub_set_timing(bemcub_ctx* ctx, int enable);
 int bemcub_get_timing(bemcub_ctx* ctx, double* host_ms_total, double* host_ms_kernel);
 
-int bemcub_get_stats(bemcub_ctx* ctx, bemcub_stats* host_stats);  /* synchronises the stream */
+/* HOST struct.  Synchronises the ctx stream when device counters of the last call are pending. */
+int bemcub_get_stats(bemcub_ctx* ctx, bemcub_stats* host_stats);
 int bemcub_reset_stats(bemcub_ctx* ctx);
 
 const char* bemcub_strerror(int code);

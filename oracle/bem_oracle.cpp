@@ -63,6 +63,15 @@ template <> inline long double tatan(long double x) { return atanl(x); }
 template <> inline double tatan(double x) { return atan(x); }
 template <class T> inline T tabs(T x) { return x < 0 ? -x : x; }
 
+inline int threads_for(int nthreads) {
+#ifdef _OPENMP
+    return nthreads > 0 ? nthreads : omp_get_max_threads();
+#else
+    (void)nthreads;
+    return 1;
+#endif
+}
+
 template <class T> struct V3 { T x, y, z; };
 template <class T> inline V3<T> sub(const V3<T>& a, const V3<T>& b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
 template <class T> inline T dot(const V3<T>& a, const V3<T>& b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
@@ -402,11 +411,10 @@ int eval_impl(int64_t n, const uint8_t* etype, const double* verts, const double
         if (rc) return rc;
     }
     const T k = (T)coulomb_k();
-#ifdef _OPENMP
-    if (nthreads > 0) omp_set_num_threads(nthreads);
-#endif
     // steps 3-5, one field point after the other: elements in index order, the rule's points in table order
-#pragma omp parallel for schedule(dynamic, 1)
+    // (nthreads > 0 limits this call only; it does not change the process-wide OpenMP setting)
+    const int nt = threads_for(nthreads);
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nt)
     for (int64_t j = 0; j < m; ++j) {
         const V3<T> P{(T)pts[3 * j], (T)pts[3 * j + 1], (T)pts[3 * j + 2]};
         T aphi = 0, aex = 0, aey = 0, aez = 0, asphi = 0, ase = 0;
@@ -815,10 +823,8 @@ int orc_assemble_rows(int64_t n, const uint8_t* etype, const double* verts, cons
         if (rc) return rc;
     }
     const T k = coulomb_k();
-#ifdef _OPENMP
-    if (nthreads > 0) omp_set_num_threads(nthreads);
-#endif
-#pragma omp parallel for schedule(dynamic, 1)
+    const int nt = threads_for(nthreads);
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nt)
     for (int64_t r = 0; r < nrows; ++r) {
         const int64_t i = rows[r];
         const V3<T> P = G[i].cen;

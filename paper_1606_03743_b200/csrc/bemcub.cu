@@ -252,8 +252,7 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) 
 
 template <typename T, int R, int MODE = kModePhiE>
 int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
-  const size_t smem = eval_smem_bytes<T>();
-  CUDA_TRY(cudaFuncSetAttribute(eval_fixed_kernel<T, R, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const size_t smem = eval_smem_bytes<T>();  // opted in once per device by configure_kernels()
   eval_fixed_kernel<T, R, MODE><<<sp.grid, kThreads, smem, c->stream>>>(fp);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
@@ -263,10 +262,44 @@ int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
 template <int R, int MODE = kModePhiE>
 int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<double>();
-  CUDA_TRY(cudaFuncSetAttribute(eval_adaptive_kernel<R, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   eval_adaptive_kernel<R, MODE><<<sp.grid, kThreads, smem, c->stream>>>(ap);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
+
+// Opt-in to more than 48 KB of dynamic shared memory for every kernel instantiation that needs it,
+// once per ctx (the attribute is per device), so that the asynchronous calls launch and nothing else.
+template <typename K>
+int opt_in_smem(K kernel, size_t bytes) {
+  CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  return BEMCUB_OK;
+}
+template <typename T, int MODE>
+int configure_fixed() {
+  int rc;
+  const size_t b = eval_smem_bytes<T>();
+  if ((rc = opt_in_smem(eval_fixed_kernel<T, 1, MODE>, b)) || (rc = opt_in_smem(eval_fixed_kernel<T, 2, MODE>, b))) return rc;
+  if constexpr (MODE != kModeGrad) rc = opt_in_smem(eval_fixed_kernel<T, 4, MODE>, b);
+  return rc;
+}
+template <int MODE>
+int configure_adaptive() {
+  int rc;
+  const size_t b = eval_smem_bytes<double>();
+  if ((rc = opt_in_smem(eval_adaptive_kernel<1, MODE>, b)) || (rc = opt_in_smem(eval_adaptive_kernel<2, MODE>, b))) return rc;
+  if constexpr (MODE != kModeGrad) rc = opt_in_smem(eval_adaptive_kernel<4, MODE>, b);
+  return rc;
+}
+int configure_kernels() {
+  int rc;
+  if ((rc = configure_fixed<double, kModePhiE>()) || (rc = configure_fixed<double, kModePhi>()) ||
+      (rc = configure_fixed<double, kModeGrad>()) || (rc = configure_fixed<float, kModePhiE>()) ||
+      (rc = configure_fixed<float, kModePhi>()) || (rc = configure_adaptive<kModePhiE>()) ||
+      (rc = configure_adaptive<kModePhi>()) || (rc = configure_adaptive<kModeGrad>()) ||
+      (rc = opt_in_smem(assemble_kernel, assemble_smem_bytes())) ||
+      (rc = opt_in_smem(inner_loop_kernel<4>, eval_smem_bytes<double>())))
+    return rc;
   return BEMCUB_OK;
 }
 
@@ -412,6 +445,7 @@ int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream) {
   }
   c->num_sms = prop.multiProcessorCount;
   int rc = upload_tables();
+  if (rc == BEMCUB_OK) rc = configure_kernels();
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_status, sizeof(GeomStatus)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
   if (rc != BEMCUB_OK) {
@@ -817,7 +851,6 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   ap.counters = c->d_counters;
   ap.queue = c->d_counters + 2;
   CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
-  CUDA_TRY(cudaFuncSetAttribute(assemble_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)assemble_smem_bytes()));
   // items = (64-row tile) x (split of the columns, a multiple of 32): about 32 per warp
   const int64_t warps = (int64_t)c->num_sms * kAsmWarps;
   ap.nrowtiles = (nrows + kAsmRows - 1) / kAsmRows;
@@ -959,7 +992,6 @@ int bemcub_inner_loop_rate(bemcub_ctx* c, double seconds, double* host_interacti
       npts_field, (double*)c->host_stage[3].ptr, kStages * kBuf, (double4*)c->host_stage[4].ptr);
   c->stats.kernel_launches += 1;
   const size_t smem = eval_smem_bytes<double>();
-  CUDA_TRY(cudaFuncSetAttribute(inner_loop_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   cudaEvent_t e0, e1;
   CUDA_TRY(cudaEventCreate(&e0));
   CUDA_TRY(cudaEventCreate(&e1));

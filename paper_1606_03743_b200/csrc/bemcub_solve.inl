@@ -11,7 +11,7 @@ struct SolveWork {
   double* basis;  // [restart + 1][n]
   double* w;      // [n]
   double* z;      // [n]
-  double* coef;   // [2 * (restart + 2)] dot products / combination coefficients
+  double* coef;   // [3 * (restart + 2)]: first and second Gram-Schmidt pass, then |w|^2; also y of the update
 };
 
 inline unsigned blocks_for(int64_t n) { return (unsigned)((n + 255) / 256); }
@@ -21,14 +21,18 @@ int solve_matvec(bemcub_ctx* c, const bemcub_policy* pol, const SolveWork& k, co
   return eval_common(c, x, BEMCUB_RULE_ADAPTIVE, pol, c->n, k.cen, out, nullptr, nullptr, BEMCUB_F64, !first);
 }
 
-int dots_to_host(bemcub_ctx* c, const SolveWork& k, int nvec, const double* basis, const double* w, double* dev_out, double* host_out) {
+// dev_out[v] = V[v] . w for v < nvec (deterministic tree reduction, one block per vector); stays on the device
+int dots_dev(bemcub_ctx* c, int nvec, const double* basis, const double* w, double* dev_out) {
   const int64_t n = c->n;
   vec_dots_kernel<<<nvec, 1024, 0, c->stream>>>(n, basis, n, w, dev_out);
   c->stats.kernel_launches += 1;
   CUDA_TRY(cudaGetLastError());
-  CUDA_TRY(cudaMemcpyAsync(host_out, dev_out, sizeof(double) * nvec, cudaMemcpyDeviceToHost, c->stream));
+  return BEMCUB_OK;
+}
+
+int to_host(bemcub_ctx* c, const double* dev, int count, double* host) {
+  CUDA_TRY(cudaMemcpyAsync(host, dev, sizeof(double) * count, cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(cudaStreamSynchronize(c->stream));
-  (void)k;
   return BEMCUB_OK;
 }
 
@@ -51,7 +55,7 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
   const int M = kGmresRestart;
   if ((rc = ensure(c->solve_buf[0], (size_t)n * 24)) || (rc = ensure(c->solve_buf[1], (size_t)n * 8)) ||
       (rc = ensure(c->solve_buf[2], (size_t)(M + 1) * n * 8)) || (rc = ensure(c->solve_buf[3], (size_t)n * 8)) ||
-      (rc = ensure(c->solve_buf[4], (size_t)n * 8)) || (rc = ensure(c->solve_buf[5], (size_t)2 * (M + 2) * 8)))
+      (rc = ensure(c->solve_buf[4], (size_t)n * 8)) || (rc = ensure(c->solve_buf[5], (size_t)3 * (M + 2) * 8)))
     return rc;
   SolveWork k;
   k.cen = (double*)c->solve_buf[0].ptr;
@@ -67,7 +71,7 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
   CUDA_TRY(cudaGetLastError());
 
   double hb = 0.0;
-  if ((rc = dots_to_host(c, k, 1, rhs, rhs, k.coef, &hb))) return rc;
+  if ((rc = dots_dev(c, 1, rhs, rhs, k.coef)) || (rc = to_host(c, k.coef, 1, &hb))) return rc;
   const double bnorm = std::sqrt(hb);
   if (bnorm == 0.0) {  // zero potential everywhere: zero charge
     CUDA_TRY(cudaMemsetAsync(sigma, 0, (size_t)n * 8, c->stream));
@@ -78,9 +82,12 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
   bool first = true;
   double relres = 1.0;
   bool converged = false;
-  double H[kGmresRestart + 1][kGmresRestart], cs[kGmresRestart], sn[kGmresRestart], gv[kGmresRestart + 1], hcol[kGmresRestart + 2],
-      hcol2[kGmresRestart + 2];
+  double H[kGmresRestart + 1][kGmresRestart], cs[kGmresRestart], sn[kGmresRestart], gv[kGmresRestart + 1];
+  double hbuf[3 * (kGmresRestart + 2)];
+  const int stride = M + 2;  // coef = [pass 1 | pass 2 | norm]
 
+  // Every cycle starts with the true residual of the current iterate, so the residual reported at the
+  // end is always that of the sigma returned; the Arnoldi loop leaves one mat-vec of the budget for it.
   while (matvecs < max_matvecs) {
     // true residual r = b - A x, V_0 = r / |r|
     if ((rc = solve_matvec(c, host_policy, k, sigma, k.w, first))) return rc;
@@ -88,7 +95,8 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
     ++matvecs;
     vec_sub_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, rhs, k.w, k.w);
     double rr = 0.0;
-    if ((rc = dots_to_host(c, k, 1, k.w, k.w, k.coef, &rr))) return rc;
+    if ((rc = dots_dev(c, 1, k.w, k.w, k.coef)) || (rc = to_host(c, k.coef, 1, &rr))) return rc;
+    c->stats.kernel_launches += 1;
     const double beta = std::sqrt(rr);
     relres = beta / bnorm;
     if (relres <= rel_tol) {
@@ -99,21 +107,23 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
     vec_scale_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, 1.0 / beta, k.w, nullptr, k.basis);
     gv[0] = beta;
     int j = 0;
-    for (; j < M && matvecs < max_matvecs; ++j) {
+    for (; j < M && matvecs < max_matvecs - 1; ++j) {
       // w = A M^-1 V_j
       vec_scale_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, 1.0, k.basis + (int64_t)j * n, k.diag, k.z);
       if ((rc = solve_matvec(c, host_policy, k, k.z, k.w, false))) return rc;
       ++matvecs;
-      // classical Gram-Schmidt, twice
-      if ((rc = dots_to_host(c, k, j + 1, k.basis, k.w, k.coef, hcol))) return rc;
+      // classical Gram-Schmidt, twice; coefficients, norm and the new basis vector all stay on the
+      // device - ONE copy to the host per step, for the Hessenberg column and the stopping test
+      if ((rc = dots_dev(c, j + 1, k.basis, k.w, k.coef))) return rc;
       vec_combine_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, j + 1, k.basis, n, k.coef, -1.0, k.w);
-      if ((rc = dots_to_host(c, k, j + 1, k.basis, k.w, k.coef, hcol2))) return rc;
-      vec_combine_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, j + 1, k.basis, n, k.coef, -1.0, k.w);
-      double ww = 0.0;
-      if ((rc = dots_to_host(c, k, 1, k.w, k.w, k.coef, &ww))) return rc;
-      c->stats.kernel_launches += 3;
-      const double hnext = std::sqrt(ww);
-      for (int i = 0; i <= j; ++i) H[i][j] = hcol[i] + hcol2[i];
+      if ((rc = dots_dev(c, j + 1, k.basis, k.w, k.coef + stride))) return rc;
+      vec_combine_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, j + 1, k.basis, n, k.coef + stride, -1.0, k.w);
+      if ((rc = dots_dev(c, 1, k.w, k.w, k.coef + 2 * stride))) return rc;
+      vec_normalise_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, k.w, k.coef + 2 * stride, k.basis + (int64_t)(j + 1) * n);
+      c->stats.kernel_launches += 4;
+      if ((rc = to_host(c, k.coef, 2 * stride + 1, hbuf))) return rc;
+      const double hnext = std::sqrt(hbuf[2 * stride]);
+      for (int i = 0; i <= j; ++i) H[i][j] = hbuf[i] + hbuf[stride + i];
       // Givens rotations of the new Hessenberg column
       for (int i = 0; i < j; ++i) {
         const double t = cs[i] * H[i][j] + sn[i] * H[i + 1][j];
@@ -127,8 +137,6 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
       gv[j + 1] = -sn[j] * gv[j];
       gv[j] = cs[j] * gv[j];
       const double est = std::fabs(gv[j + 1]) / bnorm;
-      if (hnext > 0.0)
-        vec_scale_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, 1.0 / hnext, k.w, nullptr, k.basis + (int64_t)(j + 1) * n);
       if (est <= rel_tol || hnext == 0.0) {
         ++j;
         break;
@@ -150,15 +158,6 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
       CUDA_TRY(cudaStreamSynchronize(c->stream));  // y lives on the host stack
     }
     CUDA_TRY(cudaGetLastError());
-  }
-  if (!converged) {  // report the true residual of the iterate we return
-    if ((rc = solve_matvec(c, host_policy, k, sigma, k.w, first))) return rc;
-    ++matvecs;
-    vec_sub_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, rhs, k.w, k.w);
-    double rr = 0.0;
-    if ((rc = dots_to_host(c, k, 1, k.w, k.w, k.coef, &rr))) return rc;
-    relres = std::sqrt(rr) / bnorm;
-    converged = relres <= rel_tol;
   }
   CUDA_TRY(cudaStreamSynchronize(c->stream));
   if (host_matvecs) *host_matvecs = matvecs;

@@ -226,32 +226,16 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
       auto fill = [&](int stage) -> int {
         for (;;) {
           if (cursor >= 32) return 0;
-          const int base = __shfl_sync(kFullMask, pre, cursor);
-          const bool after = lane >= cursor;
-          const unsigned nofit = __ballot_sync(kFullMask, after && (pre + cnt - base > kBuf));
-          const int next = nofit ? (__ffs(nofit) - 1) : 32;
-          const int pre_next = __shfl_sync(kFullMask, pre, next & 31);
-          const int endp = (next < 32) ? pre_next : total;
-          const int nstage = endp - base;
-          const bool inc = after && lane < next && cnt > 0;
-          const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
-          const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
-          const bool cont = inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == p.stride[lvl];
-          const unsigned incmask = __ballot_sync(kFullMask, inc);
-          const unsigned heads = __ballot_sync(kFullMask, inc && !cont);
-          const unsigned higher = heads & ~((2u << lane) - 1u);
-          const int h2 = higher ? (__ffs(higher) - 1) : 32;
-          const int pre_h2 = __shfl_sync(kFullMask, pre, h2 & 31);
-          const int run_end = (h2 < 32) ? pre_h2 : endp;
-          cursor = next;
-          if (nstage == 0) continue;
-          if (inc) sm.seg[stage][__popc(incmask & lt_mask)] = (uint32_t)lane | ((uint32_t)cnt << 8) | ((uint32_t)(pre - base) << 16);
-          if (lane == 0) mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
+          const StagePlan sp = plan_stage(cursor, lane, cnt, pre, total, lvl, p.stride);
+          cursor = sp.next;
+          if (sp.nstage == 0) continue;
+          if (sp.inc) sm.seg[stage][__popc(sp.incmask & lt_mask)] = (uint32_t)lane | ((uint32_t)cnt << 8) | ((uint32_t)(pre - sp.base) << 16);
+          if (lane == 0) mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(sp.nstage * sizeof(double4)));
           __syncwarp();
-          if (inc && !cont)
-            tma_load_1d(win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
-                        (uint32_t)((run_end - pre) * sizeof(double4)), bar0 + 8 * stage);
-          return __popc(incmask);
+          if (sp.head)
+            tma_load_1d(win0 + (uint32_t)((stage * kBuf + (pre - sp.base)) * sizeof(double4)), src,
+                        (uint32_t)((sp.run_end - pre) * sizeof(double4)), bar0 + 8 * stage);
+          return __popc(sp.incmask);
         }
       };
       // output group (8 consecutive columns) being collected in sm.tile, and which of its columns

@@ -263,6 +263,45 @@ __device__ __forceinline__ WarpSmem<P4> warp_smem(unsigned char* smem_raw, int w
   return w;
 }
 
+// Packing of a classified 32-element batch into a warp's window (adaptive evaluation and matrix fill
+// share it).  Lane l holds element l of the batch: cnt points (0 = not streamed) of level lvl, pre =
+// exclusive prefix of cnt, total = its sum.  Starting at lane `cursor`, the next stage takes whole
+// elements while they fit into kBuf points; consecutive elements of one level whose records are
+// adjacent in memory (cnt == stride of the level) are merged into one bulk copy, issued by the run's
+// first lane.
+struct StagePlan {
+  int base;      // pre of the first lane of the stage
+  int next;      // first lane that does not fit (32 = batch exhausted): the next cursor
+  int nstage;    // points of the stage
+  int run_end;   // this lane heads a copy run: pre of the lane after the run
+  bool inc;      // this lane's element is in the stage
+  bool head;     // ... and starts a copy run
+  unsigned incmask;
+};
+__device__ __forceinline__ StagePlan plan_stage(int cursor, int lane, int cnt, int pre, int total, int lvl, const int (&stride)[5]) {
+  StagePlan s;
+  s.base = __shfl_sync(kFullMask, pre, cursor);
+  const bool after = lane >= cursor;
+  const unsigned nofit = __ballot_sync(kFullMask, after && (pre + cnt - s.base > kBuf));
+  s.next = nofit ? (__ffs(nofit) - 1) : 32;
+  const int pre_next = __shfl_sync(kFullMask, pre, s.next & 31);
+  const int endp = (s.next < 32) ? pre_next : total;
+  s.nstage = endp - s.base;
+  s.inc = after && lane < s.next && cnt > 0;
+  const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
+  const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
+  // a lane continues its predecessor's copy if that one ends exactly where this one starts
+  const bool cont = s.inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == stride[lvl < 0 ? 0 : lvl];
+  s.incmask = __ballot_sync(kFullMask, s.inc);
+  s.head = s.inc && !cont;
+  const unsigned heads = __ballot_sync(kFullMask, s.head);
+  const unsigned higher = heads & ~((2u << lane) - 1u);
+  const int h2 = higher ? (__ffs(higher) - 1) : 32;
+  const int pre_h2 = __shfl_sync(kFullMask, pre, h2 & 31);
+  s.run_end = (h2 < 32) ? pre_h2 : endp;
+  return s;
+}
+
 struct FixedParams {
   const void* pts;          // Point4<T>[npts], one rule level
   int64_t npts;             // n * stride
@@ -552,30 +591,15 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     auto produce = [&](int stage) -> int {
       for (;;) {
         if (cursor < 32) {
-          const int base = __shfl_sync(kFullMask, pre, cursor);
-          const bool after = lane >= cursor;
-          const unsigned nofit = __ballot_sync(kFullMask, after && (pre + cnt - base > kBuf));
-          const int next = nofit ? (__ffs(nofit) - 1) : 32;
-          const int pre_next = __shfl_sync(kFullMask, pre, next & 31);
-          const int endp = (next < 32) ? pre_next : total;
-          const int nstage = endp - base;
-          const bool inc = after && lane < next && cnt > 0;
-          const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
-          const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
-          // a lane continues its predecessor's copy if that one ends exactly where this one starts
-          const bool cont = inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == p.stride[lvl];
-          const unsigned heads = __ballot_sync(kFullMask, inc && !cont);
-          const unsigned higher = heads & ~((2u << lane) - 1u);
-          const int h2 = higher ? (__ffs(higher) - 1) : 32;
-          const int pre_h2 = __shfl_sync(kFullMask, pre, h2 & 31);
-          const int run_end = (h2 < 32) ? pre_h2 : endp;
-          cursor = next;
+          const StagePlan sp = plan_stage(cursor, lane, cnt, pre, total, lvl, p.stride);
+          const int nstage = sp.nstage;
+          cursor = sp.next;
           if (nstage == 0) continue;
           if (lane == 0) mbar_arrive_expect_tx(ws.bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
           __syncwarp();
-          if (inc && !cont)
-            tma_load_1d(ws.win0 + (uint32_t)((stage * kBuf + (pre - base)) * sizeof(double4)), src,
-                        (uint32_t)((run_end - pre) * sizeof(double4)), ws.bar0 + 8 * stage);
+          if (sp.head)
+            tma_load_1d(ws.win0 + (uint32_t)((stage * kBuf + (pre - sp.base)) * sizeof(double4)), src,
+                        (uint32_t)((sp.run_end - pre) * sizeof(double4)), ws.bar0 + 8 * stage);
           if (lane == 0) scr->n_inter += (unsigned long long)nstage * scr->nvalid;
           return nstage;
         }
@@ -669,7 +693,9 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
 // kFewM field points of the pass are shared by all lanes, every (element, point) pair gets its
 // rule from its own distance ratio (the per-pair policy of L159, exactly), and the partial sums
 // of the lanes are combined with warp shuffles, then across the warps of the CTA; a6 adds the CTAs.
-// The pass is bound by reading every expanded point once (HBM), not by the FP64 pipe.
+// Such a call is latency-bound, not bandwidth-bound: for one field point it reads 121 bytes per element
+// (vertices, centroid, L, area, sigma) - 121 MB for 10^6 elements in 0.10 ms = 1.2 TB/s, 18 % of the HBM
+// copy rate - in a single grid-stride pass with one dependent chain per thread, then two tiny launches.
 constexpr int kFewM = 4;        // field points per pass (grid.y)
 constexpr int kFewMaxM = 64;    // above this the tiled kernels win (10^6 elements: 1.4 ms at m = 64 either way; 2.9 ms tiled with a new sigma)
 constexpr int kFewWarps = 8;

@@ -63,10 +63,18 @@ __global__ void vec_scale_kernel(int64_t n, double alpha, const double* __restri
   dst[i] = d ? alpha * a[i] / d[i] : alpha * a[i];
 }
 
-// dst = a - b
-__global__ void vec_sub_kernel(int64_t n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ dst) {
+// dst = a - b   (dst may be b: no __restrict__ on those two)
+__global__ void vec_sub_kernel(int64_t n, const double* __restrict__ a, const double* b, double* dst) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i < n) dst[i] = a[i] - b[i];
+}
+
+// dst = a / sqrt(*norm2)   (normalisation by a squared norm that is still on the device; 0 -> copy)
+__global__ void vec_normalise_kernel(int64_t n, const double* __restrict__ a, const double* __restrict__ norm2, double* __restrict__ dst) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double s = *norm2;
+  dst[i] = s > 0.0 ? a[i] / sqrt(s) : a[i];
 }
 
 // x += u / d

@@ -93,3 +93,74 @@ def test_two_rank_gloo_field_point_and_row_sharding():
     assert np.array_equal(full[:, 0], ref["phi"]) and np.array_equal(full[:, 1:], ref["E"])
     rows, _ = oracle.assemble_rows(c["etype"], c["verts"], np.arange(len(c["etype"])), oracle.default_policy(False))
     assert np.array_equal(mat, rows)
+
+
+# ------------------------------------------------------------------ the product under torch.distributed
+def _gpu_worker(rank: int, ws: int, port: int, q):
+    """One rank of a 2-process job sharing cuda:0: its own bemcub ctx, its contiguous range of the field
+    points (bemcub_eval) and of the matrix rows (bemcub_assemble_rows), results gathered on rank 0."""
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+
+    from paper_1606_03743_b200 import bemcub as b
+    from paper_1606_03743_b200 import multi, synth
+
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=ws)
+    try:
+        c = synth.config4(scale=0.002, ntracks=23, npts_per_track=31)     # 713 field points: ragged split
+        n, m = len(c["etype"]), len(c["pts"])
+        with b.Context(0) as ctx:
+            h = ctx.handle
+            d = lambda a: torch.as_tensor(np.ascontiguousarray(a)).cuda()
+            b.bemcub_set_elements(h, n, d(c["etype"]), d(c["verts"]))
+            lo, hi = multi.my_range(m)
+            phi = torch.empty(hi - lo, dtype=torch.float64, device="cuda")
+            E = torch.empty((hi - lo, 3), dtype=torch.float64, device="cuda")
+            pol = b.bemcub_default_policy(True)
+            b.bemcub_eval(h, d(c["sigma"]), b.RULE_ADAPTIVE, pol, hi - lo, d(c["pts"][lo:hi]), phi, E, b.F64)
+            torch.cuda.synchronize()
+            full = multi.gather_rows(torch.cat([phi[:, None], E], dim=1).cpu(), m)
+            rlo, rhi = multi.my_range(n)
+            rows = torch.empty((rhi - rlo, n), dtype=torch.float64, device="cuda")
+            b.bemcub_assemble_rows(h, b.bemcub_default_policy(False), rlo, rhi - rlo, rows, n)
+            torch.cuda.synchronize()
+            mat = multi.gather_rows(rows.cpu(), n)
+            launches = multi.sum_over_ranks(float(b.bemcub_get_stats(h)["kernel_launches"]))
+        dist.barrier()
+        q.put((rank, None if full is None else full.numpy(), None if mat is None else mat.numpy(), launches))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+@pytest.mark.timeout(300)
+def test_two_processes_one_gpu_product_path():
+    """The first time two bemcub contexts run side by side under torch.distributed must not be the
+    multi-GPU bench: two gloo ranks share cuda:0, each evaluates its range with the CUDA library, and
+    the gathered result meets the parity bar against the oracle."""
+    import torch.multiprocessing as mp
+
+    import oracle
+    from paper_1606_03743_b200 import synth
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_gpu_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted([q.get(timeout=240) for _ in procs], key=lambda g: g[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (_, full, mat, launches), (_, full1, mat1, _) = got
+    assert full1 is None and mat1 is None and launches > 0
+    c = synth.config4(scale=0.002, ntracks=23, npts_per_track=31)
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=oracle.default_policy(True), want_counts=True)
+    tol = np.where(ref["nana"] > 0, 1e-10, 1e-12)
+    assert np.all(np.abs(full[:, 0] - ref["phi"]) <= tol * ref["Sphi"])
+    assert np.all(np.abs(full[:, 1:] - ref["E"]).max(axis=1) <= tol * ref["SE"])
+    A, code = oracle.assemble_rows(c["etype"], c["verts"], np.arange(len(c["etype"])), oracle.default_policy(False))
+    rel = np.abs(mat - A) / np.abs(A)
+    assert rel[code < 5].max() <= 1e-12 and rel[code == 5].max() <= 1e-10
