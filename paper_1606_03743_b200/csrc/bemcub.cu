@@ -226,7 +226,8 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) 
   // Largest R that still leaves enough items per warp.  A fixed rule only gains from a larger R
   // (more chains per lane), so it may use many splits; in adaptive mode a larger tile of FEW field
   // points is also a looser tile (more upgraded elements), so R grows only when tiles are plentiful
-  // (measured on 1.5e6 elements x 1e4 points: fixed rule +4 % with R = 4, adaptive -5 %).
+  // (measured on 1.5e6 elements x 1e4 points: fixed rule +4 % with R = 4, adaptive -5 %; round 2, forcing
+  // R = 4: that shape -6 %, the mat-vec of the level-5 icosphere solve -6 %).
   const int64_t split_cap = adaptive ? 64 : 512, per_warp = adaptive ? 8 : 16;
   for (int R = max_r; R > 1; R >>= 1) {
     const int64_t nt = (m + 32 * R - 1) / (32 * R);
