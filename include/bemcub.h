@@ -121,10 +121,14 @@ typedef struct {
 int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream);
 int bemcub_destroy(bemcub_ctx* ctx);
 
-/* HOST struct.  want_field = 0: the printed triangle-potential limits 3/8/20/80/1500 (L159) for
- * both element types; want_field = 1: limits for Phi and E together ("slightly higher", L159):
- * triangles 4/10/25/100/2000, rectangles 6/15/40/150/3000 (reading 7).
- * allow_upgrade = 1, use_levels_mask = 63. */
+/* HOST struct.  want_field = BEMCUB_POLICY_POTENTIAL (0): the printed triangle-potential limits
+ * 3/8/20/80/1500 (L159) for both element types; BEMCUB_POLICY_FIELD (1): limits for Phi and E together
+ * ("slightly higher", L159): triangles 4/10/25/100/2000, rectangles 6/15/40/150/3000 (DESIGN.md
+ * reading 7); BEMCUB_POLICY_FIELD_F32 (2): limits for calls with BEMCUB_F32 - the distance ratio from
+ * which a rule's own field error is below the FP32 rounding floor of 1e-7 (triangles 2/2/3/6/25,
+ * rectangles 2/3/4/8/30; Sec. 4 protocol, profiles/r2_accuracy_sweep.txt).
+ * allow_upgrade = 1, use_levels_mask = 63.  Any other want_field: INVALID_ARG. */
+enum { BEMCUB_POLICY_POTENTIAL = 0, BEMCUB_POLICY_FIELD = 1, BEMCUB_POLICY_FIELD_F32 = 2 };
 int bemcub_default_policy(bemcub_policy* host_policy, int want_field);
 
 /* Copies the mesh into the ctx and computes centroid, area and L of every element (Eq. 3.2/3.3,
@@ -136,10 +140,11 @@ int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const d
  *   sigma[n]; rule_id = BEMCUB_RULE_L0..L4 (fixed rule for every pair; no near-field switching: a
  *   field point that coincides with a Gaussian point gives IEEE inf/nan) or BEMCUB_RULE_ADAPTIVE
  *   (policy must be non-NULL; HOST pointer); field_pts[m][3]; out_phi[m]; out_E[m][3] or NULL.
- *   precision = BEMCUB_F64, or BEMCUB_F32 (fixed rules only: BEMCUB_RULE_ADAPTIVE with BEMCUB_F32 returns
- *   INVALID_ARG - the distance-ratio limits are accuracy limits of FP64 arithmetic): points, field
- *   points and the interaction arithmetic are FP32, sums of at most 128 terms are FP32 and those
- *   block sums are accumulated in FP64; buffers keep their double type.
+ *   precision = BEMCUB_F64, or BEMCUB_F32: points, field points and the interaction arithmetic are
+ *   FP32, sums of at most 128 terms are FP32 and those block sums are accumulated in FP64; the rule
+ *   choice of BEMCUB_RULE_ADAPTIVE and the analytic branch stay FP64 (use the limits of
+ *   BEMCUB_POLICY_FIELD_F32: the FP64 limits only buy points whose gain FP32 rounding hides);
+ *   buffers keep their double type.
  * sigma == NULL: evaluate with the sigma of the previous call on this ctx that passed one (the ctx
  *   keeps a copy; INVALID_ARG if there is none).  Rule levels already expanded for that sigma are
  *   reused, so the preprocessing pass a1 is skipped - what a particle tracker wants, which asks
@@ -236,16 +241,18 @@ int bemcub_expand_points(bemcub_ctx* ctx, const double* sigma, int rule_id, doub
 int bemcub_get_geometry(bemcub_ctx* ctx, double* out_cen, double* out_area, double* out_L);
 
 /* Roofline denominator: the issue rate of the plain FP64 pipe.  bemcub_fp64_issue_sweep runs, for
- * about `seconds_per_variant` each, kernels that issue nothing but independent chains of one FP64
- * instruction kind - mix 0: DFMA, 1: DADD, 2: DMUL, 3: the 8 DFMA : 6 DMUL : 4 DADD mix of Eq. 4.1 -
- * at 8, 16 and 32 warps per SM, every instruction reading at most two vector registers (the second
- * source is a uniform register: an FP64 instruction with three distinct vector-register sources
- * issues at 2/3 of the rate).  HOST outputs, index = mix * 3 + occupancy:
- * host_rates[12] in FP64 lane-instructions per second (warp instructions x 32), host_sm_mhz[12]
- * (may be NULL) the SM clock during that launch (cycle counter / global timer).
+ * about `seconds_per_variant` each, kernels that issue nothing but independent chains of FP64
+ * instructions - mix 0: DFMA, 1: DADD, 2: DMUL, 3: the 8 DFMA : 6 DMUL : 4 DADD mix of Eq. 4.1, every
+ * instruction reading at most two vector registers (the second source is a uniform register) - at 8,
+ * 16 and 32 warps per SM.  Two further mixes document what costs issue cycles
+ * and never win: 4: DFMA with three distinct, changing vector-register sources; 5: mix 0 with one
+ * integer multiply-add after every second DFMA (its rate still counts the DFMAs only).
+ * HOST outputs, index = mix * 3 + occupancy: host_rates[BEMCUB_PEAK_VARIANTS] in FP64
+ * lane-instructions per second (warp instructions x 32), host_sm_mhz[BEMCUB_PEAK_VARIANTS] (may be
+ * NULL) the SM clock during that launch (cycle counter / global timer).
  * bemcub_fp64_peak = the maximum of such a sweep lasting about `seconds` in total; flop/s = 2x (every
  * instruction counted as an FMA).  Both synchronise. */
-#define BEMCUB_PEAK_VARIANTS 12
+#define BEMCUB_PEAK_VARIANTS 18
 int bemcub_fp64_issue_sweep(bemcub_ctx* ctx, double seconds_per_variant, double* host_rates, double* host_sm_mhz);
 int bemcub_fp64_peak(bemcub_ctx* ctx, double seconds, double* host_fp64_inst_per_s);
 

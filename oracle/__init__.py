@@ -109,9 +109,13 @@ def points(etype, verts, sigma, level: int):
     return out
 
 
-def default_policy(want_field: bool) -> np.ndarray:
+def default_policy(want_field) -> np.ndarray:
+    """dr[2][5]; want_field 0 / False: printed potential limits (L159), 1 / True: Phi+E limits,
+    2: limits for single-precision evaluation."""
     dr = np.zeros((2, 5))
-    lib().orc_default_policy(_p(dr), int(want_field))
+    rc = lib().orc_default_policy(_p(dr), int(want_field))
+    if rc:
+        raise ValueError(f"orc_default_policy rc={rc}")
     return dr
 
 

@@ -730,9 +730,14 @@ int orc_default_policy(double* dr, int want_field) {
     static const double pot[5] = {3, 8, 20, 80, 1500};
     static const double ftri[5] = {4, 10, 25, 100, 2000};
     static const double frect[5] = {6, 15, 40, 150, 3000};
+    // want_field = 2: limits for single-precision evaluation - the distance ratio from which each
+    // rule's own field error is below the FP32 rounding floor of 1e-7 (same protocol, reading 7)
+    static const double f32tri[5] = {2, 2, 3, 6, 25};
+    static const double f32rect[5] = {2, 3, 4, 8, 30};
+    if (want_field < 0 || want_field > 2) return ERR_INVALID;
     for (int b = 0; b < 5; ++b) {
-        dr[b] = want_field ? ftri[b] : pot[b];
-        dr[5 + b] = want_field ? frect[b] : pot[b];
+        dr[b] = want_field == 2 ? f32tri[b] : want_field ? ftri[b] : pot[b];
+        dr[5 + b] = want_field == 2 ? f32rect[b] : want_field ? frect[b] : pot[b];
     }
     return ERR_OK;
 }

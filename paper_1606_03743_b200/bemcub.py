@@ -153,7 +153,10 @@ def bemcub_destroy(ctx) -> None:
     _check(_lib.bemcub_destroy(ctx), "bemcub_destroy")
 
 
-def bemcub_default_policy(want_field: bool) -> bemcub_policy:
+POLICY_POTENTIAL, POLICY_FIELD, POLICY_FIELD_F32 = 0, 1, 2
+
+
+def bemcub_default_policy(want_field) -> bemcub_policy:
     p = bemcub_policy()
     _check(_lib.bemcub_default_policy(C.byref(p), int(want_field)), "bemcub_default_policy")
     return p
@@ -259,13 +262,14 @@ def bemcub_fp64_peak(ctx, seconds: float) -> float:
     return v.value
 
 
-PEAK_VARIANTS = 12
-PEAK_MIXES = ("DFMA", "DADD", "DMUL", "mix 8 DFMA : 6 DMUL : 4 DADD")
+PEAK_VARIANTS = 18
+PEAK_MIXES = ("DFMA", "DADD", "DMUL", "mix 8 DFMA : 6 DMUL : 4 DADD", "DFMA, 3 distinct vector-register sources (model evidence)",
+              "DFMA + 1 IMAD per 2 DFMA, DFMAs counted (model evidence)")
 PEAK_WARPS = (8, 16, 32)
 
 
 def bemcub_fp64_issue_sweep(ctx, seconds_per_variant: float):
-    """(rates[12] FP64 lane-instructions/s, sm_mhz[12]); index = mix * 3 + occupancy."""
+    """(rates[18] FP64 lane-instructions/s, sm_mhz[18]); index = mix * 3 + occupancy."""
     rates, mhz = np.zeros(PEAK_VARIANTS), np.zeros(PEAK_VARIANTS)
     _check(_lib.bemcub_fp64_issue_sweep(ctx, seconds_per_variant, _hptr(rates), _hptr(mhz)), "bemcub_fp64_issue_sweep")
     return rates, mhz

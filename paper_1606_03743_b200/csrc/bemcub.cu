@@ -260,10 +260,10 @@ int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
   return BEMCUB_OK;
 }
 
-template <int R, int MODE = kModePhiE>
+template <typename T, int R, int MODE = kModePhiE>
 int launch_adaptive(bemcub_ctx* c, const AdaptiveParams& ap, const SplitPlan& sp) {
-  const size_t smem = eval_smem_bytes<double>();
-  eval_adaptive_kernel<R, MODE><<<sp.grid, kThreads, smem, c->stream>>>(ap);
+  const size_t smem = eval_smem_bytes<T>();
+  eval_adaptive_kernel<T, R, MODE><<<sp.grid, kThreads, smem, c->stream>>>(ap);
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   return BEMCUB_OK;
@@ -284,20 +284,21 @@ int configure_fixed() {
   if constexpr (MODE != kModeGrad) rc = opt_in_smem(eval_fixed_kernel<T, 4, MODE>, b);
   return rc;
 }
-template <int MODE>
+template <typename T, int MODE>
 int configure_adaptive() {
   int rc;
-  const size_t b = eval_smem_bytes<double>();
-  if ((rc = opt_in_smem(eval_adaptive_kernel<1, MODE>, b)) || (rc = opt_in_smem(eval_adaptive_kernel<2, MODE>, b))) return rc;
-  if constexpr (MODE != kModeGrad) rc = opt_in_smem(eval_adaptive_kernel<4, MODE>, b);
+  const size_t b = eval_smem_bytes<T>();
+  if ((rc = opt_in_smem(eval_adaptive_kernel<T, 1, MODE>, b)) || (rc = opt_in_smem(eval_adaptive_kernel<T, 2, MODE>, b))) return rc;
+  if constexpr (MODE != kModeGrad) rc = opt_in_smem(eval_adaptive_kernel<T, 4, MODE>, b);
   return rc;
 }
 int configure_kernels() {
   int rc;
   if ((rc = configure_fixed<double, kModePhiE>()) || (rc = configure_fixed<double, kModePhi>()) ||
       (rc = configure_fixed<double, kModeGrad>()) || (rc = configure_fixed<float, kModePhiE>()) ||
-      (rc = configure_fixed<float, kModePhi>()) || (rc = configure_adaptive<kModePhiE>()) ||
-      (rc = configure_adaptive<kModePhi>()) || (rc = configure_adaptive<kModeGrad>()) ||
+      (rc = configure_fixed<float, kModePhi>()) || (rc = configure_adaptive<double, kModePhiE>()) ||
+      (rc = configure_adaptive<double, kModePhi>()) || (rc = configure_adaptive<double, kModeGrad>()) ||
+      (rc = configure_adaptive<float, kModePhiE>()) || (rc = configure_adaptive<float, kModePhi>()) ||
       (rc = opt_in_smem(assemble_kernel, assemble_smem_bytes())) ||
       (rc = opt_in_smem(inner_loop_kernel<4>, eval_smem_bytes<double>())))
     return rc;
@@ -416,9 +417,14 @@ int bemcub_default_policy(bemcub_policy* hp, int want_field) {
   static const double pot[5] = {3, 8, 20, 80, 1500};
   static const double ftri[5] = {4, 10, 25, 100, 2000};
   static const double frect[5] = {6, 15, 40, 150, 3000};
+  // BEMCUB_POLICY_FIELD_F32: where each rule's own error of the field falls below the FP32 rounding
+  // floor (1e-7; profiles/r2_accuracy_sweep.txt) - N = 33 is never worth its points in FP32 on triangles
+  static const double f32tri[5] = {2, 2, 3, 6, 25};
+  static const double f32rect[5] = {2, 3, 4, 8, 30};
+  if (want_field < 0 || want_field > BEMCUB_POLICY_FIELD_F32) return BEMCUB_ERR_INVALID_ARG;
   for (int b = 0; b < 5; ++b) {
-    hp->dr[0][b] = want_field ? ftri[b] : pot[b];
-    hp->dr[1][b] = want_field ? frect[b] : pot[b];
+    hp->dr[0][b] = want_field == BEMCUB_POLICY_FIELD_F32 ? f32tri[b] : want_field ? ftri[b] : pot[b];
+    hp->dr[1][b] = want_field == BEMCUB_POLICY_FIELD_F32 ? f32rect[b] : want_field ? frect[b] : pot[b];
   }
   hp->allow_upgrade = 1;
   hp->use_levels_mask = 63;
@@ -564,7 +570,6 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   if (grad && precision != BEMCUB_F64) return BEMCUB_ERR_INVALID_ARG;  // the gradient is FP64 only
   PolicyDev pol;
   if (adaptive) {
-    if (precision != BEMCUB_F64) return BEMCUB_ERR_INVALID_ARG;  // the adaptive path is FP64 only
     int rc = build_policy(host_policy, &pol);
     if (rc) return rc;
     // derivatives exist for the point charges only (L273): no analytic branch in a gradient call
@@ -714,7 +719,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   } else {
     AdaptiveParams ap;
     for (int l = 0; l < 5; ++l) {
-      ap.lvl_pts[l] = (const double4*)c->pts64[l].ptr;
+      ap.lvl_pts[l] = precision == BEMCUB_F64 ? c->pts64[l].ptr : c->pts32[l].ptr;
       ap.stride[l] = c->stride[l];
     }
     ap.cenL = (const double4*)c->cenL.ptr;
@@ -734,9 +739,15 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     ap.queue = c->d_counters + 2;
     ap.counters = c->d_counters;
     CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
-    if (grad) rc = sp.R == 2 ? launch_adaptive<2, kModeGrad>(c, ap, sp) : launch_adaptive<1, kModeGrad>(c, ap, sp);
-    else if (!out_E) rc = sp.R == 4 ? launch_adaptive<4, kModePhi>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2, kModePhi>(c, ap, sp) : launch_adaptive<1, kModePhi>(c, ap, sp);
-    else rc = sp.R == 4 ? launch_adaptive<4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<2>(c, ap, sp) : launch_adaptive<1>(c, ap, sp);
+    if (grad) rc = sp.R == 2 ? launch_adaptive<double, 2, kModeGrad>(c, ap, sp) : launch_adaptive<double, 1, kModeGrad>(c, ap, sp);
+    else if (precision == BEMCUB_F64 && !out_E)
+      rc = sp.R == 4 ? launch_adaptive<double, 4, kModePhi>(c, ap, sp) : sp.R == 2 ? launch_adaptive<double, 2, kModePhi>(c, ap, sp) : launch_adaptive<double, 1, kModePhi>(c, ap, sp);
+    else if (precision == BEMCUB_F64)
+      rc = sp.R == 4 ? launch_adaptive<double, 4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<double, 2>(c, ap, sp) : launch_adaptive<double, 1>(c, ap, sp);
+    else if (!out_E)
+      rc = sp.R == 4 ? launch_adaptive<float, 4, kModePhi>(c, ap, sp) : sp.R == 2 ? launch_adaptive<float, 2, kModePhi>(c, ap, sp) : launch_adaptive<float, 1, kModePhi>(c, ap, sp);
+    else
+      rc = sp.R == 4 ? launch_adaptive<float, 4>(c, ap, sp) : sp.R == 2 ? launch_adaptive<float, 2>(c, ap, sp) : launch_adaptive<float, 1>(c, ap, sp);
     if (rc) return rc;
     c->counters_pending = true;
     c->counters_counted = true;
@@ -932,10 +943,12 @@ int bemcub_fp64_issue_sweep(bemcub_ctx* c, double seconds_per_variant, double* h
     CUDA_TRY(cudaEventRecord(e0, c->stream));
     double* out = (double*)c->partial.ptr;
     switch (mix) {
-      case 0: fp64_issue_kernel<0><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
-      case 1: fp64_issue_kernel<1><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
-      case 2: fp64_issue_kernel<2><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
-      default: fp64_issue_kernel<3><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9); break;
+      case 0: fp64_issue_kernel<0><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9, 3); break;
+      case 1: fp64_issue_kernel<1><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9, 3); break;
+      case 2: fp64_issue_kernel<2><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9, 3); break;
+      case 3: fp64_issue_kernel<3><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9, 3); break;
+      case 4: fp64_issue_kernel<4><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9, 3); break;
+      default: fp64_issue_kernel<5><<<blocks, threads, 0, c->stream>>>(out, clk, iters, 0.999999, 1e-9, 3); break;
     }
     c->stats.kernel_launches += 1;
     CUDA_TRY(cudaGetLastError());
@@ -944,7 +957,7 @@ int bemcub_fp64_issue_sweep(bemcub_ctx* c, double seconds_per_variant, double* h
     CUDA_TRY(cudaEventElapsedTime(ms, e0, e1));
     return BEMCUB_OK;
   };
-  for (int mix = 0; mix < 4; ++mix) {
+  for (int mix = 0; mix < BEMCUB_PEAK_VARIANTS / 3; ++mix) {
     const int chains = mix == 3 ? 18 : 16;
     for (int occ = 0; occ < 3; ++occ) {
       const int per_sm = 1 << occ;  // CTAs of 8 warps per SM: 8, 16, 32 warps

@@ -202,6 +202,9 @@ __device__ __forceinline__ void consume_into(const float4* buf, int cnt, const f
   }
 }
 
+__device__ __forceinline__ double4 ldg_point(const double4* p) { return ldg4(p); }
+__device__ __forceinline__ float4 ldg_point(const float4* p) { return __ldg(p); }
+
 template <typename T, int R>
 __device__ __forceinline__ void load_field_points(const double* __restrict__ field, int64_t m, int64_t tile, int lane,
                                                   T (&px)[R], T (&py)[R], T (&pz)[R]) {
@@ -391,7 +394,7 @@ __device__ __forceinline__ int rule_npts(int type, int level) {
 }
 
 struct AdaptiveParams {
-  const double4* lvl_pts[5];  // expanded points per level (FP64), may be null for disabled levels
+  const void* lvl_pts[5];  // expanded points per level (Point4<T> records), may be null for disabled levels
   int stride[5];
   const double4* cenL;
   const uint8_t* type;
@@ -448,10 +451,13 @@ __device__ __forceinline__ void analytic_element(const AdaptiveParams& p, int64_
 }
 
 // Element `e` with the exact per-pair rule choice (tile straddles a band limit and the policy
-// does not allow, or the analytic limit forbids, an upgrade).
-template <int R, int MODE>
-__device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, int lane,
-                                           Accum<double, R, MODE>& tot, WarpScratch* scr) {
+// does not allow, or the analytic limit forbids, an upgrade).  T = float: points and interaction
+// arithmetic in FP32 (one element's sum: at most 33 terms), added to the FP64 totals.
+template <typename T, int R, int MODE>
+__device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e, const WarpTile<R>& w, const T (&qx)[R],
+                                              const T (&qy)[R], const T (&qz)[R], int lane, Accum<double, R, MODE>& tot,
+                                              WarpScratch* scr) {
+  typedef typename Point4<T>::type P4;
   const double4 c = ldg4(p.cenL + e);
   const int t = __ldg(p.type + e);
   int lev[R];
@@ -478,28 +484,28 @@ __device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e
       if (lane == 0) scr->n_ana += (unsigned long long)all;
     } else {
       const int N = rule_npts(t, l);
-      const double4* src = p.lvl_pts[l] + e * p.stride[l];
+      const P4* src = reinterpret_cast<const P4*>(p.lvl_pts[l]) + e * p.stride[l];
       // The level's sum is formed for every field point of the lane and then SELECTED, not masked
       // by a zero charge: a field point that does not take this level may sit exactly on one of its
       // nodes (an element's own centroid is a node of the 7- and 19-point rules), and 0 * inf = NaN.
-      Accum<double, R, MODE> part;
+      Accum<T, R, MODE> part;
       part.zero();
-      double4 s = ldg4(src);
+      P4 s = ldg_point(src);
       const double c375 = c_three_eighths;
 #pragma unroll 1
       for (int i = 0; i < N; ++i) {
-        const double4 nxt = ldg4(src + min(i + 1, N - 1));  // prefetch: hides the global-load latency
-        interact<double, R, MODE>(s, w.px, w.py, w.pz, part, c375);
+        const P4 nxt = ldg_point(src + min(i + 1, N - 1));  // prefetch: hides the global-load latency
+        interact<T, R, MODE>(s, qx, qy, qz, part, c375);
         s = nxt;
       }
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         if (!take[r]) continue;
-        tot.phi[r] += part.phi[r];
+        tot.phi[r] += (double)part.phi[r];
         if constexpr (MODE != kModePhi) {
-          tot.ex[r] += part.ex[r];
-          tot.ey[r] += part.ey[r];
-          tot.ez[r] += part.ez[r];
+          tot.ex[r] += (double)part.ex[r];
+          tot.ey[r] += (double)part.ey[r];
+          tot.ez[r] += (double)part.ez[r];
         }
         if constexpr (MODE == kModeGrad) {
           tot.sg[r] += part.sg[r];
@@ -515,11 +521,16 @@ __device__ __forceinline__ void mixed_element(const AdaptiveParams& p, int64_t e
   }
 }
 
-template <int R, int MODE = kModePhiE>
+// T = double: the FP64 path.  T = float: the points, the field points of the interaction and its
+// arithmetic are FP32 (window sums of <= kBuf terms, added to FP64 totals); the rule choice and the
+// analytic branch stay FP64.
+template <typename T, int R, int MODE = kModePhiE>
 __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid_constant__ AdaptiveParams p) {
+  typedef typename Point4<T>::type P4;
+  static_assert(sizeof(T) == 8 || MODE != kModeGrad, "the field gradient is FP64 only");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const WarpSmem<double4> ws = warp_smem<double4>(smem_raw, warp, lane);
+  const WarpSmem<P4> ws = warp_smem<P4>(smem_raw, warp, lane);
   WarpScratch* const scr = ws.scr;
   uint32_t phases = 0;
   KernelClock clk;
@@ -534,6 +545,13 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     w.first = tile * (32 * R);
     w.m = p.m;
     load_field_points<double, R>(p.field, p.m, tile, lane, w.px, w.py, w.pz);
+    float fx[sizeof(T) == 8 ? 1 : R], fy[sizeof(T) == 8 ? 1 : R], fz[sizeof(T) == 8 ? 1 : R];  // FP32 path: narrowed copies
+    if constexpr (sizeof(T) == 4) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        fx[r] = (float)w.px[r]; fy[r] = (float)w.py[r]; fz[r] = (float)w.pz[r];
+      }
+    }
     {  // bounding sphere of the tile (clamped duplicates lie inside it by construction).  Points
        // with a non-finite coordinate are left out: their own result is NaN whatever the rule, and
        // they must not spoil the rule choice of the other points of the tile.
@@ -585,7 +603,7 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
     // memory between two produce() calls was measured: no gain at scale 0.25, 3 % slower at full size.)
     int64_t batch_next = e_begin;
     int cnt = 0, pre = 0, total = 0, lvl = 0, cursor = 32;
-    const double4* src = nullptr;
+    const P4* src = nullptr;
 
     // Fills `stage` with the next round of whole elements; returns the number of points (0 = done).
     auto produce = [&](int stage) -> int {
@@ -595,11 +613,11 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
           const int nstage = sp.nstage;
           cursor = sp.next;
           if (nstage == 0) continue;
-          if (lane == 0) mbar_arrive_expect_tx(ws.bar0 + 8 * stage, (uint32_t)(nstage * sizeof(double4)));
+          if (lane == 0) mbar_arrive_expect_tx(ws.bar0 + 8 * stage, (uint32_t)(nstage * sizeof(P4)));
           __syncwarp();
           if (sp.head)
-            tma_load_1d(ws.win0 + (uint32_t)((stage * kBuf + (pre - sp.base)) * sizeof(double4)), src,
-                        (uint32_t)((sp.run_end - pre) * sizeof(double4)), ws.bar0 + 8 * stage);
+            tma_load_1d(ws.win0 + (uint32_t)((stage * kBuf + (pre - sp.base)) * sizeof(P4)), src,
+                        (uint32_t)((sp.run_end - pre) * sizeof(P4)), ws.bar0 + 8 * stage);
           if (lane == 0) scr->n_inter += (unsigned long long)nstage * scr->nvalid;
           return nstage;
         }
@@ -635,7 +653,7 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
               is_ana = true;
             } else {
               cnt = rule_npts(t, lvl);
-              src = p.lvl_pts[lvl] + e * p.stride[lvl];
+              src = reinterpret_cast<const P4*>(p.lvl_pts[lvl]) + e * p.stride[lvl];
             }
           }
         }
@@ -656,7 +674,8 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
         while (xmask) {
           const int l = __ffs(xmask) - 1;
           xmask &= xmask - 1;
-          mixed_element<R, MODE>(p, batch0 + l, w, lane, tot, scr);
+          if constexpr (sizeof(T) == 8) mixed_element<double, R, MODE>(p, batch0 + l, w, w.px, w.py, w.pz, lane, tot, scr);
+          else mixed_element<float, R, MODE>(p, batch0 + l, w, fx, fy, fz, lane, tot, scr);
         }
       }
     };
@@ -668,7 +687,8 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
       if (cur > 0) {
         mbar_wait(ws.bar0 + 8 * stage, (phases >> stage) & 1u);
         phases ^= 1u << stage;
-        consume_into<R, MODE>(ws.win + stage * kBuf, cur, w.px, w.py, w.pz, tot);
+        if constexpr (sizeof(T) == 8) consume_into<R, MODE>(ws.win + stage * kBuf, cur, w.px, w.py, w.pz, tot);
+        else consume_into<R, MODE>(ws.win + stage * kBuf, cur, fx, fy, fz, tot);
         __syncwarp();
       }
       if (nxt == 0) break;

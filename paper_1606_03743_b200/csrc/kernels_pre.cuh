@@ -193,13 +193,20 @@ __global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride,
 // one FP64 instruction kind, the second operand in a uniform register so that an instruction reads at
 // most two vector registers - the form in which the pipe issues one warp instruction per two cycles
 // per scheduler.  MIX 0: DFMA, 1: DADD, 2: DMUL, 3: the 8 DFMA : 6 DMUL : 4 DADD mix of Eq. 4.1.
+// Two more mixes are not candidates for the peak but evidence for the issue model the kernels are
+// written for: MIX 4: DFMA whose three sources are three different, changing
+// vector registers (3 dispatch cycles instead of 2); MIX 5: the DFMA loop of MIX 0 with one integer
+// multiply-add after every second DFMA (a non-FP64 instruction takes a dispatch cycle of its own).
 // clk[0] = SM cycles, clk[1] = nanoseconds of the launch as thread 0 of CTA 0 saw them.
 template <int MIX>
-__global__ void fp64_issue_kernel(double* out, unsigned long long* clk, int iters, double a, double b) {
+__global__ void fp64_issue_kernel(double* out, unsigned long long* clk, int iters, double a, double b, int ia) {
   constexpr int C = (MIX == 3) ? 18 : 16;
   double x[C];
+  int n[8];
 #pragma unroll
   for (int k = 0; k < C; ++k) x[k] = 1.0 + (double)(threadIdx.x + k) * 1e-3;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) n[k] = threadIdx.x + k;
   KernelClock kc;
   kc.begin();
   for (int i = 0; i < iters; ++i) {
@@ -207,9 +214,11 @@ __global__ void fp64_issue_kernel(double* out, unsigned long long* clk, int iter
     for (int u = 0; u < 4; ++u) {
 #pragma unroll
       for (int k = 0; k < C; ++k) {
-        if (MIX == 0 || (MIX == 3 && k < 8)) x[k] = __fma_rn(x[k], a, b);
+        if (MIX == 4) x[k] = __fma_rn(x[k], x[(k + 5) % C], x[(k + 11) % C]);
+        else if (MIX == 0 || MIX == 5 || (MIX == 3 && k < 8)) x[k] = __fma_rn(x[k], a, b);
         else if (MIX == 1 || (MIX == 3 && k >= 14)) x[k] = __dadd_rn(x[k], b);
         else x[k] = __dmul_rn(x[k], a);
+        if (MIX == 5 && (k & 1)) n[k >> 1] = n[k >> 1] * ia + i;
       }
     }
   }
@@ -220,6 +229,10 @@ __global__ void fp64_issue_kernel(double* out, unsigned long long* clk, int iter
   double s = 0.0;
 #pragma unroll
   for (int k = 0; k < C; ++k) s += x[k];
+  if (MIX == 5) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += (double)n[k];
+  }
   out[blockIdx.x * (int64_t)blockDim.x + threadIdx.x] = s;
 }
 

@@ -391,3 +391,33 @@ def test_sub_ranges_reproduce_the_full_call(world):
     torch.cuda.synchronize()
     assert torch.equal(torch.cat(pieces, dim=0), A)                      # per-pair policy: bit-identical
     g.close()
+
+
+# ------------------------------------------------------------------ FP32 with the distance-ratio choice
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+def test_adaptive_f32_small_mixed_and_single_element(allow_upgrade):
+    """BEMCUB_RULE_ADAPTIVE with BEMCUB_F32: rule choice and analytic branch in FP64, points and
+    interactions in FP32, with the limits of BEMCUB_POLICY_FIELD_F32.  Parity 1e-5 against the
+    long-double oracle under the same limits; with allow_upgrade = 0 the same interaction count; and
+    the result is as accurate as FP32 allows (the limits are not too low)."""
+    dr32 = oracle.default_policy(2)
+    for c in (synth.config4(scale=0.002, ntracks=40, npts_per_track=53),
+              synth.config5(synth.TRI, m=20000, dr_lo=0.3, dr_hi=1e4),
+              synth.config5(synth.RECT, m=20000, dr_lo=0.3, dr_hi=1e4)):
+        g = Gpu(c["etype"], c["verts"])
+        pol = g.b.bemcub_default_policy(g.b.POLICY_FIELD_F32)
+        assert [list(pol.dr[0]), list(pol.dr[1])] == dr32.tolist()
+        pol.allow_upgrade = allow_upgrade
+        ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=dr32, want_counts=True)
+        for want_E in (True, False):
+            phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol, precision=1, want_E=want_E)
+            assert_parity(phi, E, ref, TOL_F32, f"adaptive f32 {c['name']} upgrade={allow_upgrade}")
+            if not allow_upgrade:
+                assert g.stats()["point_interactions"] == int(ref["npi"].sum())
+        # against the accurate answer (FP64 limits, long double): at the FP32 rounding floor
+        exact = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=oracle.default_policy(True))
+        phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol, precision=1)
+        e_phi = np.abs(phi - exact["phi"]) / exact["Sphi"]
+        e_E = np.abs(E - exact["E"]).max(axis=1) / exact["SE"]
+        assert e_phi.mean() <= 2e-7 and e_E.mean() <= 4e-7, (c["name"], e_phi.mean(), e_E.mean())
+        g.close()

@@ -440,6 +440,32 @@ def test_field_dr_limits_by_the_papers_protocol(kind):
     assert list(fdr) == expect
 
 
+@pytest.mark.parametrize("kind", [TRI, RECT])
+def test_single_precision_limits_sit_at_the_fp32_floor(kind):
+    """want_field = 2: at each limit the rule that takes over has a field error (long-double arithmetic,
+    i.e. the rule's own truncation error) at or below the FP32 rounding floor of 1e-7, and is above it
+    40 % nearer - so in FP32 the more accurate rule would buy nothing there."""
+    dr32 = oracle.default_policy(2)[kind]
+    assert np.all(np.diff(dr32) >= 0) and np.all(dr32 <= oracle.default_policy(True)[kind])
+    n = 1000
+    et, verts = synth.random_elements(kind, n, seed=4321 + kind)
+    cen, _, L = oracle.geometry(et, verts)
+    dirs = synth.isotropic_directions(np.random.default_rng(78 + kind), n)
+
+    def field_error(level, ratio):
+        P = cen + dirs * (ratio * L)[:, None]
+        ref = oracle.evaluate_pairs(et, verts, P, 5 if ratio < 12.0 else 4)
+        r = oracle.evaluate_pairs(et, verts, P, level)
+        return float((np.abs(r["E"] - ref["E"]).sum(axis=1) / np.linalg.norm(ref["E"], axis=1)).mean())
+
+    for band, level in ((4, 0), (3, 1), (2, 2), (1, 3), (0, 4)):
+        lim = float(dr32[band])
+        if band < 4 and lim == float(dr32[band + 1]):
+            continue                                  # empty range [dr[band], dr[band + 1]): this rule is never chosen
+        assert field_error(level, lim) <= 1.3e-7, (kind, level, lim, field_error(level, lim))
+        assert field_error(level, 0.6 * lim) > 1.3e-7, (kind, level, 0.6 * lim)
+
+
 def test_adaptive_sum_uses_per_pair_rule():
     """Adaptive evaluation = sum over elements of the fixed-rule value at the level the policy
     picks per pair; point-interaction counts follow; the analytic branch is taken below the
