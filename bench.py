@@ -57,7 +57,8 @@ def parse_args():
                     choices=["cfg4", "cfg1", "cfg2", "cfg3", "cfg5", "solve", "table3", "accuracy"])
     ap.add_argument("--scale", type=float, default=1.0, help="config-4 size factor (profiling only)")
     ap.add_argument("--rule", type=int, default=1, help="fixed rule level of --workload cfg2 / cfg5 / table3 (-1 = adaptive)")
-    ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="fixed-rule workloads only")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
+                    help="f32: the FP32 variant (adaptive workloads then use the BEMCUB_POLICY_FIELD_F32 limits); not the bench line")
     ap.add_argument("--gradient", action="store_true",
                     help="also compute the field gradient (bemcub_eval_gradient; cubature levels only) - not the bench line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -460,7 +461,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     h, dev, n, m = r.h, r.dev, r.n, r.m
     is_matrix = args.workload in ("cfg3", "solve")
     is_solve = args.workload == "solve"
-    precision = b.F32 if (args.workload in ("cfg2", "cfg5") and args.precision == "f32") else b.F64
+    precision = b.F32 if (args.precision == "f32" and not is_matrix and not args.gradient) else b.F64
     adaptive = c["rule"] == -1
     solve_info = {}
     if is_solve:
@@ -477,7 +478,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         out = torch.empty((n, n), dtype=torch.float64, device=dev)
         step = lambda: b.bemcub_assemble(h, pol, out, n)
     else:
-        pol = b.bemcub_default_policy(True) if adaptive else None
+        # FP32 with the distance-ratio choice takes the limits made for it (BEMCUB_POLICY_FIELD_F32)
+        pol = b.bemcub_default_policy(b.POLICY_FIELD_F32 if precision == b.F32 else b.POLICY_FIELD) if adaptive else None
         phi = torch.empty(m, dtype=torch.float64, device=dev)
         E = torch.empty((m, 3), dtype=torch.float64, device=dev)
         if args.gradient:
@@ -511,7 +513,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     fpi = FLOP_PER_INTERACTION_PHI if is_matrix else (FLOP_PER_INTERACTION_GRAD if args.gradient else FLOP_PER_INTERACTION)
     ipi = 12 if is_matrix else (28 if args.gradient else 18)   # FP64 instructions per interaction
     inter_own = None
-    if (adaptive and not args.gradient) or args.workload == "cfg3":
+    if (adaptive and not args.gradient and precision == b.F64) or args.workload == "cfg3":
         # the method's own work: one untimed call with the exact per-pair policy, counted on the device
         pol_pp = b.bemcub_default_policy(not is_matrix)
         pol_pp.allow_upgrade = 0
