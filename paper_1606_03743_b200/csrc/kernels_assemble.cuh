@@ -46,20 +46,21 @@ struct AssembleParams {
   unsigned long long* counters;
 };
 
-constexpr int kAsmWarps = 16;
+// Measured on config 3 (round 2): 4 rows per lane x 2 points per trip at 12 warps/SM 5.65 ms, 2 x 4 at 16
+// warps 5.80 ms, 2 x 4 at 12 warps 5.76 ms, 4 x 1 at 12 warps 6.20 ms.
+constexpr int kAsmWarps = 12;
 constexpr int kAsmThreads = kAsmWarps * 32;
-constexpr int kAsmR = 2;               // rows per lane
-constexpr int kAsmU = 4;               // points per trip; the expanded elements are padded to a multiple of it
+constexpr int kAsmR = 4;               // rows per lane
+constexpr int kAsmU = 2;               // points per trip; the expanded elements are padded to a multiple of it
 constexpr int kAsmRows = 32 * kAsmR;   // rows per tile
 constexpr int kGroupCols = 8;          // columns per output group: 64-byte row segments = two full sectors
-constexpr int kTilePad = kGroupCols + 2;  // row stride of the output tile: 16-byte aligned rows
-constexpr int kAqCap = 128;            // analytic pair queue (ring), entries = row << 26 | column
-constexpr int64_t kAsmMaxN = (int64_t)1 << 26;  // ... hence this many elements at most (a 2^26-square matrix is out of reach anyway)
+constexpr int kAqCap = kAsmR <= 2 ? 128 : 256;  // analytic pair queue (ring, >= 32 + 32 kAsmR), entries = row << 25 | column
+constexpr int64_t kAsmMaxN = (int64_t)1 << 25;  // ... hence this many elements at most (a 2^26-square matrix is out of reach anyway)
 
 // per-warp shared memory: window | output tile | segment tables | analytic queue | mbarriers | tallies
 struct AsmWarpSmem {
   double4 win[kStages][kBuf];
-  double tile[kAsmRows * kTilePad];
+  double tile[kGroupCols * kAsmRows];  // [column of the group][row]: conflict-free both ways
   uint32_t seg[kStages][32];  // col | npts << 8 | first << 16
   uint32_t aq[kAqCap];
   uint64_t bar[kStages];
@@ -97,11 +98,15 @@ __device__ __forceinline__ void phi_segment(const double4* __restrict__ pts, int
       for (int r = 0; r < kAsmR; ++r) part[u][r] = phi_one(s[u], s[u].w, px[r], py[r], pz[r], part[u][r], c375);
   }
 #pragma unroll
-  for (int r = 0; r < kAsmR; ++r) acc[r] = (part[0][r] + part[1][r]) + (part[2][r] + part[3][r]);
+  for (int r = 0; r < kAsmR; ++r) {
+    if constexpr (U == 4) acc[r] = (part[0][r] + part[1][r]) + (part[2][r] + part[3][r]);
+    else if constexpr (U == 2) acc[r] = part[0][r] + part[1][r];
+    else acc[r] = part[0][r];
+  }
 }
 
 __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_constant__ AssembleParams p) {
-  static_assert(kAsmU == 4, "phi_segment adds four partial sums");
+  static_assert(kAsmU == 4 || kAsmU == 2 || kAsmU == 1, "phi_segment's sum tree");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   AsmWarpSmem& sm = reinterpret_cast<AsmWarpSmem*>(smem_raw)[warp];
@@ -158,13 +163,13 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
 
     // analytic pair queue of this item: [aq_head, aq_tail) in the ring sm.aq
     int aq_head = 0, aq_tail = 0;
-    // Evaluates `take` (<= 32) queued pairs, one per lane: entry = row << 26 | column.
+    // Evaluates `take` (<= 32) queued pairs, one per lane: entry = row << 25 | column.
     auto drain = [&](int take) {
       __syncwarp();
       if (lane < take) {
         const uint32_t ent = sm.aq[(aq_head + lane) & (kAqCap - 1)];
-        const int row = (int)(ent >> 26);
-        const int64_t col = (int64_t)(ent & 0x3ffffffu);
+        const int row = (int)(ent >> 25);
+        const int64_t col = (int64_t)(ent & 0x1ffffffu);
         const double4 ci = ldg4(p.cenL + p.row0 + r0 + row);
         Vec3 V[4];
         const int nv = load_polygon(p.type, p.verts, col, V);
@@ -251,9 +256,10 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
             for (int r = 0; r < kAsmR; ++r) {
               const int row = r * 32 + lane;
               if (row < nrow_here) {
-                const double2* t = reinterpret_cast<const double2*>(&sm.tile[row * kTilePad]);
+                const double* t = &sm.tile[row];
                 double2* o = reinterpret_cast<double2*>(p.out + (r0 + row) * p.ld + jg);
-                const double2 a = t[0], b = t[1], c = t[2], d = t[3];
+                const double2 a = make_double2(t[0], t[kAsmRows]), b = make_double2(t[2 * kAsmRows], t[3 * kAsmRows]);
+                const double2 c = make_double2(t[4 * kAsmRows], t[5 * kAsmRows]), d = make_double2(t[6 * kAsmRows], t[7 * kAsmRows]);
                 o[0] = a; o[1] = b; o[2] = c; o[3] = d;
               }
             }
@@ -261,8 +267,8 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
             const int c = lane & (kGroupCols - 1);
             if ((gmask >> c) & 1u) {
               double* o = p.out + (r0 + (lane >> 3)) * p.ld + jg + c;
-              const double* t = &sm.tile[(lane >> 3) * kTilePad + c];
-              for (int row = lane >> 3; row < nrow_here; row += 4, o += 4 * p.ld, t += 4 * kTilePad) *o = *t;
+              const double* t = &sm.tile[c * kAsmRows + (lane >> 3)];
+              for (int row = lane >> 3; row < nrow_here; row += 4, o += 4 * p.ld, t += 4) *o = *t;
             }
           }
         }
@@ -282,7 +288,7 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
           double acc[kAsmR];
           phi_segment(&sm.win[stage][d >> 16], (int)((d >> 8) & 255u), px, py, pz, acc, c375);
 #pragma unroll
-          for (int r = 0; r < kAsmR; ++r) sm.tile[(r * 32 + lane) * kTilePad + (col & (kGroupCols - 1))] = acc[r];
+          for (int r = 0; r < kAsmR; ++r) sm.tile[(col & (kGroupCols - 1)) * kAsmRows + r * 32 + lane] = acc[r];
           gmask |= 1u << (col & (kGroupCols - 1));
         }
         __syncwarp();
@@ -375,7 +381,7 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
           const double D2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
           const bool take = ok[r] && p.pol.map[want_level(D2, c.w, p.pol.dr[t])] == 5;
           const unsigned bal = __ballot_sync(kFullMask, take);
-          if (take) sm.aq[(aq_tail + __popc(bal & lt_mask)) & (kAqCap - 1)] = ((uint32_t)(r * 32 + lane) << 26) | (uint32_t)j;
+          if (take) sm.aq[(aq_tail + __popc(bal & lt_mask)) & (kAqCap - 1)] = ((uint32_t)(r * 32 + lane) << 25) | (uint32_t)j;
           aq_tail += __popc(bal);
         }
         while (aq_tail - aq_head >= 32) drain(32);
