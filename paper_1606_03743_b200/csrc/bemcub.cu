@@ -863,11 +863,13 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   ap.counters = c->d_counters;
   ap.queue = c->d_counters + 2;
   CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
-  // items = (64-row tile) x (split of the columns, a multiple of 32): about 32 per warp
+  // items = (128-row tile) x (split of the columns, a multiple of 32): about 16 per warp, each met twice - the kernel
+  // runs the queue once for the expensive column batches of every item and once for the cheap ones (measured on
+  // config 3: 8 - 16 items per warp 5.25 ms, 32: 5.39, 64: 5.58, 4: 5.44; one pass over the queue: 5.33 ms at best)
   const int64_t warps = (int64_t)c->num_sms * kAsmWarps;
   ap.nrowtiles = (nrows + kAsmRows - 1) / kAsmRows;
   const int64_t batches = (c->n + 31) / 32;
-  int64_t nsplit = std::max<int64_t>(1, std::min<int64_t>(batches, (32 * warps + ap.nrowtiles - 1) / ap.nrowtiles));
+  int64_t nsplit = std::max<int64_t>(1, std::min<int64_t>(batches, (16 * warps + ap.nrowtiles - 1) / ap.nrowtiles));
   ap.cols_per_split = ((batches + nsplit - 1) / nsplit) * 32;
   nsplit = (c->n + ap.cols_per_split - 1) / ap.cols_per_split;
   ap.nitems = ap.nrowtiles * nsplit;

@@ -134,6 +134,14 @@ __device__ __forceinline__ double warp_max(double v) {
   for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(kFullMask, v, o));
   return v;
 }
+// FP32 min / max over the warp with one REDUX each (order-preserving map to unsigned; no NaN expected)
+__device__ __forceinline__ unsigned ordered_u32(float x) {
+  const unsigned b = __float_as_uint(x);
+  return (b >> 31) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float from_ordered_u32(unsigned u) { return __uint_as_float((u >> 31) ? (u & 0x7fffffffu) : ~u); }
+__device__ __forceinline__ float warp_min_f32(float v) { return from_ordered_u32(__reduce_min_sync(kFullMask, ordered_u32(v))); }
+__device__ __forceinline__ float warp_max_f32(float v) { return from_ordered_u32(__reduce_max_sync(kFullMask, ordered_u32(v))); }
 __device__ __forceinline__ int warp_excl_scan(int v, int lane, int* total) {
   int x = v;
 #pragma unroll

@@ -4,21 +4,23 @@
 // analytic integral below the first limit (self term: D = 0).
 //
 // Same execution model as the evaluation kernels (kernels_eval.cuh): persistent CTAs, every warp
-// pulls items from an atomic queue (16 warps per SM here).  One item = (tile of 64 rows) x (split of
-// the columns).  A lane owns rows i0 + lane and i0 + 32 + lane (their centroids sit in registers).
-// Columns are taken 32 at a time: lane l classifies column j0+l against the bounding sphere of the
-// row centroids, so the rule of a column is warp-uniform unless the tile straddles a band limit
-// (then: the more accurate rule, or the exact per-pair choice with masks).  The point records of the
-// batch's columns are streamed through the warp's double-buffered shared-memory window by bulk TMA,
-// whole elements per stage, with a small segment table (column, first point, number of points)
-// beside each stage.
+// pulls items from an atomic queue (12 warps per SM).  One item = (tile of 128 rows) x (split of the
+// columns).  A lane owns rows i0 + r * 32 + lane, r < 4 (their centroids sit in registers); the 32 rows
+// of one r are a "row group".  Columns are taken 32 at a time: lane l classifies column j0 + l against
+// the bounding sphere of the tile's centroids.  Where the whole tile falls into one distance-ratio band
+// the column has one rule; where it straddles a limit, the lane classifies the column against the sphere
+// of each row group, and the column is streamed once per rule its groups ask for, each copy applied to
+// those groups' rows only (or, without allow_upgrade, the column takes the exact per-pair choice with
+// masks).  The point records of the batch's columns are streamed through the warp's double-buffered
+// shared-memory window by bulk TMA, whole elements per stage, with a small segment table (column, row
+// groups, first point, number of points) beside each stage.
 //
 // The kernel is bound by the issue port, so everything around the 12 FP64
 // instructions of an interaction is kept short:
 //  * the elements are expanded with k folded into the charges and padded with zero charges to a
 //    multiple of kAsmU points, so a column is whole trips of kAsmU points and its sum needs neither a
 //    remainder loop nor a final scaling;
-//  * results of 8 consecutive columns go through a 64 x 8 shared-memory tile and leave as 64-byte row
+//  * results of 8 consecutive columns go through a 128 x 8 shared-memory tile and leave as 64-byte row
 //    segments, each lane storing its own rows with four 16-byte stores;
 //  * entries below the analytic limit are not evaluated where they are met (a warp-wide call for a
 //    handful of rows): their (row, column) pairs are queued in shared memory and evaluated 32 at a
@@ -61,7 +63,8 @@ constexpr int64_t kAsmMaxN = (int64_t)1 << 25;  // ... hence this many elements 
 struct AsmWarpSmem {
   double4 win[kStages][kBuf];
   double tile[kGroupCols * kAsmRows];  // [column of the group][row]: conflict-free both ways
-  uint32_t seg[kStages][32];  // col | npts << 8 | first << 16
+  uint32_t seg[kStages][32];  // col | row-group mask << 5 | npts << 9 | first << 16
+  double sub[kAsmR][4];       // bounding spheres of the tile's 32-row groups (centre, radius)
   uint32_t aq[kAqCap];
   uint64_t bar[kStages];
   unsigned long long n_inter, n_ana;
@@ -105,6 +108,52 @@ __device__ __forceinline__ void phi_segment(const double4* __restrict__ pts, int
   }
 }
 
+// The same for NR < 4 of the lane's rows (the rows of the row groups that take this rule; the other
+// groups of the column take another one, see the classification below), handed over in a compact copy.
+// Fewer rows per lane, more points per trip: 4 - 8 chains as well.  Only tiles of an upgrading policy
+// come here, so the per-pair results (allow_upgrade = 0), which promise not to depend on the tile, never do.
+template <int NR>
+__device__ __forceinline__ void phi_segment_rows(const double4* __restrict__ pts, int npts, const double (&qx)[NR],
+                                                 const double (&qy)[NR], const double (&qz)[NR], double (&acc)[NR], double c375) {
+  constexpr int U = NR >= 3 ? 2 : 4;  // npts is a multiple of kAsmU = 2: a U = 4 loop may leave one pair
+  static_assert(kAsmU == 2, "phi_segment_rows takes pairs of points");
+  double part[U][NR];
+#pragma unroll
+  for (int u = 0; u < U; ++u)
+#pragma unroll
+    for (int r = 0; r < NR; ++r) part[u][r] = 0.0;
+  int i = 0;
+#pragma unroll 1
+  for (; i + U <= npts; i += U) {
+    double4 s[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) s[u] = pts[i + u];
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+      for (int r = 0; r < NR; ++r) part[u][r] = phi_one(s[u], s[u].w, qx[r], qy[r], qz[r], part[u][r], c375);
+  }
+  if (U == 4 && i < npts) {
+    const double4 s0 = pts[i], s1 = pts[i + 1];
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+      part[0][r] = phi_one(s0, s0.w, qx[r], qy[r], qz[r], part[0][r], c375);
+      part[1][r] = phi_one(s1, s1.w, qx[r], qy[r], qz[r], part[1][r], c375);
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    if constexpr (U == 4) acc[r] = (part[0][r] + part[1][r]) + (part[2][r] + part[3][r]);
+    else acc[r] = part[0][r] + part[1][r];
+  }
+}
+// row `i` of the lane's four (a warp-uniform index)
+__device__ __forceinline__ double pick_row(const double (&v)[kAsmR], int i) {
+  static_assert(kAsmR == 4, "pick_row: four rows per lane");
+  const double lo = (i & 1) ? v[1] : v[0], hi = (i & 1) ? v[3] : v[2];
+  return (i & 2) ? hi : lo;
+}
+
 __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_constant__ AssembleParams p) {
   static_assert(kAsmU == 4 || kAsmU == 2 || kAsmU == 1, "phi_segment's sum tree");
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -128,8 +177,14 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
   clk.begin();
 
   for (;;) {
-    const int64_t item = next_item(p.queue, lane);
-    if (item >= p.nitems) break;
+    // The queue is run through twice.  The first pass takes the expensive column batches of an item
+    // (near the tile: 19 points and more per column, analytic entries, several rules per column), the
+    // second pass the cheap rest, so the launch ends on items of equal, small cost: its tail (the warps
+    // that find the queue empty while others still work) is half a cheap item instead of half an expensive one.
+    int64_t item = next_item(p.queue, lane);
+    if (item >= 2 * p.nitems) break;
+    const bool second_pass = item >= p.nitems;
+    if (second_pass) item -= p.nitems;
     const int64_t split = item / p.nrowtiles, rt = item - split * p.nrowtiles;
     const int64_t r0 = rt * kAsmRows;  // first row of the tile, relative to row0
     const int nrow_here = (int)min((int64_t)kAsmRows, p.nrows - r0);
@@ -143,23 +198,39 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
       const double4 ci = p.cenL[p.row0 + r0 + min(r * 32 + lane, nrow_here - 1)];
       px[r] = ci.x; py[r] = ci.y; pz[r] = ci.z;
     }
-    double lox = px[0], hix = px[0], loy = py[0], hiy = py[0], loz = pz[0], hiz = pz[0];
+    // Bounding spheres of every 32-row group (rows r * 32 + lane: consecutive elements, a compact patch of
+    // a spatially ordered mesh; kept in shared memory) and of the whole tile.  The boxes are taken in FP32
+    // (one REDUX per bound): any centre will do as long as the radius about it is not under-estimated, so
+    // the radius is the FP64 distance of the farthest centroid, rounded up on its way through FP32.
+    float lox = CUDART_INF_F, hix = -CUDART_INF_F, loy = CUDART_INF_F, hiy = -CUDART_INF_F, loz = CUDART_INF_F, hiz = -CUDART_INF_F;
+    __syncwarp();
 #pragma unroll
-    for (int r = 1; r < kAsmR; ++r) {
-      lox = fmin(lox, px[r]); hix = fmax(hix, px[r]);
-      loy = fmin(loy, py[r]); hiy = fmax(hiy, py[r]);
-      loz = fmin(loz, pz[r]); hiz = fmax(hiz, pz[r]);
+    for (int r = 0; r < kAsmR; ++r) {
+      const float fx = (float)px[r], fy = (float)py[r], fz = (float)pz[r];
+      const float ax = warp_min_f32(fx), bx = warp_max_f32(fx), ay = warp_min_f32(fy), by = warp_max_f32(fy);
+      const float az = warp_min_f32(fz), bz = warp_max_f32(fz);
+      const double sx = 0.5 * ((double)ax + (double)bx), sy = 0.5 * ((double)ay + (double)by), sz = 0.5 * ((double)az + (double)bz);
+      const double s2 = (px[r] - sx) * (px[r] - sx) + (py[r] - sy) * (py[r] - sy) + (pz[r] - sz) * (pz[r] - sz);
+      const float srho = __fsqrt_ru(warp_max_f32(__double2float_ru(s2)));
+      if (lane == 0) {
+        sm.sub[r][0] = sx; sm.sub[r][1] = sy; sm.sub[r][2] = sz; sm.sub[r][3] = (double)srho;
+      }
+      lox = fminf(lox, ax); hix = fmaxf(hix, bx);
+      loy = fminf(loy, ay); hiy = fmaxf(hiy, by);
+      loz = fminf(loz, az); hiz = fmaxf(hiz, bz);
     }
-    lox = warp_min(lox); hix = warp_max(hix);
-    loy = warp_min(loy); hiy = warp_max(hiy);
-    loz = warp_min(loz); hiz = warp_max(hiz);
-    const double cx = 0.5 * (lox + hix), cy = 0.5 * (loy + hiy), cz = 0.5 * (loz + hiz);
+    __syncwarp();
+    const double cx = 0.5 * ((double)lox + (double)hix), cy = 0.5 * ((double)loy + (double)hiy), cz = 0.5 * ((double)loz + (double)hiz);
     double d2 = 0.0;
 #pragma unroll
     for (int r = 0; r < kAsmR; ++r)
       d2 = fmax(d2, (px[r] - cx) * (px[r] - cx) + (py[r] - cy) * (py[r] - cy) + (pz[r] - cz) * (pz[r] - cz));
-    const double rho = sqrt(warp_max(d2));
+    const double rho = (double)__fsqrt_ru(warp_max_f32(__double2float_ru(d2)));
     const double mag = fmax(fmax(fabs(cx), fabs(cy)), fabs(cz)) + rho;
+    // valid rows of each group, one byte per group (for the interaction tally)
+    uint32_t vrows = 0;
+#pragma unroll
+    for (int r = 0; r < kAsmR; ++r) vrows |= (uint32_t)max(0, min(32, nrow_here - 32 * r)) << (8 * r);
 
     // analytic pair queue of this item: [aq_head, aq_tail) in the ring sm.aq
     int aq_head = 0, aq_tail = 0;
@@ -188,59 +259,115 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
       const int ncol = (int)min((int64_t)32, col_end - j0);
       // ---- classify column j0 + lane against the row tile's bounding sphere
       const int64_t e = j0 + lane;
-      int cnt = 0, lvl = -1;  // cnt: the column's points in the stream, zero-charge padding included
-      int real = 0;           // ... and without it
-      bool is_ana = false, is_mixed = false, is_fix = false;
+      // lm: which row groups take which cubature level, 4 bits per level (bit 4 L + r: group r, level L).
+      // A column the whole tile sees in one band has one level with all four groups; where the tile
+      // straddles a band limit (and the policy allows upgrades) every 32-row group is classified by its own
+      // sphere, so the more accurate rule is paid by the groups that need it only.
+      uint32_t lm = 0;
+      int cnt = 0, lvl = -1;  // cnt: the column's points in the stream (all its levels), zero-charge padding included
+      int real = 0;           // point-charge interactions of the column with the valid rows, without the padding
+      int nseg = 0;           // levels of the column = its segments in the stream
+      bool has_ana = false, is_mixed = false;
       const double4* src = nullptr;
+      int t = 0;
       if (lane < ncol) {
         const double4 c = p.cenL[e];
-        const int t = p.type[e];
+        t = p.type[e];
+        const double cmag = fmax(fmax(fabs(c.x), fabs(c.y)), fabs(c.z));
         const double dx = cx - c.x, dy = cy - c.y, dz = cz - c.z;
         const double Dc = sqrt(dx * dx + dy * dy + dz * dz);
-        const double slack = 1e-9 * (Dc + rho) + 1e-12 * (mag + fmax(fmax(fabs(c.x), fabs(c.y)), fabs(c.z)));
+        const double slack = 1e-9 * (Dc + rho) + 1e-12 * (mag + cmag);
         const double Dhi = Dc + rho + slack, Dlo = fmax(Dc - rho - slack, 0.0);
         const int lfar = p.pol.map[want_level(Dhi * Dhi, c.w, p.pol.dr[t])];
         const int lnear = p.pol.map[want_level(Dlo * Dlo, c.w, p.pol.dr[t])];
-        // the analytic formula is never an "upgrade" (see eval_adaptive_kernel): a tile straddling
-        // the analytic limit keeps the exact per-pair choice
-        if (lnear != lfar && lnear == 5 && p.pol.allow_upgrade && p.pol.map[4] != 5) {
-          // tile straddles the analytic limit: the column is streamed with the most accurate
-          // cubature rule, and the rows below the limit are overwritten analytically afterwards
-          is_fix = true;
-          lvl = p.pol.map[4];
-        } else if (lnear != lfar && (!p.pol.allow_upgrade || lnear == 5)) {
-          is_mixed = true;
+        if (lnear == lfar) {
+          if (lnear == 5) has_ana = true;  // every row below the analytic limit: nothing streamed
+          else lm = 0xfu << (4 * lnear);
+        } else if (!p.pol.allow_upgrade) {
+          is_mixed = true;  // exact per-pair choice
         } else {
-          lvl = lnear;
-          is_ana = lvl == 5;
+          // The analytic formula is never an "upgrade" (see eval_adaptive_kernel).  A group that
+          // straddles the analytic limit is streamed with the most accurate cubature rule and its
+          // rows below the limit are overwritten analytically afterwards; a group entirely below the
+          // limit is not streamed at all.
+#pragma unroll 1
+          for (int r = 0; r < kAsmR; ++r) {
+            const double sx = sm.sub[r][0] - c.x, sy = sm.sub[r][1] - c.y, sz = sm.sub[r][2] - c.z, srho = sm.sub[r][3];
+            const double Ds = sqrt(sx * sx + sy * sy + sz * sz);
+            const double sl = 1e-9 * (Ds + srho) + 1e-12 * (mag + cmag);
+            const double Shi = Ds + srho + sl, Slo = fmax(Ds - srho - sl, 0.0);
+            const int gfar = p.pol.map[want_level(Shi * Shi, c.w, p.pol.dr[t])];
+            const int gnear = p.pol.map[want_level(Slo * Slo, c.w, p.pol.dr[t])];
+            if (gnear == 5) {
+              has_ana = true;
+              if (gfar != 5) {
+                if (p.pol.map[4] == 5) is_mixed = true;  // no cubature level to fall back on
+                else lm |= 1u << (4 * p.pol.map[4] + r);
+              }
+            } else {
+              lm |= 1u << (4 * gnear + r);
+            }
+          }
+          if (is_mixed) {
+            lm = 0;
+            has_ana = false;
+          }
         }
-        if (lvl >= 0 && lvl < 5) {
-          real = rule_npts(t, lvl);
-          cnt = (real + kAsmU - 1) / kAsmU * kAsmU;
-          src = p.lvl_pts[lvl] + e * p.stride[lvl];
+#pragma unroll
+        for (int L = 0; L < 5; ++L) {
+          const uint32_t g = (lm >> (4 * L)) & 15u;
+          if (g) {
+            const int N = rule_npts(t, L);
+            cnt += (N + kAsmU - 1) / kAsmU * kAsmU;
+            real += N * (int)__dp4a(vrows, ((g & 1u) | ((g & 2u) << 7) | ((g & 4u) << 14) | ((g & 8u) << 21)), 0u);
+            lvl = nseg ? -2 : L;  // -2: several levels, its copies are never merged with a neighbour's
+            src = p.lvl_pts[L] + e * p.stride[L];
+            ++nseg;
+          }
         }
       }
-      // point-charge interactions of the batch's streamed columns (padding not counted)
+      const bool costly = __any_sync(kFullMask, lvl >= 3 || lvl == -2 || has_ana || is_mixed);
+      if (costly == second_pass) continue;
+      // point-charge interactions of the batch's streamed columns (padding and clamped rows not counted)
       const int real_pts = warp_sum(real);
-      if (lane == 0) sm.n_inter += (unsigned long long)real_pts * nrow_here;
-      int total;
+      if (lane == 0) sm.n_inter += (unsigned long long)real_pts;
+      int total, ktotal;
       const int pre = warp_excl_scan(cnt, lane, &total);
+      const int kpre = warp_excl_scan(nseg, lane, &ktotal);
       int cursor = 0;
 
       // Fills `stage` with the next whole elements of the batch; returns how many (0 = batch done).
       auto fill = [&](int stage) -> int {
         for (;;) {
           if (cursor >= 32) return 0;
+          const int kbase = __shfl_sync(kFullMask, kpre, cursor);
           const StagePlan sp = plan_stage(cursor, lane, cnt, pre, total, lvl, p.stride);
           cursor = sp.next;
           if (sp.nstage == 0) continue;
-          if (sp.inc) sm.seg[stage][__popc(sp.incmask & lt_mask)] = (uint32_t)lane | ((uint32_t)cnt << 8) | ((uint32_t)(pre - sp.base) << 16);
+          const int kend = __shfl_sync(kFullMask, kpre, sp.next & 31);
+          const uint32_t dst = win0 + (uint32_t)((stage * kBuf + (pre - sp.base)) * sizeof(double4));
           if (lane == 0) mbar_arrive_expect_tx(bar0 + 8 * stage, (uint32_t)(sp.nstage * sizeof(double4)));
+          if (sp.inc && lvl >= 0)
+            sm.seg[stage][kpre - kbase] = (uint32_t)lane | (((lm >> (4 * lvl)) & 15u) << 5) | ((uint32_t)cnt << 9) | ((uint32_t)(pre - sp.base) << 16);
           __syncwarp();
-          if (sp.head)
-            tma_load_1d(win0 + (uint32_t)((stage * kBuf + (pre - sp.base)) * sizeof(double4)), src,
-                        (uint32_t)((sp.run_end - pre) * sizeof(double4)), bar0 + 8 * stage);
-          return __popc(sp.incmask);
+          if (sp.inc) {
+            if (lvl >= 0) {  // one level: consecutive columns share a copy
+              if (sp.head) tma_load_1d(dst, src, (uint32_t)((sp.run_end - pre) * sizeof(double4)), bar0 + 8 * stage);
+            } else {  // one segment and one copy per level, the most accurate first
+              int k = kpre - kbase, off = 0;
+              for (int L = 4; L >= 0; --L) {
+                const uint32_t g = (lm >> (4 * L)) & 15u;
+                if (!g) continue;
+                const int np = (rule_npts(t, L) + kAsmU - 1) / kAsmU * kAsmU;
+                sm.seg[stage][k++] = (uint32_t)lane | (g << 5) | ((uint32_t)np << 9) | ((uint32_t)(pre - sp.base + off) << 16);
+                tma_load_1d(dst + (uint32_t)(off * sizeof(double4)), p.lvl_pts[L] + e * p.stride[L], (uint32_t)(np * sizeof(double4)),
+                            bar0 + 8 * stage);
+                off += np;
+              }
+            }
+          }
+          __syncwarp();  // the segment table is complete before any lane reads it
+          return (sp.next < 32 ? kend : ktotal) - kbase;
         }
       };
       // output group (8 consecutive columns) being collected in sm.tile, and which of its columns
@@ -285,18 +412,49 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
             cur_group = col >> 3;
             gmask = 0;
           }
-          double acc[kAsmR];
-          phi_segment(&sm.win[stage][d >> 16], (int)((d >> 8) & 255u), px, py, pz, acc, c375);
+          const double4* pts = &sm.win[stage][d >> 16];
+          const int npts = (int)((d >> 9) & 127u);
+          __builtin_assume(npts >= kAsmU);  // a segment is never empty
+          const uint32_t g = (d >> 5) & 15u;
+          double* trow = &sm.tile[(col & (kGroupCols - 1)) * kAsmRows + lane];
+          if (g == 15u) {
+            double acc[kAsmR];
+            phi_segment(pts, npts, px, py, pz, acc, c375);
 #pragma unroll
-          for (int r = 0; r < kAsmR; ++r) sm.tile[(col & (kGroupCols - 1)) * kAsmRows + r * 32 + lane] = acc[r];
+            for (int r = 0; r < kAsmR; ++r) trow[r * 32] = acc[r];
+          } else if (__popc(g) == 3) {  // all rows but one
+            const int skip = __ffs(~g) - 1;
+            double qx[3], qy[3], qz[3], acc[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+              qx[i] = i < skip ? px[i] : px[i + 1];
+              qy[i] = i < skip ? py[i] : py[i + 1];
+              qz[i] = i < skip ? pz[i] : pz[i + 1];
+            }
+            phi_segment_rows<3>(pts, npts, qx, qy, qz, acc, c375);
+#pragma unroll
+            for (int i = 0; i < 3; ++i) trow[(i < skip ? i : i + 1) * 32] = acc[i];
+          } else if (__popc(g) == 2) {
+            const int i0 = __ffs(g) - 1, i1 = 31 - __clz(g);
+            const double qx[2] = {pick_row(px, i0), pick_row(px, i1)}, qy[2] = {pick_row(py, i0), pick_row(py, i1)};
+            const double qz[2] = {pick_row(pz, i0), pick_row(pz, i1)};
+            double acc[2];
+            phi_segment_rows<2>(pts, npts, qx, qy, qz, acc, c375);
+            trow[i0 * 32] = acc[0];
+            trow[i1 * 32] = acc[1];
+          } else {
+            const int i0 = __ffs(g) - 1;
+            const double qx[1] = {pick_row(px, i0)}, qy[1] = {pick_row(py, i0)}, qz[1] = {pick_row(pz, i0)};
+            double acc[1];
+            phi_segment_rows<1>(pts, npts, qx, qy, qz, acc, c375);
+            trow[i0 * 32] = acc[0];
+          }
           gmask |= 1u << (col & (kGroupCols - 1));
         }
         __syncwarp();
       };
 
-      int na = fill(0);
-      int nb = na ? fill(1) : 0;
-      // while the first copies fly: the rare columns that need the exact per-pair choice, stored directly
+      // the columns that need the exact per-pair choice (none under an upgrading policy), stored directly
       unsigned xmask = __ballot_sync(kFullMask, is_mixed);
       while (xmask) {
         const int l = __ffs(xmask) - 1;
@@ -354,21 +512,21 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
         for (int r = 0; r < kAsmR; ++r)
           if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j] = val[r];
       }
-      // ---- streamed columns
-      for (;;) {
-        if (!na) break;
-        consume_stage(0, na);
-        na = fill(0);
-        if (!nb) break;
-        consume_stage(1, nb);
-        nb = fill(1);
+      // ---- streamed columns: fill the other stage, then consume this one (one call site each: the
+      // kernel has to fit the instruction cache)
+      for (int stage = 1, cur = 0;;) {
+        const int nxt = fill(stage ^ 1);
+        if (cur > 0) consume_stage(stage, cur);
+        if (nxt == 0) break;
+        stage ^= 1;
+        cur = nxt;
       }
       flush_group();
-      // ---- entries below the analytic limit: every row of a column the whole tile sees that near,
-      // and - by the exact per-pair test - the rows of the straddling columns streamed above (their
-      // cubature values are overwritten: flush_group has synchronised the warp).  Queued, then
+      // ---- entries below the analytic limit: every row of a column the whole tile (or a row group) sees
+      // that near, and - by the exact per-pair test - the rows of the straddling groups streamed above
+      // (their cubature values are overwritten: flush_group has synchronised the warp).  Queued, then
       // evaluated one pair per lane.
-      unsigned qmask = __ballot_sync(kFullMask, is_ana || is_fix);
+      unsigned qmask = __ballot_sync(kFullMask, has_ana);
       while (qmask) {
         const int l = __ffs(qmask) - 1;
         qmask &= qmask - 1;

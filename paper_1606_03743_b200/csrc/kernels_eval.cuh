@@ -294,7 +294,7 @@ __device__ __forceinline__ StagePlan plan_stage(int cursor, int lane, int cnt, i
   const int prev_cnt = __shfl_up_sync(kFullMask, cnt, 1);
   const int prev_lvl = __shfl_up_sync(kFullMask, lvl, 1);
   // a lane continues its predecessor's copy if that one ends exactly where this one starts
-  const bool cont = s.inc && lane > cursor && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == stride[lvl < 0 ? 0 : lvl];
+  const bool cont = s.inc && lane > cursor && lvl >= 0 && prev_cnt > 0 && prev_lvl == lvl && prev_cnt == stride[lvl];
   s.incmask = __ballot_sync(kFullMask, s.inc);
   s.head = s.inc && !cont;
   const unsigned heads = __ballot_sync(kFullMask, s.head);
