@@ -64,6 +64,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="default workload only: skip the secondary block")
+    ap.add_argument("--store-matrix", action="store_true",
+                    help="--workload solve: let the solve keep the matrix (bemcub_solve_storage): one matrix fill, GEMV mat-vecs")
     ap.add_argument("--out", default=None, help="--workload accuracy: text file for the tables")
     return ap.parse_args()
 
@@ -468,6 +470,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         pol = b.bemcub_default_policy(False)
         d_V = torch.ones(n, dtype=torch.float64, device=dev)
         d_s = torch.zeros(n, dtype=torch.float64, device=dev)
+        if args.store_matrix:
+            b.bemcub_solve_storage(h, 8 * n * n)
+            c["desc"] = c["desc"].replace("matrix-free BEM solve", "BEM solve with the matrix kept in HBM (bemcub_solve_storage)") \
+                                 .replace("every mat-vec = potential-only adaptive evaluation at the centroids",
+                                          "one matrix fill, every mat-vec = bemcub_matvec")
 
         def step():
             d_s.zero_()
@@ -506,6 +513,34 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         areas = 0.5 * np.linalg.norm(np.cross(c["verts"][:, 1] - c["verts"][:, 0], c["verts"][:, 2] - c["verts"][:, 0]), axis=1)
         q_tot = float((d_s.cpu().numpy() * areas).sum())
         solve_info["capacitance_over_4pi_eps0_R"] = q_tot / (4 * np.pi * 8.8541878128e-12)
+        if args.store_matrix:
+            # the mat-vec of this mode on its own: HBM-bound, 8 n^2 bytes per call against the measured copy rate
+            b.bemcub_solve_storage(h, 0)
+            A = torch.empty((n, n), dtype=torch.float64, device=dev)
+            y = torch.empty(n, dtype=torch.float64, device=dev)
+            b.bemcub_assemble(h, pol, A, n)
+            for _ in range(3):
+                b.bemcub_matvec(h, A, n, d_s, y)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(dev)
+            e0.record()
+            for _ in range(50):
+                b.bemcub_matvec(h, A, n, d_s, y)
+            e1.record()
+            torch.cuda.synchronize(dev)
+            g_ms = e0.elapsed_time(e1) / 50
+            hbm = None
+            try:
+                hbm = float(json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "MEASURED_PEAKS.json")))["hbm_gbs"])
+            except Exception:
+                pass
+            peak_gbs = hbm if hbm else 6500.0
+            solve_info["matvec_roofline"] = {
+                "bound": "hbm", "kernel": "gemv_rows_kernel", "ms": g_ms, "achieved": 8.0 * n * n / (g_ms * 1e-3) / 1e9,
+                "peak": peak_gbs, "unit": "GB/s", "frac": 8.0 * n * n / (g_ms * 1e-3) / 1e9 / peak_gbs,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy: read + write)" if hbm else "fallback 6500 GB/s (B200_PROFILING.md)",
+                "bytes_per_call": 8.0 * n * n, "l2": "matrix (3.36 GB) larger than L2"}
+            del A
     value = units_per_step * world / (ms_max * 1e-3)
 
     # dominant kernel against the FP64-ALU roofline
@@ -524,7 +559,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         inter_own = float(b.bemcub_get_stats(h)["point_interactions"])
     elif not is_matrix and not adaptive:
         inter_own = inter
-    kernel = ("eval_adaptive_kernel<kModePhi>" if is_solve else "assemble_kernel" if is_matrix else
+    kernel = ("assemble_kernel" if (is_solve and args.store_matrix) else "eval_adaptive_kernel<kModePhi>" if is_solve else
+              "assemble_kernel" if is_matrix else
               ("eval_adaptive_kernel" if adaptive else "eval_fixed_kernel"))
     if precision == b.F32:
         roof = {"bound": "alu", "achieved": inter * fpi / (k_ms * 1e-3) / 1e12, "peak": None, "unit": "TFLOP/s", "frac": None,
@@ -621,7 +657,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             line["metric"] = "FP64 potential-only element.point interactions/s inside bemcub_solve"
             line["unit"] = "element.point interactions/s"
             line["solve"] = solve_info
-            line["roofline"]["note"] = "kernel_ms / interactions are those of the LAST mat-vec of the solve"
+            line["roofline"]["note"] = ("kernel_ms / interactions are those of the solve's one matrix fill; the mat-vecs are "
+                                        "solve.matvec_roofline (HBM-bound); value counts every mat-vec as n^2 element.point pairs"
+                                        if args.store_matrix else
+                                        "kernel_ms / interactions are those of the LAST mat-vec of the solve")
         print(json.dumps(line), flush=True)
     if r is not None:
         r.close()

@@ -207,6 +207,12 @@ int bemcub_assemble(bemcub_ctx* ctx, const bemcub_policy* host_policy, double* o
 int bemcub_assemble_rows(bemcub_ctx* ctx, const bemcub_policy* host_policy, int64_t row0, int64_t nrows,
                          double* out_rows, int64_t ld);
 
+/* y[i] = sum_j matrix[i*ld + j] x[j], i, j < n: the product of a matrix filled by bemcub_assemble (or any
+ * other n x n row-major FP64 matrix, ld >= n) with a vector - the potentials at the centroids for the
+ * charge densities x (L34).  Bound by the HBM read of the matrix.  x and y must not overlap.  The sum of
+ * a row is formed in a fixed order: results are reproducible.  Asynchronous. */
+int bemcub_matvec(bemcub_ctx* ctx, const double* matrix, int64_t ld, const double* x, double* y);
+
 /* Matrix-free solve of the collocation system (L34; "shell matrices ... not stored", L200):
  *     sum_j A_ij sigma_j = rhs_potential[i],  A as bemcub_assemble defines it (never formed),
  * by right-preconditioned (diagonal = analytic self terms) restarted GMRES(30); every mat-vec is
@@ -219,6 +225,15 @@ int bemcub_assemble_rows(bemcub_ctx* ctx, const bemcub_policy* host_policy, int6
  * Synchronous.  The policy's allow_upgrade changes the operator only at the rules' truncation level. */
 int bemcub_solve(bemcub_ctx* ctx, const bemcub_policy* host_policy, const double* rhs_potential, double* sigma,
                  double rel_tol, int max_matvecs, int* host_matvecs, double* host_rel_residual);
+
+/* Lets bemcub_solve keep the matrix.  The paper's solver does not store it (L200) because its
+ * meshes do not fit (1.5e6 elements: 18 TB); a B200 holds n up to about 1.4e5 (8 n^2 bytes of its 180 GB).
+ * With max_matrix_bytes >= 8 n^2 a solve first fills the n x n matrix (as bemcub_assemble, under the
+ * solve's policy) into ctx-owned memory - BEMCUB_ERR_NOMEM if that allocation fails - and every
+ * mat-vec is a matrix-vector product read from HBM; larger meshes, and every mesh after
+ * max_matrix_bytes = 0 (the default; it also frees the matrix), are solved matrix-free.  The two
+ * operators differ at the rounding level of the entries only (same rules, same limits). */
+int bemcub_solve_storage(bemcub_ctx* ctx, int64_t max_matrix_bytes);
 
 /* Same as bemcub_set_elements / bemcub_eval with HOST buffers: copies the inputs to ctx-owned
  * device memory, runs, copies phi / E back and synchronises (the end-to-end path bench.py times). */

@@ -63,6 +63,8 @@ def _load() -> C.CDLL:
         "bemcub_eval_pairs": [vp, i64, vp, vp, vp, C.c_int, PP, vp, vp, vp, C.c_int],
         "bemcub_eval_linear": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
         "bemcub_solve": [vp, PP, vp, vp, dbl, C.c_int, C.POINTER(C.c_int), C.POINTER(dbl)],
+        "bemcub_solve_storage": [vp, i64],
+        "bemcub_matvec": [vp, vp, i64, vp, vp],
         "bemcub_assemble": [vp, PP, vp, i64],
         "bemcub_assemble_rows": [vp, PP, i64, i64, vp, i64],
         "bemcub_set_elements_host": [vp, i64, vp, vp],
@@ -90,7 +92,7 @@ def _load() -> C.CDLL:
 
 _lib = _load()
 EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval",
-            "bemcub_eval_gradient", "bemcub_eval_linear", "bemcub_eval_pairs", "bemcub_solve",
+            "bemcub_eval_gradient", "bemcub_eval_linear", "bemcub_eval_pairs", "bemcub_solve", "bemcub_solve_storage", "bemcub_matvec",
             "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
             "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
             "bemcub_fp64_peak", "bemcub_fp64_issue_sweep", "bemcub_inner_loop_rate", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
@@ -210,6 +212,14 @@ def bemcub_solve(ctx, policy, rhs_potential, sigma, rel_tol: float, max_matvecs:
     if rc not in (0, ERR_NOT_CONVERGED):
         _check(rc, "bemcub_solve")
     return mv.value, res.value, rc == 0
+
+
+def bemcub_matvec(ctx, matrix, ld: int, x, y) -> None:
+    _check(_lib.bemcub_matvec(ctx, _dptr(matrix), ld, _dptr(x), _dptr(y)), "bemcub_matvec")
+
+
+def bemcub_solve_storage(ctx, max_matrix_bytes: int) -> None:
+    _check(_lib.bemcub_solve_storage(ctx, max_matrix_bytes), "bemcub_solve_storage")
 
 
 def bemcub_assemble(ctx, policy, out_matrix, ld: int) -> None:

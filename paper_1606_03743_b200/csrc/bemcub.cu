@@ -60,6 +60,8 @@ struct bemcub_ctx {
   const double* sort_src = nullptr;
   int64_t sort_m = 0;
   DevBuf solve_buf[6];  // GMRES: centroids, diagonal, basis, w, z/residual, small coefficient block
+  DevBuf solve_matrix;   // the collocation matrix of a solve that keeps it (bemcub_solve_storage)
+  int64_t solve_matrix_limit = 0;  // bytes; 0 = every solve is matrix-free
   DevBuf host_stage[5];  // device copies of host inputs/outputs for the *_host entry points
   unsigned long long* d_counters = nullptr;
   bemcub_stats stats{};
@@ -472,6 +474,7 @@ int bemcub_destroy(bemcub_ctx* c) {
   for (int i = 0; i < 2; ++i) { release(c->sort_key[i]); release(c->sort_idx[i]); }
   release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
   for (int i = 0; i < 6; ++i) release(c->solve_buf[i]);
+  release(c->solve_matrix);
   if (c->d_status) cudaFree(c->d_status);
   if (c->d_counters) cudaFree(c->d_counters);
   for (int i = 0; i < 4; ++i)

@@ -1,6 +1,8 @@
 // Host loop of bemcub_solve (included by bemcub.cu): right-preconditioned restarted GMRES around
 // the potential-only evaluation kernel.  SURVEY.md §8(f).2; PAPER.md L34 (the BEM system for the
 // unknown charge densities), L200 (matrix elements computed on the fly, matrix not stored).
+// Where the caller allows it and 8 n^2 bytes fit (bemcub_solve_storage; 180 GB of HBM hold n = 1.4e5),
+// the matrix is filled once by the matrix-fill kernel and every mat-vec is an HBM-bound GEMV.
 namespace {
 
 constexpr int kGmresRestart = 30;
@@ -12,12 +14,14 @@ struct SolveWork {
   double* w;      // [n]
   double* z;      // [n]
   double* coef;   // [3 * (restart + 2)]: first and second Gram-Schmidt pass, then |w|^2; also y of the update
+  const double* matrix;  // [n][n] when the solve keeps it, else null
 };
 
 inline unsigned blocks_for(int64_t n) { return (unsigned)((n + 255) / 256); }
 
 // out = A * x   (one adaptive potential-only evaluation at the centroids; the sort is reused)
 int solve_matvec(bemcub_ctx* c, const bemcub_policy* pol, const SolveWork& k, const double* x, double* out, bool first) {
+  if (k.matrix) return bemcub_matvec(c, k.matrix, c->n, x, out);
   return eval_common(c, x, BEMCUB_RULE_ADAPTIVE, pol, c->n, k.cen, out, nullptr, nullptr, BEMCUB_F64, !first);
 }
 
@@ -37,6 +41,31 @@ int to_host(bemcub_ctx* c, const double* dev, int count, double* host) {
 }
 
 }  // namespace
+
+extern "C" int bemcub_matvec(bemcub_ctx* c, const double* matrix, int64_t ld, const double* x, double* y) {
+  if (!c) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  const int64_t n = c->n;
+  if (n == 0) return BEMCUB_OK;
+  if (!matrix || !x || !y || ld < n || x == y) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  const int grid = (int)std::min<int64_t>(n, (int64_t)c->num_sms * kGemvCtasPerSm);
+  gemv_rows_kernel<<<grid, kGemvThreads, 0, c->stream>>>(n, matrix, ld, x, y);
+  count_launch(c);
+  CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
+
+extern "C" int bemcub_solve_storage(bemcub_ctx* c, int64_t max_matrix_bytes) {
+  if (!c || max_matrix_bytes < 0) return BEMCUB_ERR_INVALID_ARG;
+  c->solve_matrix_limit = max_matrix_bytes;
+  if (max_matrix_bytes == 0) {
+    DeviceGuard g(c->device);
+    cudaStreamSynchronize(c->stream);
+    release(c->solve_matrix);
+  }
+  return BEMCUB_OK;
+}
 
 extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, const double* rhs, double* sigma, double rel_tol,
                             int max_matvecs, int* host_matvecs, double* host_rel_residual) {
@@ -64,6 +93,12 @@ extern "C" int bemcub_solve(bemcub_ctx* c, const bemcub_policy* host_policy, con
   k.w = (double*)c->solve_buf[3].ptr;
   k.z = (double*)c->solve_buf[4].ptr;
   k.coef = (double*)c->solve_buf[5].ptr;
+  k.matrix = nullptr;
+  if (n <= ((int64_t)1 << 30) && (int64_t)sizeof(double) * n * n <= c->solve_matrix_limit) {
+    if ((rc = ensure(c->solve_matrix, sizeof(double) * (size_t)n * (size_t)n))) return rc;
+    if ((rc = bemcub_assemble_rows(c, host_policy, 0, n, (double*)c->solve_matrix.ptr, n))) return rc;
+    k.matrix = (const double*)c->solve_matrix.ptr;
+  }
   CUDA_TRY(cudaMemcpy2DAsync(k.cen, 24, c->cenL.ptr, 32, 24, (size_t)n, cudaMemcpyDeviceToDevice, c->stream));
   self_term_kernel<<<blocks_for(n), 256, 0, c->stream>>>(n, (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr,
                                                         (const double4*)c->cenL.ptr, coulomb_k(), k.diag);

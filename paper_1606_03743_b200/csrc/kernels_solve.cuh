@@ -83,4 +83,55 @@ __global__ void vec_add_scaled_kernel(int64_t n, const double* __restrict__ u, c
   if (i < n) x[i] += u[i] / d[i];
 }
 
+// out[i] = sum_j A[i * ld + j] x[j]: the mat-vec of a solve whose matrix is kept in device memory
+// (bemcub_solve_storage).  Bound by the HBM read of the 8 n^2 bytes of A: one CTA takes one row at a
+// time, every thread 16-byte streaming loads, four in flight; x comes from L1 / L2.  The sums are
+// combined in a fixed order (four per thread, warp shuffles, the warps in index order).
+constexpr int kGemvThreads = 256;
+constexpr int kGemvCtasPerSm = 8;
+__global__ void __launch_bounds__(kGemvThreads) gemv_rows_kernel(int64_t n, const double* __restrict__ A, int64_t ld,
+                                                                 const double* __restrict__ x, double* __restrict__ out) {
+  __shared__ double red[kGemvThreads / 32];
+  constexpr int T = kGemvThreads;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool vec = ((ld & 1) == 0) && ((reinterpret_cast<uintptr_t>(A) & 15u) == 0) && ((reinterpret_cast<uintptr_t>(x) & 15u) == 0);
+  for (int64_t i = blockIdx.x; i < n; i += gridDim.x) {
+    const double* row = A + i * ld;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    if (vec) {
+      const double2* r2 = reinterpret_cast<const double2*>(row);
+      const double2* x2 = reinterpret_cast<const double2*>(x);
+      const int64_t n2 = n >> 1;
+      int64_t j = threadIdx.x;
+      for (; j + 3 * T < n2; j += 4 * T) {
+        const double2 a0 = __ldcs(r2 + j), a1 = __ldcs(r2 + j + T), a2 = __ldcs(r2 + j + 2 * T), a3 = __ldcs(r2 + j + 3 * T);
+        const double2 b0 = x2[j], b1 = x2[j + T], b2 = x2[j + 2 * T], b3 = x2[j + 3 * T];
+        s0 = fma(a0.y, b0.y, fma(a0.x, b0.x, s0));
+        s1 = fma(a1.y, b1.y, fma(a1.x, b1.x, s1));
+        s2 = fma(a2.y, b2.y, fma(a2.x, b2.x, s2));
+        s3 = fma(a3.y, b3.y, fma(a3.x, b3.x, s3));
+      }
+      for (; j < n2; j += T) {
+        const double2 a0 = __ldcs(r2 + j), b0 = x2[j];
+        s0 = fma(a0.y, b0.y, fma(a0.x, b0.x, s0));
+      }
+      if ((n & 1) && threadIdx.x == 0) s1 = fma(row[n - 1], x[n - 1], s1);
+    } else {
+      for (int64_t j = threadIdx.x; j < n; j += T) s0 = fma(__ldcs(row + j), x[j], s0);
+    }
+    double s = (s0 + s1) + (s2 + s3);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(kFullMask, s, o);
+    if (lane == 0) red[warp] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double t = 0.0;
+#pragma unroll
+      for (int w = 0; w < T / 32; ++w) t += red[w];
+      out[i] = t;
+    }
+    __syncthreads();
+  }
+}
+
 }  // namespace bemcub
