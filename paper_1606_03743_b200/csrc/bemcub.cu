@@ -34,6 +34,7 @@ struct DevBuf {
 
 }  // namespace
 
+constexpr int kCounterSlots = 8 + (kFewMaxM * 4 + 7) / 8;  // tallies, work queue, clock | eval_few_kernel's done counters
 struct bemcub_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
@@ -456,7 +457,7 @@ int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream) {
   int rc = upload_tables();
   if (rc == BEMCUB_OK) rc = configure_kernels();
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_status, sizeof(GeomStatus)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
-  if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
+  if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, kCounterSlots * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
   if (rc != BEMCUB_OK) {
     bemcub_destroy(c);
     return rc;
@@ -620,6 +621,8 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   }
   const bool few = !grad && precision == BEMCUB_F64 && m <= kFewMaxM;
   if (few) {
+    // a pass takes 4 field points (2 or 1 if that is all there is: no work on clamped duplicates)
+    const int per_pass = m >= 3 ? kFewM : (int)m;
     const int blocks = c->num_sms * 2;
     if ((rc = ensure(c->partial, (size_t)blocks * (size_t)m * sizeof(double4)))) return rc;
     FewParams fw;
@@ -636,21 +639,29 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     fw.counters = c->d_counters;
     fw.area = (const double*)c->area.ptr;
     fw.sigma_v = sigma_v;
-    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+    fw.done = reinterpret_cast<unsigned*>(c->d_counters + 8);  // one per pass (<= kFewMaxM)
+    fw.k = coulomb_k();
+    fw.out_phi = out_phi;
+    fw.out_E = out_E;
+    CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, kCounterSlots * sizeof(unsigned long long), c->stream));
     mark(c, 1);
-    const dim3 grid((unsigned)blocks, (unsigned)((m + kFewM - 1) / kFewM));
+    const dim3 grid((unsigned)blocks, (unsigned)((m + per_pass - 1) / per_pass));
     // points on the fly from the vertices (measured faster than reading kept points: 121 instead of
     // 260 bytes per element; 0.119 vs 0.144 ms for one field point on 1e6 elements)
-    if (out_E) eval_few_kernel<kModePhiE><<<grid, kFewWarps * 32, 0, c->stream>>>(fw);
-    else eval_few_kernel<kModePhi><<<grid, kFewWarps * 32, 0, c->stream>>>(fw);
+    const int threads = kFewWarps * 32;
+    if (out_E) {
+      if (per_pass == 1) eval_few_kernel<kModePhiE, 1><<<grid, threads, 0, c->stream>>>(fw);
+      else if (per_pass == 2) eval_few_kernel<kModePhiE, 2><<<grid, threads, 0, c->stream>>>(fw);
+      else eval_few_kernel<kModePhiE, kFewM><<<grid, threads, 0, c->stream>>>(fw);
+    } else {
+      if (per_pass == 1) eval_few_kernel<kModePhi, 1><<<grid, threads, 0, c->stream>>>(fw);
+      else if (per_pass == 2) eval_few_kernel<kModePhi, 2><<<grid, threads, 0, c->stream>>>(fw);
+      else eval_few_kernel<kModePhi, kFewM><<<grid, threads, 0, c->stream>>>(fw);
+    }
     count_launch(c);
     CUDA_TRY(cudaGetLastError());
     mark(c, 2);
-    reduce_scale_kernel<<<(unsigned)((m + 31) / 32), 32, 0, c->stream>>>(m, blocks, m, (const double4*)c->partial.ptr, nullptr, coulomb_k(), nullptr,
-                                                 out_phi, out_E, nullptr);
-    count_launch(c);
-    CUDA_TRY(cudaGetLastError());
-    mark(c, 3);
+    mark(c, 3);  // a6 (sum over the CTAs, k) happens in the last CTA of every pass
     c->timing_valid = c->timing;
     c->counters_pending = true;
     c->counters_counted = true;

@@ -710,13 +710,18 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
 // ------------------------------------------------------------------------------------------------
 // Few field points (m <= kFewMaxM; particle tracking asks for the field at one point after the
 // other): the roles are swapped.  Every THREAD owns elements (grid-stride), the
-// kFewM field points of the pass are shared by all lanes, every (element, point) pair gets its
-// rule from its own distance ratio (the per-pair policy of L159, exactly), and the partial sums
-// of the lanes are combined with warp shuffles, then across the warps of the CTA; a6 adds the CTAs.
-// Such a call is latency-bound, not bandwidth-bound: for one field point it reads 121 bytes per element
-// (vertices, centroid, L, area, sigma) - 121 MB for 10^6 elements in 0.10 ms = 1.2 TB/s, 18 % of the HBM
-// copy rate - in a single grid-stride pass with one dependent chain per thread, then two tiny launches.
-constexpr int kFewM = 4;        // field points per pass (grid.y)
+// field points of the pass (4; 1 or 2 if the call has no more) are shared by all lanes, every (element,
+// point) pair gets its rule from its own distance ratio (the per-pair policy of L159, exactly), and the
+// partial sums of the lanes are combined with warp shuffles, then across the warps of the CTA; the last
+// CTA of a pass to finish adds the CTAs' sums in CTA order and applies k (step a6 inside the same launch).
+// Such a call is bound by latency, not bandwidth: for one field point it reads 121 bytes per element
+// (vertices, centroid, L, area, sigma) - 121 MB for 10^6 elements.  Round 2 measured where the 0.10 ms of
+// such a call went: a pass of 4 with three clamped duplicates, one dependent load chain per thread, and a
+// second launch whose single thread added 296 partial sums one L2 round trip after the other (45 us).
+// Now: passes of 1 / 2 / 4 points, the next element's record loaded ahead of this one's arithmetic (1 / 2
+// points: the registers allow it), the sum over the CTAs inside the kernel: 0.049 ms for one point,
+// 0.066 ms for two, 0.099 ms for four (config-4 mesh, 10^6 elements, sigma kept).
+constexpr int kFewM = 4;        // field points per pass (grid.y); calls with 1 or 2 points run passes of 1 or 2
 constexpr int kFewMaxM = 64;    // above this the tiled kernels win (10^6 elements: 1.4 ms at m = 64 either way; 2.9 ms tiled with a new sigma)
 constexpr int kFewWarps = 8;
 
@@ -734,6 +739,10 @@ struct FewParams {
   unsigned long long* counters;
   const double* area;
   const double* sigma_v;  // linear density (may be null; then sigma is the constant density)
+  unsigned* done;         // [gridDim.y] CTAs of each pass that have written their partial sums (zeroed before the launch)
+  double k;               // 1/(4 pi eps0)
+  double* out_phi;        // [m]
+  double* out_E;          // [m][3] or null
 };
 
 __device__ __forceinline__ double warp_sum_f64(double v) {
@@ -745,8 +754,10 @@ __device__ __forceinline__ double warp_sum_f64(double v) {
 // The Gaussian points are computed on the fly from the vertices (the paper's own CPU variant, L218;
 // Table 4 compares it with precomputed points): no preprocessing pass, 121 instead of 260 bytes
 // read per element (reading precomputed points was measured 20 % slower here).
-template <int MODE>
+// (4 CTAs per SM at 64 registers were measured for the one-point kernel: spills, 127 instead of 76 us)
+template <int MODE, int M>
 __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __grid_constant__ FewParams p) {
+  constexpr int kFewM = M;  // field points of this pass
   __shared__ double red[kFewWarps][kFewM][4];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t j0 = (int64_t)blockIdx.y * kFewM;
@@ -764,13 +775,39 @@ __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __gri
   const double c375 = c_three_eighths;
   unsigned long long n_inter = 0, n_ana = 0;
 
-  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < p.n; e += (int64_t)gridDim.x * blockDim.x) {
-    const double4 c = p.cenL[e];
-    const int t = p.type[e];
+  // One element per thread and trip; the record of the next trip's element is loaded before this
+  // trip's arithmetic starts (a call with few points is bound by the latency of these loads).
+  struct Rec {
+    double4 c;
     double v[9];
+    double sg, ar;
+    int t;
+  };
+  auto load_rec = [&](int64_t e, Rec& r) {
+    r.c = p.cenL[e];
+    r.t = p.type[e];
 #pragma unroll
-    for (int k = 0; k < 9; ++k) v[k] = __ldg(p.verts + 9 * e + k);
-    const double q = (p.sigma ? __ldg(p.sigma + e) : 1.0) * __ldg(p.area + e);
+    for (int k = 0; k < 9; ++k) r.v[k] = __ldg(p.verts + 9 * e + k);
+    r.sg = p.sigma ? __ldg(p.sigma + e) : 1.0;
+    r.ar = __ldg(p.area + e);
+  };
+  const int64_t e_step = (int64_t)gridDim.x * blockDim.x;
+  int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  constexpr bool kPrefetch = M <= 2;  // four points per pass: the second record does not fit the registers
+  Rec nxt;
+  if (kPrefetch && e < p.n) load_rec(e, nxt);
+  for (; e < p.n; e += e_step) {
+    Rec cur;
+    if constexpr (kPrefetch) {
+      cur = nxt;
+      if (e + e_step < p.n) load_rec(e + e_step, nxt);
+    } else {
+      load_rec(e, cur);
+    }
+    const double4 c = cur.c;
+    const int t = cur.t;
+    const double (&v)[9] = cur.v;
+    const double q = cur.sg * cur.ar;
     const double* sv = p.sigma_v ? p.sigma_v + 3 * e : nullptr;
     auto point = [&](int level, int i) -> double4 {
       double4 pt;
@@ -828,7 +865,9 @@ __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __gri
     }
   }
 
-  // lanes -> warp (shuffles) -> CTA (shared memory, fixed order) -> partial[blockIdx.x]
+  // lanes -> warp (shuffles) -> CTA (shared memory, fixed order) -> partial[blockIdx.x] -> the pass's last
+  // CTA adds the CTAs' sums (fixed order too: a call is reproducible bit for bit) and writes the result
+  __shared__ bool is_last;
 #pragma unroll
   for (int j = 0; j < kFewM; ++j) {
     const double a = warp_sum_f64(acc.phi[j]);
@@ -860,6 +899,38 @@ __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __gri
     if (lane == 0) {
       if (n_inter) atomicAdd(p.counters, n_inter);
       if (n_ana) atomicAdd(p.counters + 1, n_ana);
+    }
+  }
+  __threadfence();  // this CTA's partial sums are visible before it counts itself done
+  __syncthreads();
+  if (threadIdx.x == 0) is_last = atomicAdd(p.done + blockIdx.y, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  for (int j = 0; j < mj; ++j) {
+    double4 s = make_double4(0, 0, 0, 0);
+    for (int bx = threadIdx.x; bx < (int)gridDim.x; bx += blockDim.x) {
+      const double2* v2 = reinterpret_cast<const double2*>(p.partial + (int64_t)bx * p.m + j0 + j);
+      const double2 lo = __ldcg(v2), hi = __ldcg(v2 + 1);  // L2: written by other CTAs of this launch
+      s.x += lo.x; s.y += lo.y; s.z += hi.x; s.w += hi.y;
+    }
+    s.x = warp_sum_f64(s.x); s.y = warp_sum_f64(s.y); s.z = warp_sum_f64(s.z); s.w = warp_sum_f64(s.w);
+    __syncthreads();  // red[] of the previous point (or of the CTA's own sums) has been read
+    if (lane == 0) {
+      red[warp][0][0] = s.x; red[warp][0][1] = s.y; red[warp][0][2] = s.z; red[warp][0][3] = s.w;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double4 tsum = make_double4(0, 0, 0, 0);
+      for (int w = 0; w < kFewWarps; ++w) {
+        tsum.x += red[w][0][0]; tsum.y += red[w][0][1]; tsum.z += red[w][0][2]; tsum.w += red[w][0][3];
+      }
+      p.out_phi[j0 + j] = p.k * tsum.x;
+      if (p.out_E) {
+        p.out_E[3 * (j0 + j)] = p.k * tsum.y;
+        p.out_E[3 * (j0 + j) + 1] = p.k * tsum.z;
+        p.out_E[3 * (j0 + j) + 2] = p.k * tsum.w;
+      }
     }
   }
 }

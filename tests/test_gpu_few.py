@@ -57,6 +57,21 @@ def test_fixed_rule_few_points_mixed_mesh(level):
     g.close()
 
 
+@pytest.mark.parametrize("m", [1, 2, 7])
+def test_few_point_calls_are_bit_reproducible(m):
+    """The CTAs of eval_few_kernel finish in any order; the last one of a pass adds their sums in CTA
+    order, so repeated calls return the same bits."""
+    c = synth.config4(scale=0.02, ntracks=3, npts_per_track=5)
+    g = Gpu(c["etype"], c["verts"])
+    pol = g.b.bemcub_default_policy(True)
+    pts = c["pts"][:m].copy()
+    a_phi, a_E = g.eval(c["sigma"], pts, -1, policy=pol)
+    for _ in range(4):
+        b_phi, b_E = g.eval(c["sigma"], pts, -1, policy=pol)
+        assert np.array_equal(a_phi, b_phi) and np.array_equal(a_E, b_E)
+    g.close()
+
+
 def test_sigma_null_reuses_the_charges_of_the_previous_call():
     c = synth.config4(scale=0.003, ntracks=12, npts_per_track=9)       # 108 points: the tiled path
     g = Gpu(c["etype"], c["verts"])
