@@ -157,9 +157,24 @@ __global__ void reduce_scale_kernel(int64_t m, int nsplit, int64_t split_stride,
                                     double* __restrict__ phi, double* __restrict__ E, double* __restrict__ G) {
   int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (j >= m) return;
+  // summed in split order; eight loads in flight per thread (a call with few field points and many
+  // splits spends its time here waiting for L2 otherwise)
   double4 s = partial[j];
-  for (int sp = 1; sp < nsplit; ++sp) {
-    const double4 p = partial[sp * split_stride + j];
+  int sp = 1;
+  for (; sp + 8 <= nsplit; sp += 8) {
+    double4 p[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) p[u] = partial[(int64_t)(sp + u) * split_stride + j];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      s.x += p[u].x;
+      s.y += p[u].y;
+      s.z += p[u].z;
+      s.w += p[u].w;
+    }
+  }
+  for (; sp < nsplit; ++sp) {
+    const double4 p = partial[(int64_t)sp * split_stride + j];
     s.x += p.x;
     s.y += p.y;
     s.z += p.z;

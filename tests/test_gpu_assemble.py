@@ -75,6 +75,36 @@ def test_mixed_mesh_rows_api_and_ragged_tiles():
     g.close()
 
 
+@pytest.mark.parametrize("mask", [0b101011, 0b110101, 0b100100])
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+def test_level_masks_and_row_groups(mask, allow_upgrade):
+    """use_levels_mask with rule levels switched off (a wanted level maps to the next more accurate one
+    that is enabled; with N = 33 off, the groups that straddle the analytic limit have no cubature rule to
+    fall back on and take the per-pair path), on a spatially ordered mesh whose 128-row tiles straddle
+    every limit of L159 (level-4 icosphere, 5120 triangles: L = 0.08, so the limits 3 / 8 / 20 L lie inside
+    a tile's reach; a row window that starts inside a 32-row group): every entry against the oracle.  (The
+    printed limits are kept: where a tile takes a more accurate rule than the pair asks for, the two differ
+    by the truncation error of the pair's rule, which is below the parity bar only at limits made for it.)"""
+    etype, verts = synth.icosphere_elements(4, 1.0)
+    n = len(etype)
+    g = Gpu(etype, verts)
+    dr = oracle.default_policy(False)
+    pol = g.b.make_policy(dr, allow_upgrade, mask)
+    row0, nrows = 1000 + 13, 3 * 128 + 57
+    out = g.torch.full((nrows, n), float("nan"), dtype=g.torch.float64, device="cuda")
+    g.b.bemcub_assemble_rows(g.ctx.handle, pol, row0, nrows, out, n)
+    g.torch.cuda.synchronize()
+    ref, code = oracle.assemble_rows(etype, verts, np.arange(row0, row0 + nrows), dr, levels_mask=mask)
+    _check_rows(out.cpu().numpy(), ref, code, f"mask {mask:06b} upgrade={allow_upgrade}")
+    assert len(np.unique(code)) >= 2
+    st = g.stats()
+    if not allow_upgrade:
+        assert st["analytic_pairs"] == int((code == 5).sum())
+        npts = np.array([4, 7, 12, 19, 33])
+        assert st["point_interactions"] == int(npts[code[code < 5]].sum())
+    g.close()
+
+
 def test_cfg3_level5_full_size_sampled_rows():
     """Config 3 at full size (20480 x 20480, 3.36 GB) in the launch configuration bench.py uses;
     the oracle recomputes 72 rows: row 0, row n-1, the two rows at four 64-row tile boundaries, and
