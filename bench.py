@@ -2,7 +2,7 @@
 """bench.py -- throughput of the bemcub hot path on B200 (driver contract: one JSON line on rank 0).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--workload cfg4|cfg1|cfg2|cfg3|cfg5|solve|table3|accuracy] [--scale S] [--no-secondary]
+                    [--workload cfg4|cfg1|cfg2|cfg3|cfg5|solve|table3|accuracy|few] [--scale S] [--no-secondary]
 
 Metric (BASELINE.json): FP64 Phi+E element.point interactions/s.  One step = one pass of the whole
 hot path (a1 preprocessing, a2 rule binning, a3 point-charge sum, a4 analytic near field, a6
@@ -54,7 +54,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4",
-                    choices=["cfg4", "cfg1", "cfg2", "cfg3", "cfg5", "solve", "table3", "accuracy"])
+                    choices=["cfg4", "cfg1", "cfg2", "cfg3", "cfg5", "solve", "table3", "accuracy", "few"])
     ap.add_argument("--scale", type=float, default=1.0, help="config-4 size factor (profiling only)")
     ap.add_argument("--rule", type=int, default=1, help="fixed rule level of --workload cfg2 / cfg5 / table3 (-1 = adaptive)")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
@@ -457,6 +457,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 
     if args.workload == "accuracy":
         return run_accuracy(args, b, torch, local_rank, barrier)
+    if args.workload == "few":
+        return run_few(args, b, torch, local_rank)
 
     c = make_workload(args.workload, args, rank)
     r = Runner(b, torch, local_rank, c)
@@ -664,6 +666,51 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         print(json.dumps(line), flush=True)
     if r is not None:
         r.close()
+
+
+# --------------------------------------------------------------------------------------------
+def run_few(args, b, torch, dev_index: int):
+    """Tracking-style calls (the field at one point after the other): bemcub_eval with 1 ... 64
+    field points on the config-4 mesh (10^6 elements at --scale 1), distance-ratio choice, Phi + E, with a
+    new sigma every call and with the sigma of the previous call (sigma = NULL).  One line: microseconds per
+    call (CUDA events around 200 back-to-back calls) and the bytes of element data a call reads per second."""
+    from paper_1606_03743_b200 import synth
+    dev = torch.device("cuda", dev_index)
+    c = synth.config4(args.scale, ntracks=1, npts_per_track=64)
+    n = len(c["etype"])
+    pol = b.bemcub_default_policy(b.POLICY_FIELD)
+    rows = []
+    with b.Context(dev_index) as ctx:
+        h = ctx.handle
+        b.bemcub_set_elements(h, n, torch.as_tensor(c["etype"]).to(dev), torch.as_tensor(c["verts"]).to(dev))
+        d_sigma = torch.as_tensor(c["sigma"]).to(dev)
+        for m in (1, 2, 4, 8, 16, 64):
+            pts = torch.as_tensor(c["pts"][:m].copy()).to(dev)
+            phi = torch.empty(m, dtype=torch.float64, device=dev)
+            E = torch.empty((m, 3), dtype=torch.float64, device=dev)
+            row = {"field_points": m}
+            for sig, key in ((d_sigma, "us_per_call_new_sigma"), (None, "us_per_call_sigma_kept")):
+                for _ in range(max(args.warmup, 3)):
+                    b.bemcub_eval(h, sig, -1, pol, m, pts, phi, E, b.F64)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize(dev)
+                e0.record()
+                for _ in range(200):
+                    b.bemcub_eval(h, sig, -1, pol, m, pts, phi, E, b.F64)
+                e1.record()
+                torch.cuda.synchronize(dev)
+                row[key] = e0.elapsed_time(e1) / 200 * 1e3
+            passes = 1 if m <= 2 else (m + 3) // 4
+            row["element_bytes_read_gb_s"] = 121.0 * n * passes / (row["us_per_call_sigma_kept"] * 1e-6) / 1e9
+            st = b.bemcub_get_stats(h)
+            row["points_per_pair"] = st["point_interactions"] / (float(n) * m)
+            row["launches_per_call"] = st["last_eval_launches"]
+            rows.append(row)
+    print(json.dumps({"metric": "microseconds per bemcub_eval call with few field points", "unit": "us", "higher_is_better": False,
+                      "n_gpus": 1, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": "config-4 mesh (%d elements), 1 ... 64 field points of one helical track, DR-adaptive "
+                                             "rules per pair, Phi+E; eval_few_kernel (121 bytes of element data per element and pass)" % n},
+                      "calls": rows}), flush=True)
 
 
 # --------------------------------------------------------------------------------------------

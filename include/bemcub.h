@@ -200,7 +200,7 @@ int bemcub_eval_linear(bemcub_ctx* ctx, const double* sigma_vertex, int rule_id,
 /* Dense collocation matrix (L34): out_matrix[i*ld + j] = k * Int_{element j} dS / |c_i - Q| (unit
  * sigma), c_i = centroid of element i, rule per pair by the policy (DR(i,j) uses L of element j;
  * the self term has D = 0 and is analytic).  Units V m^2 / C.  ld >= n.  The policy's
- * allow_upgrade is honoured per 64-row tile.  Asynchronous.
+ * allow_upgrade is honoured per 32-row group of a 128-row tile.  Asynchronous.
  * bemcub_assemble_rows fills rows [row0, row0+nrows) only, into out_rows[(i-row0)*ld + j]
  * (row sharding across GPUs; sampling). */
 int bemcub_assemble(bemcub_ctx* ctx, const bemcub_policy* host_policy, double* out_matrix, int64_t ld);
