@@ -155,6 +155,8 @@ int upload_tables() {
   }
   toff[5] = nt;
   roff[5] = nr;
+  for (int l = 0; l < 6; ++l)  // the unrolled point generator (rule_point_ct) has these offsets compiled in
+    if (toff[l] != kTriOffCt[l] || roff[l] != kRectOffCt[l]) return BEMCUB_ERR_BAD_RULE;
   CUDA_TRY(cudaMemcpyToSymbol(c_tri_tab, tri, sizeof(tri)));
   CUDA_TRY(cudaMemcpyToSymbol(c_rect_tab, rect, sizeof(rect)));
   CUDA_TRY(cudaMemcpyToSymbol(c_tri_off, toff, sizeof(toff)));

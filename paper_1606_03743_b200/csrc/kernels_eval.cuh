@@ -25,6 +25,7 @@
 // exact per-pair choice; elements below the analytic limit go through analytic_integrals().
 #pragma once
 #include <math_constants.h>
+#include <type_traits>
 #include "analytic.cuh"
 #include "device_utils.cuh"
 #include "kernels_pre.cuh"
@@ -719,8 +720,9 @@ __global__ void __launch_bounds__(kThreads, 1) eval_adaptive_kernel(const __grid
 // such a call went: a pass of 4 with three clamped duplicates, one dependent load chain per thread, and a
 // second launch whose single thread added 296 partial sums one L2 round trip after the other (45 us).
 // Now: passes of 1 / 2 / 4 points, the next element's record loaded ahead of this one's arithmetic (1 / 2
-// points: the registers allow it), the sum over the CTAs inside the kernel: 0.049 ms for one point,
-// 0.066 ms for two, 0.099 ms for four (config-4 mesh, 10^6 elements, sigma kept).
+// points: the registers allow it), the 7- and 12-point rules of such passes as straight-line code with the
+// tables as constant operands (rule_point_ct), the sum over the CTAs inside the kernel: 0.041 ms for one
+// point, 0.062 ms for two, 0.098 ms for four (config-4 mesh, 10^6 elements, sigma kept).
 constexpr int kFewM = 4;        // field points per pass (grid.y); calls with 1 or 2 points run passes of 1 or 2
 constexpr int kFewMaxM = 64;    // above this the tiled kernels win (10^6 elements: 1.4 ms at m = 64 either way; 2.9 ms tiled with a new sigma)
 constexpr int kFewWarps = 8;
@@ -829,7 +831,30 @@ __global__ void __launch_bounds__(kFewWarps * 32, 2) eval_few_kernel(const __gri
     }
     if (same && lev[0] != 5) {  // the usual case: one rule for all points of the pass
       const int N = rule_npts(t, lev[0]);
-      for (int i = 0; i < N; ++i) interact<double, kFewM, MODE>(point(lev[0], i), px, py, pz, acc, c375);
+      // the 7- and 12-point rules (most pairs of a mesh seen from a distance, L181) with the tables as
+      // constant operands of fully unrolled code; any other rule through the general rule_point()
+      auto unrolled = [&](auto tt, auto ll) {
+        constexpr int T = decltype(tt)::value, L = decltype(ll)::value;
+        constexpr int NN = (T == 0 ? kTriOffCt[L + 1] - kTriOffCt[L] : kRectOffCt[L + 1] - kRectOffCt[L]);
+#pragma unroll
+        for (int i = 0; i < NN; ++i) {
+          double4 pt;
+          rule_point_ct<T, L>(i, v, c, q, sv, pt);
+          interact<double, kFewM, MODE>(pt, px, py, pz, acc, c375);
+        }
+      };
+      using std::integral_constant;
+      // (four points per pass: the straight-line code of 28 - 48 interactions was measured 12 - 22 % slower
+      // than the loop - registers and instruction cache - so only passes of one or two points take it)
+      constexpr bool kUnrolled = M <= 2;
+      if (!kUnrolled)
+        for (int i = 0; i < N; ++i) interact<double, kFewM, MODE>(point(lev[0], i), px, py, pz, acc, c375);
+      else if (lev[0] == 1 && t == 1) unrolled(integral_constant<int, 1>{}, integral_constant<int, 1>{});
+      else if (lev[0] == 1 && t == 0) unrolled(integral_constant<int, 0>{}, integral_constant<int, 1>{});
+      else if (lev[0] == 2 && t == 1) unrolled(integral_constant<int, 1>{}, integral_constant<int, 2>{});
+      else if (lev[0] == 2 && t == 0) unrolled(integral_constant<int, 0>{}, integral_constant<int, 2>{});
+      else
+        for (int i = 0; i < N; ++i) interact<double, kFewM, MODE>(point(lev[0], i), px, py, pz, acc, c375);
       n_inter += (unsigned long long)N * mj;
       continue;
     }

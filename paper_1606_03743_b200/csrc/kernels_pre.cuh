@@ -110,6 +110,34 @@ __device__ __forceinline__ bool rule_point(int t, int level, int i, const double
   return true;
 }
 
+// The same point with element type, level and index known at compile time (fully unrolled callers): the
+// table entries become constant-bank operands of the FP64 instructions, with no address arithmetic and no
+// load instruction - what the kernel for few field points spends most of its non-FP64 instructions on
+// otherwise.  Same operations in the same order as rule_point(): bit-identical points.
+constexpr int kTriOffCt[6] = {0, 4, 11, 23, 42, 75};   // = c_tri_off / c_rect_off (checked by bemcub_create)
+constexpr int kRectOffCt[6] = {0, 4, 11, 23, 40, 73};
+template <int T, int LEVEL>
+__device__ __forceinline__ void rule_point_ct(int i, const double* __restrict__ v, const double4 c, double q,
+                                              const double* __restrict__ sv, double4& out) {
+  if constexpr (T == 0) {
+    const double* r = c_tri_tab + 4 * (kTriOffCt[LEVEL] + i);
+    const double la = r[0], lb = r[1], lc = r[2];
+    out.x = fma(lc, v[6], fma(lb, v[3], la * v[0]));
+    out.y = fma(lc, v[7], fma(lb, v[4], la * v[1]));
+    out.z = fma(lc, v[8], fma(lb, v[5], la * v[2]));
+    const double sq = sv ? fma(lc, sv[2], fma(lb, sv[1], la * sv[0])) : 1.0;
+    out.w = r[3] * q * sq;
+  } else {
+    const double* r = c_rect_tab + 4 * (kRectOffCt[LEVEL] + i);
+    const double xs = 0.5 * r[0], ys = 0.5 * r[1];
+    out.x = fma(ys, v[6] - v[0], fma(xs, v[3] - v[0], c.x));
+    out.y = fma(ys, v[7] - v[1], fma(xs, v[4] - v[1], c.y));
+    out.z = fma(ys, v[8] - v[2], fma(xs, v[5] - v[2], c.z));
+    const double sq = sv ? fma(0.5 + ys, sv[2] - sv[0], fma(0.5 + xs, sv[1] - sv[0], sv[0])) : 1.0;
+    out.w = r[2] * q * sq;
+  }
+}
+
 template <typename T> struct Point4;
 template <> struct Point4<double> { typedef double4 type; };
 template <> struct Point4<float> { typedef float4 type; };
