@@ -61,6 +61,9 @@ struct bemcub_ctx {
   const double* sort_src = nullptr;
   int64_t sort_m = 0;
   DevBuf solve_buf[6];  // GMRES: centroids, diagonal, basis, w, z/residual, small coefficient block
+  // matrix fill: the rows of the last call in Morton order of their centroids (kept until the mesh changes)
+  DevBuf asm_cen, asm_perm;
+  int64_t asm_perm_row0 = -1, asm_perm_nrows = -1;
   DevBuf solve_matrix;   // the collocation matrix of a solve that keeps it (bemcub_solve_storage)
   int64_t solve_matrix_limit = 0;  // bytes; 0 = every solve is matrix-free
   DevBuf host_stage[5];  // device copies of host inputs/outputs for the *_host entry points
@@ -478,6 +481,7 @@ int bemcub_destroy(bemcub_ctx* c) {
   release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
   for (int i = 0; i < 6; ++i) release(c->solve_buf[i]);
   release(c->solve_matrix);
+  release(c->asm_cen); release(c->asm_perm);
   if (c->d_status) cudaFree(c->d_status);
   if (c->d_counters) cudaFree(c->d_counters);
   for (int i = 0; i < 4; ++i)
@@ -492,6 +496,7 @@ int bemcub_set_elements(bemcub_ctx* c, int64_t n, const uint8_t* type, const dou
   c->has_mesh = false;
   c->n = 0;
   c->sort_perm = nullptr;
+  c->asm_perm_row0 = c->asm_perm_nrows = -1;
   c->sigma_kept = false;
   for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = false;
   int rc;
@@ -865,6 +870,38 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
     ap.stride[l] = (c->stride[l] + kAsmU - 1) / kAsmU * kAsmU;
     if (used && (rc = expand_level<double>(c, l, nullptr, c->pts64[l], nullptr, ap.stride[l], coulomb_k()))) return rc;
     ap.lvl_pts[l] = (const double4*)c->pts64[l].ptr;
+  }
+  // A tile is 128 consecutive rows and its row groups 32: they have to be compact patches whatever the
+  // order the caller's elements come in (a shuffled level-5 icosphere otherwise executes 33 points for
+  // every entry: 12.1 instead of 5.3 ms).  So the centroids are put in Morton order - the sort of step a2
+  // (kernels_sort.cuh), once per mesh and row window - and the rows are taken in that order where it gives
+  // clearly tighter 32-row groups than the caller's own (a device flag: no host round trip).
+  ap.row_perm = nullptr;
+  ap.use_perm = nullptr;
+  if (nrows > kAsmRows && nrows < ((int64_t)1 << 31)) {
+    if (c->asm_perm_row0 != row0 || c->asm_perm_nrows != nrows) {
+      c->asm_perm_row0 = c->asm_perm_nrows = -1;
+      if ((rc = ensure(c->asm_cen, (size_t)nrows * 24)) || (rc = ensure(c->asm_perm, (size_t)nrows * 4 + 32))) return rc;
+      CUDA_TRY(cudaMemcpy2DAsync(c->asm_cen.ptr, 24, (const double4*)c->cenL.ptr + row0, 32, 24, (size_t)nrows,
+                                 cudaMemcpyDeviceToDevice, c->stream));
+      const uint32_t* perm = nullptr;
+      const double* sorted = nullptr;
+      c->sort_perm = nullptr;  // the sort buffers are shared with the evaluation calls
+      if ((rc = sort_field_points(c, nrows, (const double*)c->asm_cen.ptr, &perm, &sorted))) return rc;
+      CUDA_TRY(cudaMemcpyAsync(c->asm_perm.ptr, perm, (size_t)nrows * 4, cudaMemcpyDeviceToDevice, c->stream));
+      const int64_t ngroups = (nrows + 31) / 32;
+      float* radius = (float*)c->asm_cen.ptr;  // the packed centroids have served the sort
+      int* flag = (int*)((char*)c->asm_perm.ptr + (((size_t)nrows * 4 + 15) & ~(size_t)15));
+      group_radius_kernel<<<(unsigned)((2 * ngroups * 32 + 255) / 256), 256, 0, c->stream>>>(
+          nrows, (const double4*)c->cenL.ptr + row0, (const uint32_t*)c->asm_perm.ptr, ngroups, radius);
+      choose_row_order_kernel<<<1, 32, 0, c->stream>>>(ngroups, radius, flag);
+      count_launch(c, 2);
+      CUDA_TRY(cudaGetLastError());
+      c->asm_perm_row0 = row0;
+      c->asm_perm_nrows = nrows;
+    }
+    ap.row_perm = (const uint32_t*)c->asm_perm.ptr;
+    ap.use_perm = (const int*)((const char*)c->asm_perm.ptr + (((size_t)nrows * 4 + 15) & ~(size_t)15));
   }
   ap.cenL = (const double4*)c->cenL.ptr;
   ap.type = (const uint8_t*)c->type.ptr;

@@ -39,6 +39,8 @@ struct AssembleParams {
   int64_t n;
   PolicyDev pol;
   int64_t row0, nrows;
+  const uint32_t* row_perm;   // [nrows] or null: the k-th row of the call, in tile order, is row0 + row_perm[k]
+  const int* use_perm;        // device flag (choose_row_order_kernel): take row_perm, or the rows as they come
   double* out;
   int64_t ld;
   double k;
@@ -65,6 +67,7 @@ struct AsmWarpSmem {
   double tile[kGroupCols * kAsmRows];  // [column of the group][row]: conflict-free both ways
   uint32_t seg[kStages][32];  // col | row-group mask << 5 | npts << 9 | first << 16
   double sub[kAsmR][4];       // bounding spheres of the tile's 32-row groups (centre, radius)
+  uint32_t rowidx[kAsmRows];  // rows of the tile, relative to row0 (tiles take the rows in Morton order of their centroids)
   uint32_t aq[kAqCap];
   uint64_t bar[kStages];
   unsigned long long n_inter, n_ana;
@@ -154,6 +157,39 @@ __device__ __forceinline__ double pick_row(const double (&v)[kAsmR], int i) {
   return (i & 2) ? hi : lo;
 }
 
+// Which order of the rows gives the tighter 32-row groups: the caller's, or the Morton order of the centroids?
+// group_radius_kernel: one warp per group and order, radius of the group's bounding sphere (about the centre of
+// its FP32 box); choose_row_order_kernel: one warp adds the radii of each order in a fixed sequence and sets the
+// flag if Morton order is clearly tighter (a mesh that arrives spatially ordered keeps its order: its groups
+// are as compact and its rows lie next to each other in the output).
+__global__ void group_radius_kernel(int64_t nrows, const double4* __restrict__ cen, const uint32_t* __restrict__ perm,
+                                    int64_t ngroups, float* __restrict__ radius) {
+  const int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (w >= 2 * ngroups) return;
+  const int which = w >= ngroups;
+  const int64_t g = which ? w - ngroups : w;
+  const int64_t k = min(g * 32 + lane, nrows - 1);
+  const double4 c = cen[which ? (int64_t)perm[k] : k];
+  const float fx = (float)c.x, fy = (float)c.y, fz = (float)c.z;
+  const double sx = 0.5 * ((double)warp_min_f32(fx) + (double)warp_max_f32(fx));
+  const double sy = 0.5 * ((double)warp_min_f32(fy) + (double)warp_max_f32(fy));
+  const double sz = 0.5 * ((double)warp_min_f32(fz) + (double)warp_max_f32(fz));
+  const double d2 = (c.x - sx) * (c.x - sx) + (c.y - sy) * (c.y - sy) + (c.z - sz) * (c.z - sz);
+  const float r = sqrtf(warp_max_f32((float)d2));
+  if (lane == 0) radius[w] = r;
+}
+__global__ void choose_row_order_kernel(int64_t ngroups, const float* __restrict__ radius, int* __restrict__ use_perm) {
+  const int lane = threadIdx.x;
+  double s[2] = {0.0, 0.0};
+  for (int which = 0; which < 2; ++which) {
+    for (int64_t g = lane; g < ngroups; g += 32) s[which] += (double)radius[which * ngroups + g];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s[which] += __shfl_xor_sync(kFullMask, s[which], o);
+  }
+  if (lane == 0) *use_perm = s[1] < 0.8 * s[0];
+}
+
 __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_constant__ AssembleParams p) {
   static_assert(kAsmU == 4 || kAsmU == 2 || kAsmU == 1, "phi_segment's sum tree");
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -186,7 +222,8 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
     const bool second_pass = item >= p.nitems;
     if (second_pass) item -= p.nitems;
     const int64_t split = item / p.nrowtiles, rt = item - split * p.nrowtiles;
-    const int64_t r0 = rt * kAsmRows;  // first row of the tile, relative to row0
+    const int64_t r0 = rt * kAsmRows;  // first row of the tile in tile order
+    const bool use_perm = p.row_perm && *p.use_perm;
     const int nrow_here = (int)min((int64_t)kAsmRows, p.nrows - r0);
 
     // rows: field points = centroids (clamped duplicates compute harmlessly and are never stored)
@@ -195,7 +232,10 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
 #pragma unroll
     for (int r = 0; r < kAsmR; ++r) {
       ok[r] = r * 32 + lane < nrow_here;
-      const double4 ci = p.cenL[p.row0 + r0 + min(r * 32 + lane, nrow_here - 1)];
+      const int64_t k = r0 + min(r * 32 + lane, nrow_here - 1);
+      const uint32_t row = use_perm ? p.row_perm[k] : (uint32_t)k;
+      sm.rowidx[r * 32 + lane] = row;
+      const double4 ci = p.cenL[p.row0 + row];
       px[r] = ci.x; py[r] = ci.y; pz[r] = ci.z;
     }
     // Bounding spheres of every 32-row group (rows r * 32 + lane: consecutive elements, a compact patch of
@@ -241,13 +281,14 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
         const uint32_t ent = sm.aq[(aq_head + lane) & (kAqCap - 1)];
         const int row = (int)(ent >> 25);
         const int64_t col = (int64_t)(ent & 0x1ffffffu);
-        const double4 ci = ldg4(p.cenL + p.row0 + r0 + row);
+        const int64_t grow = sm.rowidx[row];
+        const double4 ci = ldg4(p.cenL + p.row0 + grow);
         Vec3 V[4];
         const int nv = load_polygon(p.type, p.verts, col, V);
         double ip;
         Vec3 ie;
         analytic_integrals<false>(V, nv, Vec3{ci.x, ci.y, ci.z}, ip, ie);
-        p.out[(r0 + row) * p.ld + col] = p.k * ip;
+        p.out[grow * p.ld + col] = p.k * ip;
       }
       aq_head += take;
       __syncwarp();
@@ -384,7 +425,7 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
               const int row = r * 32 + lane;
               if (row < nrow_here) {
                 const double* t = &sm.tile[row];
-                double2* o = reinterpret_cast<double2*>(p.out + (r0 + row) * p.ld + jg);
+                double2* o = reinterpret_cast<double2*>(p.out + (int64_t)sm.rowidx[row] * p.ld + jg);
                 const double2 a = make_double2(t[0], t[kAsmRows]), b = make_double2(t[2 * kAsmRows], t[3 * kAsmRows]);
                 const double2 c = make_double2(t[4 * kAsmRows], t[5 * kAsmRows]), d = make_double2(t[6 * kAsmRows], t[7 * kAsmRows]);
                 o[0] = a; o[1] = b; o[2] = c; o[3] = d;
@@ -393,9 +434,8 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
           } else {
             const int c = lane & (kGroupCols - 1);
             if ((gmask >> c) & 1u) {
-              double* o = p.out + (r0 + (lane >> 3)) * p.ld + jg + c;
               const double* t = &sm.tile[c * kAsmRows + (lane >> 3)];
-              for (int row = lane >> 3; row < nrow_here; row += 4, o += 4 * p.ld, t += 4) *o = *t;
+              for (int row = lane >> 3; row < nrow_here; row += 4, t += 4) p.out[(int64_t)sm.rowidx[row] * p.ld + jg + c] = *t;
             }
           }
         }
@@ -510,7 +550,7 @@ __global__ void __launch_bounds__(kAsmThreads, 1) assemble_kernel(const __grid_c
         }
 #pragma unroll
         for (int r = 0; r < kAsmR; ++r)
-          if (ok[r]) p.out[(r0 + r * 32 + lane) * p.ld + j] = val[r];
+          if (ok[r]) p.out[(int64_t)sm.rowidx[r * 32 + lane] * p.ld + j] = val[r];
       }
       // ---- streamed columns: fill the other stage, then consume this one (one call site each: the
       // kernel has to fit the instruction cache)
