@@ -5,7 +5,13 @@ the full element list (field points are independent, element contr
 `torch.distributed` is used only for the barrier, the max-over-ranks timing and, when the caller
 wants the whole result on one rank, a gather of the outputs.
 
-No arithmetic of the method lives here.  Works with any backend (`nccl` on GPUs, `gloo` in the
+For a handful of field points (a tracker's calls, L32) the other natural sharding is by ELEMENTS:
+every rank holds a contiguous range of the mesh, evaluates the same field points against it, and the
+per-point sums (32 bytes per field point) are added over the ranks - the one exchange step this path
+has, and a tiny one.  `sum_in_rank_order` does it as an all-gather followed by a sum in rank order, so
+every rank ends with the same bits whatever the backend's reduction order.
+
+No arithmetic of the method lives here beyond that sum.  Works with any backend (`nccl` on GPUs, `gloo` in the
 CPU tests).
 """
 from __future__ import annotations
@@ -69,3 +75,19 @@ def gather_rows(local, total: int, dst: int = 0):
     if rank != dst:
         return None
     return torch.cat([b[: hi - lo] for b, (lo, hi) in zip(bufs, sizes)], dim=0)
+
+
+def sum_in_rank_order(local):
+    """Element-sharded evaluation: `local` = this rank's partial Phi / E sums for the SAME field points
+    (any shape, same on every rank).  Returns their sum over the ranks, added in rank order, on every rank."""
+    import torch
+    import torch.distributed as dist
+    rank, ws = world()
+    if ws == 1:
+        return local
+    bufs = [torch.empty_like(local) for _ in range(ws)]
+    dist.all_gather(bufs, local.contiguous())
+    total = bufs[0].clone()
+    for b in bufs[1:]:
+        total += b
+    return total

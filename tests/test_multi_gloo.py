@@ -44,12 +44,16 @@ def _worker(rank: int, ws: int, port: int, q):
         mat = multi.gather_rows(torch.as_tensor(rows), n)
         t = multi.max_over_ranks(10.0 + rank)
         u = multi.sum_over_ranks(float(hi - lo))
+        # element sharding for few field points: each rank's elements, the same points, sums in rank order
+        elo, ehi = multi.my_range(n)
+        part = oracle.evaluate(c["etype"][elo:ehi], c["verts"][elo:ehi], c["sigma"][elo:ehi], c["pts"][:3], 1)
+        tot = multi.sum_in_rank_order(torch.as_tensor(np.concatenate([part["phi"][:, None], part["E"]], axis=1))).numpy()
         dist.barrier()
         if rank == 0:
-            q.put((lo, hi, full.numpy(), mat.numpy(), t, u))
+            q.put((lo, hi, full.numpy(), mat.numpy(), t, u, tot))
         else:
             assert full is None and mat is None
-            q.put((lo, hi, None, None, t, u))
+            q.put((lo, hi, None, None, t, u, tot))
     finally:
         dist.destroy_process_group()
 
@@ -83,7 +87,7 @@ def test_two_rank_gloo_field_point_and_row_sharding():
         p.join(timeout=30)
         assert p.exitcode == 0
     got.sort(key=lambda g: g[0])
-    (lo0, hi0, full, mat, t0, u0), (lo1, hi1, _, _, t1, u1) = got
+    (lo0, hi0, full, mat, t0, u0, tot0), (lo1, hi1, _, _, t1, u1, tot1) = got
     assert (lo0, hi0, lo1, hi1) == (0, 51, 51, 101)
     assert t0 == t1 == 11.0                 # max over ranks
     assert u0 == u1 == 101.0                # whole-job units
@@ -93,6 +97,9 @@ def test_two_rank_gloo_field_point_and_row_sharding():
     assert np.array_equal(full[:, 0], ref["phi"]) and np.array_equal(full[:, 1:], ref["E"])
     rows, _ = oracle.assemble_rows(c["etype"], c["verts"], np.arange(len(c["etype"])), oracle.default_policy(False))
     assert np.array_equal(mat, rows)
+    # element-sharded sums: the same bits on both ranks, and the full sum up to the order of two additions
+    assert np.array_equal(tot0, tot1)
+    assert np.allclose(tot0[:, 0], ref["phi"][:3], rtol=1e-13, atol=0) and np.allclose(tot0[:, 1:], ref["E"][:3], rtol=1e-12, atol=1e-300)
 
 
 # ------------------------------------------------------------------ the product under torch.distributed
@@ -127,8 +134,17 @@ def _gpu_worker(rank: int, ws: int, port: int, q):
             torch.cuda.synchronize()
             mat = multi.gather_rows(rows.cpu(), n)
             launches = multi.sum_over_ranks(float(b.bemcub_get_stats(h)["kernel_launches"]))
+            # the other sharding (few field points): this rank's contiguous range of the ELEMENTS, the same
+            # five field points on every rank, per-point sums added in rank order
+            elo, ehi = multi.my_range(n)
+            b.bemcub_set_elements(h, ehi - elo, d(c["etype"][elo:ehi]), d(c["verts"][elo:ehi]))
+            p5 = torch.empty(5, dtype=torch.float64, device="cuda")
+            e5 = torch.empty((5, 3), dtype=torch.float64, device="cuda")
+            b.bemcub_eval(h, d(c["sigma"][elo:ehi]), b.RULE_ADAPTIVE, pol, 5, d(c["pts"][:5]), p5, e5, b.F64)
+            torch.cuda.synchronize()
+            few = multi.sum_in_rank_order(torch.cat([p5[:, None], e5], dim=1).cpu())
         dist.barrier()
-        q.put((rank, None if full is None else full.numpy(), None if mat is None else mat.numpy(), launches))
+        q.put((rank, None if full is None else full.numpy(), None if mat is None else mat.numpy(), launches, few.numpy()))
     finally:
         dist.destroy_process_group()
 
@@ -154,7 +170,7 @@ def test_two_processes_one_gpu_product_path():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    (_, full, mat, launches), (_, full1, mat1, _) = got
+    (_, full, mat, launches, few0), (_, full1, mat1, _, few1) = got
     assert full1 is None and mat1 is None and launches > 0
     c = synth.config4(scale=0.002, ntracks=23, npts_per_track=31)
     ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=oracle.default_policy(True), want_counts=True)
@@ -164,3 +180,7 @@ def test_two_processes_one_gpu_product_path():
     A, code = oracle.assemble_rows(c["etype"], c["verts"], np.arange(len(c["etype"])), oracle.default_policy(False))
     rel = np.abs(mat - A) / np.abs(A)
     assert rel[code < 5].max() <= 1e-12 and rel[code == 5].max() <= 1e-10
+    # element-sharded few-point evaluation: identical bits on both ranks, parity with the oracle's full sum
+    assert np.array_equal(few0, few1)
+    assert np.all(np.abs(few0[:, 0] - ref["phi"][:5]) <= tol[:5] * ref["Sphi"][:5])
+    assert np.all(np.abs(few0[:, 1:] - ref["E"][:5]).max(axis=1) <= tol[:5] * ref["SE"][:5])
