@@ -72,6 +72,31 @@ def test_few_point_calls_are_bit_reproducible(m):
     g.close()
 
 
+@pytest.mark.parametrize("n_el", [1, 2, 33])
+@pytest.mark.parametrize("m", [1, 2, 3])
+def test_tiny_meshes_few_points(n_el, m):
+    """Fewer elements than threads (most CTAs of eval_few_kernel have nothing to add, the last one still
+    sums all of them), triangles and rectangles mixed, every rule level and the distance-ratio choice."""
+    et, vt = synth.random_elements(synth.TRI, n_el, 71)
+    er, vr = synth.random_elements(synth.RECT, n_el, 72)
+    etype, verts = np.concatenate([et, er]), np.concatenate([vt, vr])
+    rng = np.random.default_rng(73 + m)
+    sigma = rng.uniform(-1, 1, len(etype))
+    pts = 2.0 + 3.0 * rng.random((m, 3))
+    g = Gpu(etype, verts)
+    for level in (0, 1, 2, 3, 4):
+        phi, E = g.eval(sigma, pts, level)
+        err = parity_errors(phi, E, oracle.evaluate(etype, verts, sigma, pts, level))
+        assert err["phi"] <= TOL_F64 and err["E"] <= TOL_F64, (level, err)
+    pol = g.b.bemcub_default_policy(True)
+    ref = oracle.evaluate(etype, verts, sigma, pts, -1, dr=oracle.default_policy(True), want_counts=True)
+    phi, E = g.eval(sigma, pts, -1, policy=pol)
+    err = parity_errors(phi, E, ref)
+    assert err["phi"] <= 1e-10 and err["E"] <= 1e-10, err
+    assert g.stats()["point_interactions"] == int(ref["npi"].sum())
+    g.close()
+
+
 def test_sigma_null_reuses_the_charges_of_the_previous_call():
     c = synth.config4(scale=0.003, ntracks=12, npts_per_track=9)       # 108 points: the tiled path
     g = Gpu(c["etype"], c["verts"])
