@@ -561,9 +561,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         inter_own = float(b.bemcub_get_stats(h)["point_interactions"])
     elif not is_matrix and not adaptive:
         inter_own = inter
+    paired = (not is_matrix) and b.bemcub_last_path(h) == b.PATH_PAIRED
     kernel = ("assemble_kernel" if (is_solve and args.store_matrix) else "eval_adaptive_kernel<kModePhi>" if is_solve else
               "assemble_kernel" if is_matrix else
-              ("eval_adaptive_kernel" if adaptive else "eval_fixed_kernel"))
+              ("eval_paired_kernel" if paired else "eval_adaptive_kernel" if adaptive else "eval_fixed_kernel"))
+    # FP64 instructions the kernel executed per interaction (device tally): 18 / 12 / 28, fewer in paired form
+    if st.get("fp64_instructions") and inter:
+        ipi = st["fp64_instructions"] / inter
     if precision == b.F32:
         roof = {"bound": "alu", "achieved": inter * fpi / (k_ms * 1e-3) / 1e12, "peak": None, "unit": "TFLOP/s", "frac": None,
                 "traffic": None, "note": "FP32 variant: reported, no FP32 peak measured"}
@@ -575,6 +579,12 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "kernel_over_ceiling": None if is_matrix else (inter / (k_ms * 1e-3)) / loop_rate,
             "source": "bemcub_inner_loop_rate: Eq. 4.1 loop (18 FP64 instr + MUFU, 8 of 18 are FMAs => at most 26/36 = 72.2% "
                       "of the FLOP peak), resident data"}
+        if paired:
+            roof["paired_form"] = ("rectangle rules evaluated in +- point pairs (kernels_paired.cuh): the same point-charge "
+                                   "interactions of Eq. 4.1 (26 flop each by the plain count, which `achieved` and `frac` use) with "
+                                   "%.2f instead of 18 FP64 instructions per interaction, so the 26/36 = 72.2 %% cap of the plain "
+                                   "instruction mix does not bind; fp64_issue_frac_arith uses the executed count; "
+                                   "inner_loop_ceiling is the PLAIN loop's rate" % ipi)
         roof["peak_sweep"] = peak["sweep"]
         if is_matrix:
             roof["store_stream_gb_s"] = float(n) * n * 8 / (k_ms * 1e-3) / 1e9

@@ -115,6 +115,10 @@ typedef struct {
   int64_t kernel_ns;           /* last eval/assemble call, read on the device (clock64 and  */
                                /* %globaltimer of one persistent CTA): cycles/ns = the SM   */
                                /* clock the kernel really ran at; 0 for calls with m <= 64  */
+  int64_t fp64_instructions;   /* FP64 instructions per field point the interactions of the */
+                               /* last eval/assemble executed: 18 (Phi+E), 12 (Phi), 28     */
+                               /* (+gradient) per interaction; fewer where the rectangle    */
+                               /* rules ran in paired form (BEMCUB_PATH_PAIRED); 0 for FP32 */
 } bemcub_stats;
 
 /* device: CUDA device ordinal.  cuda_stream: a cudaStream_t cast to void* (NULL = default).    */
@@ -285,6 +289,17 @@ int bemcub_inner_loop_rate(bemcub_ctx* ctx, double seconds, double* host_interac
  * milliseconds (HOST outputs, either may be NULL); INVALID_ARG if no timed call has been made. */
 int bemcub_set_timing(bemcub_ctx* ctx, int enable);
 int bemcub_get_timing(bemcub_ctx* ctx, double* host_ms_total, double* host_ms_kernel);
+
+/* Which kernel the last bemcub_eval* call of this ctx ran its field points through (HOST output): the
+ * tests use it to know that a parity case exercised the path it was written for. */
+enum {
+  BEMCUB_PATH_NONE = 0,
+  BEMCUB_PATH_FIXED = 1,     /* eval_fixed_kernel: one rule for every pair                               */
+  BEMCUB_PATH_ADAPTIVE = 2,  /* eval_adaptive_kernel: rule per (element, tile) by distance ratio         */
+  BEMCUB_PATH_PAIRED = 3,    /* eval_paired_kernel: the same with the rectangle rules' points in +- pairs */
+  BEMCUB_PATH_FEW = 4        /* eval_few_kernel: m <= 64, elements over the threads, rule per pair        */
+};
+int bemcub_last_path(bemcub_ctx* ctx, int* host_path);
 
 /* HOST struct.  Synchronises the ctx stream when device counters of the last call are pending. */
 int bemcub_get_stats(bemcub_ctx* ctx, bemcub_stats* host_stats);

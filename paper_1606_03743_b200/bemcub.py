@@ -33,7 +33,7 @@ class bemcub_policy(C.Structure):
 class bemcub_stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_int64), ("point_interactions", C.c_int64),
                 ("analytic_pairs", C.c_int64), ("last_eval_launches", C.c_int64),
-                ("kernel_cycles", C.c_int64), ("kernel_ns", C.c_int64)]
+                ("kernel_cycles", C.c_int64), ("kernel_ns", C.c_int64), ("fp64_instructions", C.c_int64)]
 
 
 class BemcubError(RuntimeError):
@@ -78,6 +78,7 @@ def _load() -> C.CDLL:
         "bemcub_inner_loop_rate": [vp, dbl, C.POINTER(dbl)],
         "bemcub_get_stats": [vp, C.POINTER(bemcub_stats)],
         "bemcub_reset_stats": [vp],
+        "bemcub_last_path": [vp, C.POINTER(C.c_int)],
         "bemcub_set_timing": [vp, C.c_int],
         "bemcub_get_timing": [vp, C.POINTER(dbl), C.POINTER(dbl)],
     }
@@ -95,7 +96,7 @@ EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_
             "bemcub_eval_gradient", "bemcub_eval_linear", "bemcub_eval_pairs", "bemcub_solve", "bemcub_solve_storage", "bemcub_matvec",
             "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
             "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
-            "bemcub_fp64_peak", "bemcub_fp64_issue_sweep", "bemcub_inner_loop_rate", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_set_timing",
+            "bemcub_fp64_peak", "bemcub_fp64_issue_sweep", "bemcub_inner_loop_rate", "bemcub_get_stats", "bemcub_reset_stats", "bemcub_last_path", "bemcub_set_timing",
             "bemcub_get_timing", "bemcub_strerror"]
 
 
@@ -216,6 +217,15 @@ def bemcub_solve(ctx, policy, rhs_potential, sigma, rel_tol: float, max_matvecs:
 
 def bemcub_matvec(ctx, matrix, ld: int, x, y) -> None:
     _check(_lib.bemcub_matvec(ctx, _dptr(matrix), ld, _dptr(x), _dptr(y)), "bemcub_matvec")
+
+
+PATH_NONE, PATH_FIXED, PATH_ADAPTIVE, PATH_PAIRED, PATH_FEW = 0, 1, 2, 3, 4
+
+
+def bemcub_last_path(ctx) -> int:
+    v = C.c_int()
+    _check(_lib.bemcub_last_path(ctx, C.byref(v)), "bemcub_last_path")
+    return v.value
 
 
 def bemcub_solve_storage(ctx, max_matrix_bytes: int) -> None:

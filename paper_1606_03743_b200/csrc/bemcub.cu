@@ -14,6 +14,7 @@
 #include "kernels_eval.cuh"
 #include "kernels_pairs.cuh"
 #include "kernels_pre.cuh"
+#include "kernels_paired.cuh"
 #include "kernels_solve.cuh"
 #include "kernels_sort.cuh"
 #include "rules.h"
@@ -49,6 +50,12 @@ struct bemcub_ctx {
   // expanded points per level (FP64 / FP32) and the stride they were built with
   DevBuf pts64[5], pts32[5];
   int stride[5] = {4, 7, 12, 19, 33};
+  // rectangles in paired form per level (kernels_paired.cuh), with the sigma of the last call like pts64
+  DevBuf pair64[5];
+  bool charged_pair[5] = {false, false, false, false, false};
+  int pair_np[5] = {0, 0, 0, 0, 0};  // pairs of the rectangle rule of each level (0: not pairable)
+  int last_path = BEMCUB_PATH_NONE;
+  int last_ipi = 0;  // FP64 instructions per interaction of the last call's kernels (0: FP32)
   // scratch
   DevBuf partial, partial_g;
   // charges of the last call that passed a sigma: which expanded levels still hold them, and the
@@ -167,6 +174,50 @@ int upload_tables() {
   return BEMCUB_OK;
 }
 
+// Pairs (x, y), (-x, -y) of equal weight in the rectangle rules (kernels_paired.cuh): found in the tables
+// themselves, so a rule that were not symmetric would simply not be paired (np = 0).
+int upload_pair_tables(int np_out[5]) {
+  double tab[5 * 16 * 4] = {0.0}, cw[5] = {0.0};
+  int np[5] = {0, 0, 0, 0, 0};
+  for (int l = 0; l < 5; ++l) {
+    bemcub_rules::RectPoint rp[bemcub_rules::kMaxN];
+    const int n = bemcub_rules::rect_points(l, rp);
+    bool used[bemcub_rules::kMaxN] = {false};
+    int k = 0;
+    bool ok = true;
+    for (int i = 0; i < n && ok; ++i) {
+      if (used[i]) continue;
+      used[i] = true;
+      if (rp[i].x == 0.0 && rp[i].y == 0.0) {
+        cw[l] += rp[i].w;
+        continue;
+      }
+      int partner = -1;
+      for (int j = i + 1; j < n; ++j)
+        if (!used[j] && rp[j].x == -rp[i].x && rp[j].y == -rp[i].y && rp[j].w == rp[i].w) {
+          partner = j;
+          break;
+        }
+      if (partner < 0 || k >= 16) {
+        ok = false;
+        break;
+      }
+      used[partner] = true;
+      tab[4 * (16 * l + k)] = rp[i].x;
+      tab[4 * (16 * l + k) + 1] = rp[i].y;
+      tab[4 * (16 * l + k) + 2] = rp[i].w;
+      ++k;
+    }
+    np[l] = ok ? k : 0;
+    if (!ok) cw[l] = 0.0;
+  }
+  CUDA_TRY(cudaMemcpyToSymbol(c_pair_tab, tab, sizeof(tab)));
+  CUDA_TRY(cudaMemcpyToSymbol(c_pair_center_w, cw, sizeof(cw)));
+  CUDA_TRY(cudaMemcpyToSymbol(c_pair_np, np, sizeof(np)));
+  for (int l = 0; l < 5; ++l) np_out[l] = np[l];
+  return BEMCUB_OK;
+}
+
 // use_levels_mask -> level actually used for each wanted level (bemcub.h: next more accurate
 // enabled one, else the most accurate enabled one below).
 int build_policy(const bemcub_policy* hp, PolicyDev* out) {
@@ -259,6 +310,13 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) 
   return s;
 }
 
+// launch configuration of eval_paired_kernel (measured on config 4)
+#ifndef BEMCUB_PR
+#define BEMCUB_PR 3
+#define BEMCUB_PW 12
+#endif
+constexpr int kPairedR = BEMCUB_PR, kPairedWarps = BEMCUB_PW;
+
 template <typename T, int R, int MODE = kModePhiE>
 int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
   const size_t smem = eval_smem_bytes<T>();  // opted in once per device by configure_kernels()
@@ -308,6 +366,7 @@ int configure_kernels() {
       (rc = configure_adaptive<double, kModePhi>()) || (rc = configure_adaptive<double, kModeGrad>()) ||
       (rc = configure_adaptive<float, kModePhiE>()) || (rc = configure_adaptive<float, kModePhi>()) ||
       (rc = opt_in_smem(assemble_kernel, assemble_smem_bytes())) ||
+      (rc = opt_in_smem(eval_paired_kernel<kPairedR, kPairedWarps>, paired_smem_bytes<kPairedWarps>())) ||
       (rc = opt_in_smem(inner_loop_kernel<4>, eval_smem_bytes<double>())))
     return rc;
   return BEMCUB_OK;
@@ -368,6 +427,7 @@ void refresh_counters(bemcub_ctx* c) {
     }
     c->stats.kernel_cycles = (int64_t)h[4];
     c->stats.kernel_ns = (int64_t)h[5];
+    c->stats.fp64_instructions = c->stats.point_interactions * c->last_ipi - (int64_t)h[3];  // h[3]: saved by the paired form
   }
   c->counters_pending = false;
 }
@@ -460,6 +520,7 @@ int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream) {
   }
   c->num_sms = prop.multiProcessorCount;
   int rc = upload_tables();
+  if (rc == BEMCUB_OK) rc = upload_pair_tables(c->pair_np);
   if (rc == BEMCUB_OK) rc = configure_kernels();
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_status, sizeof(GeomStatus)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, kCounterSlots * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
@@ -476,7 +537,7 @@ int bemcub_destroy(bemcub_ctx* c) {
   DeviceGuard g(c->device);
   cudaStreamSynchronize(c->stream);
   release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial); release(c->partial_g); release(c->sigma_keep);
-  for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); }
+  for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); release(c->pair64[l]); }
   for (int i = 0; i < 2; ++i) { release(c->sort_key[i]); release(c->sort_idx[i]); }
   release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
   for (int i = 0; i < 6; ++i) release(c->solve_buf[i]);
@@ -498,7 +559,7 @@ int bemcub_set_elements(bemcub_ctx* c, int64_t n, const uint8_t* type, const dou
   c->sort_perm = nullptr;
   c->asm_perm_row0 = c->asm_perm_nrows = -1;
   c->sigma_kept = false;
-  for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = false;
+  for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = c->charged_pair[l] = false;
   int rc;
   const size_t nn = (size_t)std::max<int64_t>(n, 1);
   if ((rc = ensure(c->type, nn)) || (rc = ensure(c->verts, nn * 72)) || (rc = ensure(c->cenL, nn * sizeof(double4))) ||
@@ -618,7 +679,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     if (!c->sigma_kept) return BEMCUB_ERR_INVALID_ARG;
     sigma = (const double*)c->sigma_keep.ptr;
   } else {
-    for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = false;  // other charges from now on
+    for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = c->charged_pair[l] = false;  // other charges from now on
     c->sigma_kept = false;
     if (sigma) {
       if ((rc = ensure(c->sigma_keep, (size_t)c->n * 8))) return rc;
@@ -669,6 +730,8 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     CUDA_TRY(cudaGetLastError());
     mark(c, 2);
     mark(c, 3);  // a6 (sum over the CTAs, k) happens in the last CTA of every pass
+    c->last_path = BEMCUB_PATH_FEW;
+    c->last_ipi = out_E ? 18 : 12;
     c->timing_valid = c->timing;
     c->counters_pending = true;
     c->counters_counted = true;
@@ -684,7 +747,29 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     charged[l] = sigma_v == nullptr;  // a linear density is not kept (sigma_keep holds constants only)
   }
 
-  const SplitPlan sp = plan_splits(c, m, grad ? 2 : 4, adaptive);  // R = 6 was measured: 2 % slower than R = 4 in the full kernel
+  // Rectangles in paired form (kernels_paired.cuh): FP64 Phi + E with the distance-ratio choice, a constant
+  // density, a policy whose analytic branch covers the rectangles below a distance ratio of 2 at least (so
+  // that |d| < |D| wherever a pair is evaluated), and field points enough for tiles of 32 kPairedR.
+  bool paired = false;
+  if (adaptive && !grad && precision == BEMCUB_F64 && out_E && !sigma_v && c->has_rect && pol.map[5] == 5 && pol.dr[1][0] >= 2.0) {
+    for (int l = 0; l < 5; ++l) paired |= need[l] && c->pair_np[l] > 0;
+    if (paired) paired = plan_splits(c, m, kPairedR, true).R == kPairedR;
+  }
+  if (paired) {
+    for (int l = 0; l < 5; ++l) {
+      const int np = c->pair_np[l];
+      if (!need[l] || np == 0 || c->charged_pair[l]) continue;
+      if ((rc = ensure(c->pair64[l], (size_t)c->n * pair_units(np) * sizeof(double4)))) return rc;
+      const int64_t total = c->n * (np + 1);
+      expand_pairs_kernel<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(
+          c->n, l, np, (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr, (const double4*)c->cenL.ptr,
+          (const double*)c->area.ptr, sigma, (double*)c->pair64[l].ptr);
+      count_launch(c);
+      CUDA_TRY(cudaGetLastError());
+      c->charged_pair[l] = true;
+    }
+  }
+  SplitPlan sp = plan_splits(c, m, paired ? kPairedR : (grad ? 2 : 4), adaptive);  // R = 6 was measured: 2 % slower than R = 4 in the full kernel
   if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
   if (grad && (rc = ensure(c->partial_g, (size_t)sp.nsplit * (size_t)m * 48))) return rc;
   // a2: tiles of spatially close field points (adaptive mode; a fixed rule has nothing to choose)
@@ -760,7 +845,19 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     ap.queue = c->d_counters + 2;
     ap.counters = c->d_counters;
     CUDA_TRY(cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
-    if (grad) rc = sp.R == 2 ? launch_adaptive<double, 2, kModeGrad>(c, ap, sp) : launch_adaptive<double, 1, kModeGrad>(c, ap, sp);
+    if (paired) {
+      PairedParams pq;
+      pq.ad = ap;
+      for (int l = 0; l < 5; ++l) {
+        pq.pair_np[l] = need[l] ? c->pair_np[l] : 0;
+        pq.pair_pts[l] = (const double4*)c->pair64[l].ptr;
+      }
+      const int grid = (int)std::min<int64_t>(c->num_sms, (sp.nitems + kPairedWarps - 1) / kPairedWarps);
+      eval_paired_kernel<kPairedR, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);
+      count_launch(c);
+      CUDA_TRY(cudaGetLastError());
+      rc = BEMCUB_OK;
+    } else if (grad) rc = sp.R == 2 ? launch_adaptive<double, 2, kModeGrad>(c, ap, sp) : launch_adaptive<double, 1, kModeGrad>(c, ap, sp);
     else if (precision == BEMCUB_F64 && !out_E)
       rc = sp.R == 4 ? launch_adaptive<double, 4, kModePhi>(c, ap, sp) : sp.R == 2 ? launch_adaptive<double, 2, kModePhi>(c, ap, sp) : launch_adaptive<double, 1, kModePhi>(c, ap, sp);
     else if (precision == BEMCUB_F64)
@@ -774,6 +871,8 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     c->counters_counted = true;
   }
 
+  c->last_path = !adaptive ? BEMCUB_PATH_FIXED : paired ? BEMCUB_PATH_PAIRED : BEMCUB_PATH_ADAPTIVE;
+  c->last_ipi = precision != BEMCUB_F64 ? 0 : grad ? 28 : out_E ? 18 : 12;
   mark(c, 2);
   // a6: cross-split reduction and the 1/(4 pi eps0) prefactor
   const int threads = 256;
@@ -929,6 +1028,7 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
   const int grid = (int)std::min<int64_t>(c->num_sms, (ap.nitems + kAsmWarps - 1) / kAsmWarps);
   mark(c, 1);
   assemble_kernel<<<grid, kAsmThreads, assemble_smem_bytes(), c->stream>>>(ap);
+  c->last_ipi = 12;
   count_launch(c);
   CUDA_TRY(cudaGetLastError());
   mark(c, 2);
@@ -1124,6 +1224,12 @@ int bemcub_get_timing(bemcub_ctx* c, double* host_ms_total, double* host_ms_kern
   CUDA_TRY(cudaEventElapsedTime(&b, c->ev[1], c->ev[2]));
   if (host_ms_total) *host_ms_total = a;
   if (host_ms_kernel) *host_ms_kernel = b;
+  return BEMCUB_OK;
+}
+
+int bemcub_last_path(bemcub_ctx* c, int* host_path) {
+  if (!c || !host_path) return BEMCUB_ERR_INVALID_ARG;
+  *host_path = c->last_path;
   return BEMCUB_OK;
 }
 

@@ -1,0 +1,127 @@
+"""-m gpu parity tests of eval_paired_kernel (csrc/kernels_paired.cuh): the distance-ratio evaluation with the
+rectangle rules' points taken in symmetric pairs (App. B, Eq. 3.2, Eq. 4.1).  The kernel is taken
+for FP64 Phi + E calls on meshes with rectangles once there are field points enough for 96-point tiles, so
+these cases are sized to reach it (bemcub_last_path says which kernel ran) while the oracle still needs
+only seconds.  Same acceptance protocol as everywhere (gpu_common.py)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1606_03743_b200 import synth
+
+from gpu_common import Gpu, TOL_ANALYTIC, TOL_F64, parity_errors
+
+pytestmark = pytest.mark.gpu
+
+
+def _split_parity(phi, E, ref, what):
+    """1e-12 where the oracle's sum used no analytic pair, 1e-10 elsewhere."""
+    assert np.all(np.isfinite(phi)) and np.all(np.isfinite(E)), what
+    ephi = np.abs(phi - ref["phi"]) / ref["Sphi"]
+    eE = np.abs(E - ref["E"]).max(axis=1) / ref["SE"]
+    tol = np.where(ref["nana"] > 0, TOL_ANALYTIC, TOL_F64)
+    assert np.all(ephi <= tol), f"{what}: potential {ephi.max():.3e}"
+    assert np.all(eE <= tol), f"{what}: field {eE.max():.3e}"
+    return float(ephi.max()), float(eE.max())
+
+
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+def test_mixed_mesh_far_field(allow_upgrade):
+    """Config 4 in small (4000 rectangles + 1000 triangles, 22 500 track points, a ragged last tile): paired
+    rectangles of the 7- and 12-point rules next to plain triangle points in the same stages."""
+    c = synth.config4(scale=0.005, ntracks=150, npts_per_track=150)
+    g = Gpu(c["etype"], c["verts"])
+    pol = g.b.bemcub_default_policy(True)
+    pol.allow_upgrade = allow_upgrade
+    phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_PAIRED
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=oracle.default_policy(True), want_counts=True)
+    _split_parity(phi, E, ref, f"mixed mesh upgrade={allow_upgrade}")
+    st = g.stats()
+    if allow_upgrade:
+        assert st["point_interactions"] >= int(ref["npi"].sum())
+    else:
+        assert st["point_interactions"] == int(ref["npi"].sum()) and st["analytic_pairs"] == int(ref["nana"].sum())
+    # Phi only and the field gradient are not paired: the call falls back to the plain kernel, same numbers
+    phi2, _ = g.eval(c["sigma"], c["pts"], -1, policy=pol, want_E=False)
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_ADAPTIVE
+    assert np.max(np.abs(phi2 - ref["phi"]) / ref["Sphi"]) <= TOL_F64
+    g.close()
+
+
+def _near_points(etype, verts, m, seed, hmin, hmax):
+    """Field points from hmin to hmax mean sides off random elements of the mesh (along the normal, with a
+    lateral offset of up to one side): every distance-ratio band, the analytic one included."""
+    cen, L = synth.mean_side_and_centre(etype, verts)
+    rng = np.random.default_rng(seed)
+    pick = rng.integers(0, len(etype), m)
+    e1 = verts[pick, 1] - verts[pick, 0]
+    e2 = verts[pick, 2] - verts[pick, 0]
+    nrm = np.cross(e1, e2)
+    nrm /= np.linalg.norm(nrm, axis=1)[:, None]
+    h = L[pick] * np.exp(rng.uniform(np.log(hmin), np.log(hmax), m))
+    lat = rng.uniform(-0.5, 0.5, (m, 2))
+    return np.ascontiguousarray(cen[pick] + nrm * h[:, None] + lat[:, :1] * e1 + lat[:, 1:] * e2)
+
+
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+def test_cube_surface_all_bands(allow_upgrade):
+    """6144 squares (the config-2 mesh), 22 000 field points from 0.3 to 300 sides off the surface: all five
+    paired rules, the analytic branch, tiles that straddle limits (upgrades, or pair by pair)."""
+    c = synth.config2(m=8)
+    etype, verts, sigma = c["etype"], c["verts"], c["sigma"]
+    pts = _near_points(etype, verts, 22000, 31, 0.3, 300.0)
+    g = Gpu(etype, verts)
+    pol = g.b.bemcub_default_policy(True)
+    pol.allow_upgrade = allow_upgrade
+    phi, E = g.eval(sigma, pts, -1, policy=pol)
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_PAIRED
+    ref = oracle.evaluate(etype, verts, sigma, pts, -1, dr=oracle.default_policy(True), want_counts=True)
+    _split_parity(phi, E, ref, f"cube upgrade={allow_upgrade}")
+    assert int(ref["nana"].sum()) > 0 and len(np.unique(ref["npi"])) > 100
+    if not allow_upgrade:
+        st = g.stats()
+        assert st["point_interactions"] == int(ref["npi"].sum()) and st["analytic_pairs"] == int(ref["nana"].sum())
+    g.close()
+
+
+def test_pairs_down_to_a_distance_ratio_of_two_and_the_fallback():
+    """A policy whose analytic limit for rectangles is exactly 2 still takes the paired kernel (|d| < |D| holds
+    there: the outermost pair of the 33-point rule sits 0.7 sides from the centre); per-pair policy, so every
+    pair uses the oracle's rule and the comparison is at the 1e-12 bar even at these close ranges.  One with a
+    lower limit, or without the analytic branch, must fall back to the plain kernel."""
+    c = synth.config2(m=8)
+    etype, verts, sigma = c["etype"], c["verts"], c["sigma"]
+    pts = _near_points(etype, verts, 22000, 32, 1.0, 60.0)
+    g = Gpu(etype, verts)
+    dr = np.array([[2.0, 4.0, 8.0, 20.0, 100.0], [2.0, 4.0, 8.0, 20.0, 100.0]])
+    ref = oracle.evaluate(etype, verts, sigma, pts, -1, dr=dr, want_counts=True)
+    phi, E = g.eval(sigma, pts, -1, policy=g.b.make_policy(dr, 0))
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_PAIRED
+    _split_parity(phi, E, ref, "limits 2/4/8/20/100")
+    assert g.stats()["point_interactions"] == int(ref["npi"].sum())
+    dr_low = dr.copy()
+    dr_low[1, 0] = 1.9
+    phi, E = g.eval(sigma, pts, -1, policy=g.b.make_policy(dr_low, 0))
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_ADAPTIVE
+    phi, E = g.eval(sigma, pts, -1, policy=g.b.make_policy(dr, 0, 0b011111))
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_ADAPTIVE
+    g.close()
+
+
+def test_level_mask_and_reproducibility():
+    """Rule levels switched off (7 -> 12, 17 -> 33 points) and repeated calls: same bits every time."""
+    c = synth.config4(scale=0.005, ntracks=150, npts_per_track=150)
+    g = Gpu(c["etype"], c["verts"])
+    mask = 0b110101
+    pol = g.b.bemcub_default_policy(True)
+    pol.use_levels_mask = mask
+    a_phi, a_E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_PAIRED
+    ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], -1, dr=oracle.default_policy(True), levels_mask=mask,
+                          want_counts=True)
+    _split_parity(a_phi, a_E, ref, "mask 110101")
+    for _ in range(3):
+        b_phi, b_E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+        assert np.array_equal(a_phi, b_phi) and np.array_equal(a_E, b_E)
+    g.close()
