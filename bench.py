@@ -44,7 +44,7 @@ FP64_LANES_PER_SM = 64          # B200: one FP64 warp instruction per scheduler 
 METRIC = "FP64 Phi+E element.point interactions/s"
 UNIT = "element.point interactions/s"
 # ncu counter of the committed capture of the bench's own launch configuration (not measured by this run)
-NCU_PIPE = {"cfg4": ("profiles/r2_cfg4_full_eval_adaptive_counters.csv", "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed")}
+NCU_PIPE = {"cfg4": ("profiles/r2_cfg4_full_eval_paired_counters.csv", "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed")}
 
 
 def parse_args():
