@@ -311,11 +311,7 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) 
 }
 
 // launch configuration of eval_paired_kernel (measured on config 4)
-#ifndef BEMCUB_PR
-#define BEMCUB_PR 3
-#define BEMCUB_PW 12
-#endif
-constexpr int kPairedR = BEMCUB_PR, kPairedWarps = BEMCUB_PW;
+constexpr int kPairedR = 3, kPairedWarps = 12;
 
 template <typename T, int R, int MODE = kModePhiE>
 int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
@@ -367,6 +363,7 @@ int configure_kernels() {
       (rc = configure_adaptive<float, kModePhiE>()) || (rc = configure_adaptive<float, kModePhi>()) ||
       (rc = opt_in_smem(assemble_kernel, assemble_smem_bytes())) ||
       (rc = opt_in_smem(eval_paired_kernel<kPairedR, kPairedWarps>, paired_smem_bytes<kPairedWarps>())) ||
+      (rc = opt_in_smem(eval_paired_kernel<1, kPairedWarps>, paired_smem_bytes<kPairedWarps>())) ||
       (rc = opt_in_smem(inner_loop_kernel<4>, eval_smem_bytes<double>())))
     return rc;
   return BEMCUB_OK;
@@ -753,7 +750,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   bool paired = false;
   if (adaptive && !grad && precision == BEMCUB_F64 && out_E && !sigma_v && c->has_rect && pol.map[5] == 5 && pol.dr[1][0] >= 2.0) {
     for (int l = 0; l < 5; ++l) paired |= need[l] && c->pair_np[l] > 0;
-    if (paired) paired = plan_splits(c, m, kPairedR, true).R == kPairedR;
+    // (with fewer field points: one per lane, as the plain kernel does - plan_splits gives 3 or 1)
   }
   if (paired) {
     for (int l = 0; l < 5; ++l) {
@@ -853,7 +850,10 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
         pq.pair_pts[l] = (const double4*)c->pair64[l].ptr;
       }
       const int grid = (int)std::min<int64_t>(c->num_sms, (sp.nitems + kPairedWarps - 1) / kPairedWarps);
-      eval_paired_kernel<kPairedR, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);
+      if (sp.R == kPairedR)
+        eval_paired_kernel<kPairedR, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);
+      else
+        eval_paired_kernel<1, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);
       count_launch(c);
       CUDA_TRY(cudaGetLastError());
       rc = BEMCUB_OK;

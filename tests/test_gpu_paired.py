@@ -1,8 +1,9 @@
 """-m gpu parity tests of eval_paired_kernel (csrc/kernels_paired.cuh): the distance-ratio evaluation with the
 rectangle rules' points taken in symmetric pairs (App. B, Eq. 3.2, Eq. 4.1).  The kernel is taken
-for FP64 Phi + E calls on meshes with rectangles once there are field points enough for 96-point tiles, so
-these cases are sized to reach it (bemcub_last_path says which kernel ran) while the oracle still needs
-only seconds.  Same acceptance protocol as everywhere (gpu_common.py)."""
+for FP64 Phi + E distance-ratio calls on meshes with rectangles (bemcub_last_path says which kernel ran):
+with 96-point tiles once there are field points enough - these cases are sized for that while the oracle
+still needs only seconds - and with 32-point tiles below (every adaptive case of test_gpu_eval.py on a
+mixed mesh).  Same acceptance protocol as everywhere (gpu_common.py)."""
 import numpy as np
 import pytest
 
