@@ -7,11 +7,11 @@
 //     |P - Q|^2 = (|D|^2 + |d|^2) -+ 2 D.d ,
 // and D, |D|^2 are shared by all points of the element, D.d by the two points of a pair.  The pair's
 // contribution to Eq. 4.1 (L139-143) is then
-//     Phi += q (y+ + y-),    E += (g+ + g-) D + (g- - g+) d ,    y = 1/|P - Q|,  g = q y^3 ,
-// with the first E term summed per element (S = sum of g, one multiply-add with D at the end).
-// That is 30 FP64 instructions per pair instead of 36, and 9 instead of 18 for the centre point:
-// 108 instead of 126 per 7-point element, 189 instead of 216 per 12-point element (bare loops on B200:
-// 1.08e12 against 0.93e12 point-charge interactions/s).  The sums are the sums of Eq. 4.1 term by term;
+//     Phi += q (y+ + y-),    E += q (y+^3 + y-^3) D + (y-^3 - y+^3) (q d) ,    y = 1/|P - Q| ,
+// with the first E term summed per element (S = sum of q y^3, one multiply-add with D at the end) and
+// q d stored beside d.  That is 28 FP64 instructions per pair instead of 36, and 9 instead of 18 for the
+// centre point: 102 instead of 126 per 7-point element, 177 instead of 216 per 12-point element (bare
+// loops on B200 with 30 per pair: 1.08e12 against 0.93e12 point-charge interactions/s).  The sums are the sums of Eq. 4.1 term by term;
 // only the rounding differs (|D|^2 + |d|^2 -+ 2 D.d loses nothing as long as |d| < |D|, i.e. at every
 // distance ratio a cubature rule is used at; the host takes this kernel only under policies whose
 // analytic limit for rectangles is >= 2).  Triangle rules have no such symmetry: triangles, and rectangles
@@ -33,8 +33,8 @@ __constant__ double c_pair_center_w[5];
 __constant__ int c_pair_np[5];
 
 // Element block of a paired rectangle, in 32-byte units of the window:
-//   [C.x C.y C.z q_centre] [d.x d.y | d.z q | |d|^2 0] x NP      = 4 + 6 NP doubles, rounded up to whole units
-__host__ __device__ constexpr int pair_units(int np) { return (4 + 6 * np + 3) / 4; }
+//   [C.x C.y C.z q_centre] [d.x d.y d.z q | |d|^2 q d.x q d.y q d.z] x NP      = 1 + 2 NP units
+__host__ __device__ constexpr int pair_units(int np) { return 1 + 2 * np; }
 
 // One thread per (element, slot): slot 0 writes the centre record, slot k > 0 pair k - 1.  Triangles are skipped.
 __global__ void expand_pairs_kernel(int64_t n, int level, int np, const uint8_t* __restrict__ type, const double* __restrict__ verts,
@@ -51,7 +51,6 @@ __global__ void expand_pairs_kernel(int64_t n, int level, int np, const uint8_t*
   if (slot == 0) {
     const double4 c = cenL[e];
     blk[0] = c.x; blk[1] = c.y; blk[2] = c.z; blk[3] = c_pair_center_w[level] * q;
-    if ((4 + 6 * np) & 3) { blk[4 + 6 * np] = 0.0; blk[4 + 6 * np + 1] = 0.0; }  // tail of the last unit
   } else {
     const double* r = c_pair_tab + 4 * (16 * level + slot - 1);
     const double xs = 0.5 * r[0], ys = 0.5 * r[1];
@@ -59,9 +58,10 @@ __global__ void expand_pairs_kernel(int64_t n, int level, int np, const uint8_t*
     const double dx = fma(ys, v[6] - v[0], xs * (v[3] - v[0]));
     const double dy = fma(ys, v[7] - v[1], xs * (v[4] - v[1]));
     const double dz = fma(ys, v[8] - v[2], xs * (v[5] - v[2]));
-    double* p = blk + 4 + 6 * (slot - 1);
-    p[0] = dx; p[1] = dy; p[2] = dz; p[3] = r[2] * q;
-    p[4] = fma(dx, dx, fma(dy, dy, dz * dz)); p[5] = 0.0;
+    double* p = blk + 4 + 8 * (slot - 1);
+    const double qk = r[2] * q;
+    p[0] = dx; p[1] = dy; p[2] = dz; p[3] = qk;
+    p[4] = fma(dx, dx, fma(dy, dy, dz * dz)); p[5] = qk * dx; p[6] = qk * dy; p[7] = qk * dz;
   }
 }
 
@@ -83,35 +83,30 @@ __device__ __forceinline__ void consume_pairs(const double4* __restrict__ buf, i
       D2[r] = __fma_rn(Dx[r], Dx[r], yz);
       if constexpr (HC) {  // the centre point: |P - Q| = |D|
         const double y = rsqrt_f64(D2[r], yz, c375);
-        const double qy = __dmul_rn(c.w, y);
-        a.phi[r] = __dadd_rn(a.phi[r], qy);
-        S[r] = __dmul_rn(qy, __dmul_rn(y, y));
+        a.phi[r] = __fma_rn(c.w, y, a.phi[r]);
+        S[r] = __dmul_rn(c.w, __dmul_rn(y, __dmul_rn(y, y)));
       } else {
         S[r] = 0.0;
       }
     }
-    const double2* pr = reinterpret_cast<const double2*>(blk + 1);
     constexpr int kUnroll = NP <= 3 ? NP : 1;  // (partial unrolling of the longer rules: no difference measured)
 #pragma unroll kUnroll
     for (int k = 0; k < NP; ++k) {
-      const double2 a0 = pr[3 * k], a1 = pr[3 * k + 1], a2 = pr[3 * k + 2];
-      const double dx = a0.x, dy = a0.y, dz = a1.x, q = a1.y, d2 = a2.x;
+      const double4 a0 = blk[1 + 2 * k], a1 = blk[2 + 2 * k];  // d, q | |d|^2, q d
 #pragma unroll
       for (int r = 0; r < R; ++r) {
-        const double B = __fma_rn(Dx[r], dx, __fma_rn(Dy[r], dy, __dmul_rn(Dz[r], dz)));  // D.d
-        const double A = __dadd_rn(D2[r], d2);
+        const double B = __fma_rn(Dx[r], a0.x, __fma_rn(Dy[r], a0.y, __dmul_rn(Dz[r], a0.z)));  // D.d
+        const double A = __dadd_rn(D2[r], a1.x);
         const double rp = __fma_rn(-2.0, B, A), rm = __fma_rn(2.0, B, A);  // |P - (C + d)|^2, |P - (C - d)|^2
         const double yp = rsqrt_f64(rp, A, c375), ym = rsqrt_f64(rm, B, c375);
-        const double qp = __dmul_rn(q, yp), qm = __dmul_rn(q, ym);
-        a.phi[r] = __dadd_rn(a.phi[r], qp);
-        a.phi[r] = __dadd_rn(a.phi[r], qm);
-        const double gp = __dmul_rn(qp, __dmul_rn(yp, yp)), gm = __dmul_rn(qm, __dmul_rn(ym, ym));
-        // E += gp (D - d) + gm (D + d) = (gp + gm) D + (gm - gp) d
-        S[r] = __dadd_rn(S[r], __dadd_rn(gp, gm));
-        const double t = __dsub_rn(gm, gp);
-        a.ex[r] = __fma_rn(t, dx, a.ex[r]);
-        a.ey[r] = __fma_rn(t, dy, a.ey[r]);
-        a.ez[r] = __fma_rn(t, dz, a.ez[r]);
+        a.phi[r] = __fma_rn(a0.w, __dadd_rn(yp, ym), a.phi[r]);
+        const double cp = __dmul_rn(yp, __dmul_rn(yp, yp)), cm = __dmul_rn(ym, __dmul_rn(ym, ym));
+        // E += q y+^3 (D - d) + q y-^3 (D + d) = q (y+^3 + y-^3) D + (y-^3 - y+^3) (q d)
+        S[r] = __fma_rn(a0.w, __dadd_rn(cp, cm), S[r]);
+        const double t = __dsub_rn(cm, cp);
+        a.ex[r] = __fma_rn(t, a1.y, a.ex[r]);
+        a.ey[r] = __fma_rn(t, a1.z, a.ey[r]);
+        a.ez[r] = __fma_rn(t, a1.w, a.ez[r]);
       }
     }
 #pragma unroll
@@ -307,8 +302,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) eval_paired_kernel(const __grid
               key = lvl;
               cnt = estride = pair_units(np);
               src = pp.pair_pts[lvl] + e * estride;
-              // 9 per element (D, |D|^2, S D), 9 for a centre point, 30 per pair - instead of 18 per point
-              saved = 18 * realn - (9 + (realn > 2 * np ? 9 : 0) + 30 * np);
+              // 9 per element (D, |D|^2, S D), 9 for a centre point, 28 per pair - instead of 18 per point
+              saved = 18 * realn - (9 + (realn > 2 * np ? 9 : 0) + 28 * np);
             } else {
               key = 8 + lvl;
               cnt = realn;
