@@ -117,8 +117,8 @@ typedef struct {
                                /* clock the kernel really ran at; 0 for calls with m <= 64  */
   int64_t fp64_instructions;   /* FP64 instructions per field point the interactions of the */
                                /* last eval/assemble executed: 18 (Phi+E), 12 (Phi), 28     */
-                               /* (+gradient) per interaction; fewer where the rectangle    */
-                               /* rules ran in paired form (BEMCUB_PATH_PAIRED); 0 for FP32 */
+                               /* (+gradient) per interaction; fewer where rules ran in      */
+                               /* paired / median form (BEMCUB_PATH_PAIRED); 0 for FP32     */
 } bemcub_stats;
 
 /* device: CUDA device ordinal.  cuda_stream: a cudaStream_t cast to void* (NULL = default).    */
@@ -297,6 +297,7 @@ enum {
   BEMCUB_PATH_FIXED = 1,     /* eval_fixed_kernel: one rule for every pair                               */
   BEMCUB_PATH_ADAPTIVE = 2,  /* eval_adaptive_kernel: rule per (element, tile) by distance ratio         */
   BEMCUB_PATH_PAIRED = 3,    /* eval_paired_kernel: the same with the rectangle rules' points in +- pairs */
+                             /* and the 7-point triangle rule's points on the medians                    */
   BEMCUB_PATH_FEW = 4        /* eval_few_kernel: m <= 64, elements over the threads, rule per pair        */
 };
 int bemcub_last_path(bemcub_ctx* ctx, int* host_path);

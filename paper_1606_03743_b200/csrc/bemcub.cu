@@ -54,6 +54,8 @@ struct bemcub_ctx {
   DevBuf pair64[5];
   bool charged_pair[5] = {false, false, false, false, false};
   int pair_np[5] = {0, 0, 0, 0, 0};  // pairs of the rectangle rule of each level (0: not pairable)
+  DevBuf tri7;             // triangles' blocks for the 7-point rule in median form
+  bool charged_tri7 = false, tri7_ok = false;
   int last_path = BEMCUB_PATH_NONE;
   int last_ipi = 0;  // FP64 instructions per interaction of the last call's kernels (0: FP32)
   // scratch
@@ -215,6 +217,50 @@ int upload_pair_tables(int np_out[5]) {
   CUDA_TRY(cudaMemcpyToSymbol(c_pair_center_w, cw, sizeof(cw)));
   CUDA_TRY(cudaMemcpyToSymbol(c_pair_np, np, sizeof(np)));
   for (int l = 0; l < 5; ++l) np_out[l] = np[l];
+  return BEMCUB_OK;
+}
+
+// The 7-point triangle rule as centroid + two orbits on the medians (kernels_paired.cuh): read off the table;
+// *ok_out = false (and zeros uploaded) if the table does not have that structure.
+int upload_tri7_tables(bool* ok_out) {
+  bemcub_rules::TriPoint tp[bemcub_rules::kMaxN];
+  const int n = bemcub_rules::tri_points(1, tp);
+  double kappa[2] = {0.0, 0.0}, w[3] = {0.0, 0.0, 0.0};
+  int seen[2][3] = {{0, 0, 0}, {0, 0, 0}};
+  int norb = 0, ncen = 0;
+  bool ok = n == 7;
+  for (int i = 0; i < n && ok; ++i) {
+    const double la = tp[i].la, lb = tp[i].lb, lc = tp[i].lc;
+    if (la == lb && lb == lc) {
+      w[0] = tp[i].w;
+      ++ncen;
+      continue;
+    }
+    int vtx;
+    double a, b;
+    if (lb == lc) { vtx = 0; a = la; b = lb; }
+    else if (la == lc) { vtx = 1; a = lb; b = la; }
+    else if (la == lb) { vtx = 2; a = lc; b = la; }
+    else { ok = false; break; }
+    const double k = a - b;
+    int o = -1;
+    for (int j = 0; j < norb; ++j)
+      if (std::fabs(kappa[j] - k) <= 1e-14) o = j;
+    if (o < 0) {
+      if (norb == 2) { ok = false; break; }
+      o = norb++;
+      kappa[o] = k;
+      w[1 + o] = tp[i].w;
+    }
+    if (tp[i].w != w[1 + o] || seen[o][vtx]) { ok = false; break; }
+    seen[o][vtx] = 1;
+  }
+  ok = ok && ncen == 1 && norb == 2;
+  for (int o = 0; o < 2 && ok; ++o) ok = seen[o][0] && seen[o][1] && seen[o][2];
+  if (!ok) kappa[0] = kappa[1] = w[0] = w[1] = w[2] = 0.0;
+  CUDA_TRY(cudaMemcpyToSymbol(c_tri7_kappa, kappa, sizeof(kappa)));
+  CUDA_TRY(cudaMemcpyToSymbol(c_tri7_w, w, sizeof(w)));
+  *ok_out = ok;
   return BEMCUB_OK;
 }
 
@@ -518,6 +564,7 @@ int bemcub_create(bemcub_ctx** out_ctx, int device, void* cuda_stream) {
   c->num_sms = prop.multiProcessorCount;
   int rc = upload_tables();
   if (rc == BEMCUB_OK) rc = upload_pair_tables(c->pair_np);
+  if (rc == BEMCUB_OK) rc = upload_tri7_tables(&c->tri7_ok);
   if (rc == BEMCUB_OK) rc = configure_kernels();
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_status, sizeof(GeomStatus)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
   if (rc == BEMCUB_OK && cudaMalloc(&c->d_counters, kCounterSlots * sizeof(unsigned long long)) != cudaSuccess) rc = BEMCUB_ERR_NOMEM;
@@ -535,6 +582,7 @@ int bemcub_destroy(bemcub_ctx* c) {
   cudaStreamSynchronize(c->stream);
   release(c->type); release(c->verts); release(c->cenL); release(c->area); release(c->partial); release(c->partial_g); release(c->sigma_keep);
   for (int l = 0; l < 5; ++l) { release(c->pts64[l]); release(c->pts32[l]); release(c->host_stage[l]); release(c->pair64[l]); }
+  release(c->tri7);
   for (int i = 0; i < 2; ++i) { release(c->sort_key[i]); release(c->sort_idx[i]); }
   release(c->sort_hist); release(c->sort_pts); release(c->sort_box);
   for (int i = 0; i < 6; ++i) release(c->solve_buf[i]);
@@ -557,6 +605,7 @@ int bemcub_set_elements(bemcub_ctx* c, int64_t n, const uint8_t* type, const dou
   c->asm_perm_row0 = c->asm_perm_nrows = -1;
   c->sigma_kept = false;
   for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = c->charged_pair[l] = false;
+  c->charged_tri7 = false;
   int rc;
   const size_t nn = (size_t)std::max<int64_t>(n, 1);
   if ((rc = ensure(c->type, nn)) || (rc = ensure(c->verts, nn * 72)) || (rc = ensure(c->cenL, nn * sizeof(double4))) ||
@@ -677,6 +726,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     sigma = (const double*)c->sigma_keep.ptr;
   } else {
     for (int l = 0; l < 5; ++l) c->charged64[l] = c->charged32[l] = c->charged_pair[l] = false;  // other charges from now on
+    c->charged_tri7 = false;
     c->sigma_kept = false;
     if (sigma) {
       if ((rc = ensure(c->sigma_keep, (size_t)c->n * 8))) return rc;
@@ -747,14 +797,27 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   // Rectangles in paired form (kernels_paired.cuh): FP64 Phi + E with the distance-ratio choice, a constant
   // density, a policy whose analytic branch covers the rectangles below a distance ratio of 2 at least (so
   // that |d| < |D| wherever a pair is evaluated), and field points enough for tiles of 32 kPairedR.
-  bool paired = false;
-  if (adaptive && !grad && precision == BEMCUB_F64 && out_E && !sigma_v && c->has_rect && pol.map[5] == 5 && pol.dr[1][0] >= 2.0) {
-    for (int l = 0; l < 5; ++l) paired |= need[l] && c->pair_np[l] > 0;
+  bool paired = false, tri7 = false;
+  if (adaptive && !grad && precision == BEMCUB_F64 && out_E && !sigma_v && pol.map[5] == 5) {
+    if (c->has_rect && pol.dr[1][0] >= 2.0)
+      for (int l = 0; l < 5; ++l) paired |= need[l] && c->pair_np[l] > 0;
+    // ... and the 7-point triangle rule in median form, under the same condition on the triangles' analytic limit
+    tri7 = c->has_tri && c->tri7_ok && need[1] && pol.dr[0][0] >= 2.0;
+    paired |= tri7;
     // (with fewer field points: one per lane, as the plain kernel does - plan_splits gives 3 or 1)
+  }
+  if (paired && tri7 && !c->charged_tri7) {
+    if ((rc = ensure(c->tri7, (size_t)c->n * kTri7Units * sizeof(double4)))) return rc;
+    expand_tri7_kernel<<<(unsigned)((4 * c->n + 255) / 256), 256, 0, c->stream>>>(
+        c->n, (const uint8_t*)c->type.ptr, (const double*)c->verts.ptr, (const double4*)c->cenL.ptr, (const double*)c->area.ptr,
+        sigma, (double*)c->tri7.ptr);
+    count_launch(c);
+    CUDA_TRY(cudaGetLastError());
+    c->charged_tri7 = true;
   }
   if (paired) {
     for (int l = 0; l < 5; ++l) {
-      const int np = c->pair_np[l];
+      const int np = (c->has_rect && pol.dr[1][0] >= 2.0) ? c->pair_np[l] : 0;
       if (!need[l] || np == 0 || c->charged_pair[l]) continue;
       if ((rc = ensure(c->pair64[l], (size_t)c->n * pair_units(np) * sizeof(double4)))) return rc;
       const int64_t total = c->n * (np + 1);
@@ -846,9 +909,10 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
       PairedParams pq;
       pq.ad = ap;
       for (int l = 0; l < 5; ++l) {
-        pq.pair_np[l] = need[l] ? c->pair_np[l] : 0;
+        pq.pair_np[l] = (need[l] && c->has_rect && pol.dr[1][0] >= 2.0) ? c->pair_np[l] : 0;
         pq.pair_pts[l] = (const double4*)c->pair64[l].ptr;
       }
+      pq.tri7_pts = tri7 ? (const double4*)c->tri7.ptr : nullptr;
       const int grid = (int)std::min<int64_t>(c->num_sms, (sp.nitems + kPairedWarps - 1) / kPairedWarps);
       if (sp.R == kPairedR)
         eval_paired_kernel<kPairedR, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);

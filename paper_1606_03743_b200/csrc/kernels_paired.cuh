@@ -11,11 +11,13 @@
 // with the first E term summed per element (S = sum of q y^3, one multiply-add with D at the end) and
 // q d stored beside d.  That is 28 FP64 instructions per pair instead of 36, and 9 instead of 18 for the
 // centre point: 102 instead of 126 per 7-point element, 177 instead of 216 per 12-point element (bare
-// loops on B200 with 30 per pair: 1.08e12 against 0.93e12 point-charge interactions/s).  The sums are the sums of Eq. 4.1 term by term;
+// loops on B200 with 30 per pair: 1.08e12 against 0.93e12 point-charge interactions/s).
+// The sums are the sums of Eq. 4.1 term by term;
 // only the rounding differs (|D|^2 + |d|^2 -+ 2 D.d loses nothing as long as |d| < |D|, i.e. at every
 // distance ratio a cubature rule is used at; the host takes this kernel only under policies whose
-// analytic limit for rectangles is >= 2).  Triangle rules have no such symmetry: triangles, and rectangles
-// in the pair-by-pair and analytic branches, go through the same code as in eval_adaptive_kernel.
+// analytic limit for rectangles is >= 2).  Triangle rules have no central symmetry; the 7-point one has its
+// points on the medians and is taken in a similar form (consume_tri7 below); the other triangle rules, and
+// all elements in the pair-by-pair and analytic branches, go through the same code as in eval_adaptive_kernel.
 //
 // Same execution model as kernels_eval.cuh (persistent CTAs, autonomous warps, atomic work queue, per-warp
 // double-buffered bulk-TMA windows).  A stage of the window holds whole elements in batch order; a small
@@ -118,17 +120,112 @@ __device__ __forceinline__ void consume_pairs(const double4* __restrict__ buf, i
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// The 7-point triangle rule (Table A2) the same way.  Its points are the centroid and two
+// orbits (a, b, b) over the three vertices, and by Eq. 3.3 a point with the large weight on vertex V is
+//     Q = a V + b (the other two) = C + kappa (V - C),   kappa = a - b,
+// so the six points sit on the three medians: with u_V = V - C and D = P - C,
+//     |P - Q|^2 = (|D|^2 + kappa^2 |u_V|^2) - 2 kappa D.u_V ,
+// D.u_V is shared by the two points of a median, D and |D|^2 by all seven points, and
+//     E += q y^3 (D - kappa u_V) = (q y^3) D + y^3 (-q kappa u_V)
+// with the first term summed per element.  14 FP64 instructions per point, 111 instead of 126 per element.
+__constant__ double c_tri7_kappa[2];  // kappa of the two orbits (0, 0: the table does not have this structure)
+__constant__ double c_tri7_w[3];      // weights: centroid, orbit 1, orbit 2
+constexpr int kTri7Units = 16;        // [C, q0] + 3 x ([u_V, 0] + 2 x ([-2 kappa, kappa^2 |u|^2, q, 0] [-q kappa u_V, 0]))
+constexpr int kClsTri7 = 6;
+
+// One thread per (element, slot): slot 0 the centroid record, slot 1..3 the records of one median.  Rectangles are skipped.
+__global__ void expand_tri7_kernel(int64_t n, const uint8_t* __restrict__ type, const double* __restrict__ verts,
+                                   const double4* __restrict__ cenL, const double* __restrict__ area,
+                                   const double* __restrict__ sigma, double* __restrict__ out) {
+  const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (idx >= 4 * n) return;
+  const int64_t e = idx >> 2;
+  const int slot = (int)(idx & 3);
+  if (type[e] != 0) return;
+  const double q = (sigma ? sigma[e] : 1.0) * area[e];  // q = sigma A (L143)
+  const double4 c = cenL[e];
+  double* blk = out + e * (int64_t)(4 * kTri7Units);
+  if (slot == 0) {
+    blk[0] = c.x; blk[1] = c.y; blk[2] = c.z; blk[3] = c_tri7_w[0] * q;
+    return;
+  }
+  const double* v = verts + 9 * e + 3 * (slot - 1);
+  const double ux = v[0] - c.x, uy = v[1] - c.y, uz = v[2] - c.z;
+  const double u2 = fma(ux, ux, fma(uy, uy, uz * uz));
+  double* p = blk + 4 + 20 * (slot - 1);
+  p[0] = ux; p[1] = uy; p[2] = uz; p[3] = 0.0;
+#pragma unroll
+  for (int o = 0; o < 2; ++o) {
+    const double k = c_tri7_kappa[o], qo = c_tri7_w[1 + o] * q;
+    double* r = p + 4 + 8 * o;
+    r[0] = -2.0 * k; r[1] = k * k * u2; r[2] = qo; r[3] = 0.0;
+    r[4] = -qo * k * ux; r[5] = -qo * k * uy; r[6] = -qo * k * uz; r[7] = 0.0;
+  }
+}
+
+template <int R>
+__device__ __forceinline__ void consume_tri7(const double4* __restrict__ buf, int nelem, const double (&px)[R], const double (&py)[R],
+                                             const double (&pz)[R], Accum<double, R, kModePhiE>& a) {
+  const double c375 = c_three_eighths;
+#pragma unroll 1
+  for (int e = 0; e < nelem; ++e) {
+    const double4* blk = buf + e * kTri7Units;
+    const double4 c = blk[0];
+    double Dx[R], Dy[R], Dz[R], D2[R], S[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      Dx[r] = __dsub_rn(px[r], c.x); Dy[r] = __dsub_rn(py[r], c.y); Dz[r] = __dsub_rn(pz[r], c.z);
+      const double yz = __fma_rn(Dy[r], Dy[r], __dmul_rn(Dz[r], Dz[r]));
+      D2[r] = __fma_rn(Dx[r], Dx[r], yz);
+      const double y = rsqrt_f64(D2[r], yz, c375);  // the centroid point
+      a.phi[r] = __fma_rn(c.w, y, a.phi[r]);
+      S[r] = __dmul_rn(c.w, __dmul_rn(y, __dmul_rn(y, y)));
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const double4 u = blk[1 + 5 * i];
+      double B[R];
+#pragma unroll
+      for (int r = 0; r < R; ++r) B[r] = __fma_rn(Dx[r], u.x, __fma_rn(Dy[r], u.y, __dmul_rn(Dz[r], u.z)));  // D.u_V
+#pragma unroll
+      for (int o = 0; o < 2; ++o) {
+        const double4 p0 = blk[2 + 5 * i + 2 * o], p1 = blk[3 + 5 * i + 2 * o];  // -2 kappa, kappa^2 |u|^2, q | -q kappa u
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const double A = __dadd_rn(D2[r], p0.y);
+          const double r2 = __fma_rn(p0.x, B[r], A);
+          const double y = rsqrt_f64(r2, A, c375);
+          a.phi[r] = __fma_rn(p0.z, y, a.phi[r]);
+          const double y3 = __dmul_rn(y, __dmul_rn(y, y));
+          S[r] = __fma_rn(p0.z, y3, S[r]);
+          a.ex[r] = __fma_rn(y3, p1.x, a.ex[r]);
+          a.ey[r] = __fma_rn(y3, p1.y, a.ey[r]);
+          a.ez[r] = __fma_rn(y3, p1.z, a.ez[r]);
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      a.ex[r] = __fma_rn(S[r], Dx[r], a.ex[r]);
+      a.ey[r] = __fma_rn(S[r], Dy[r], a.ey[r]);
+      a.ez[r] = __fma_rn(S[r], Dz[r], a.ez[r]);
+    }
+  }
+}
+
 struct PairedParams {
   AdaptiveParams ad;           // everything eval_adaptive_kernel takes (lvl_pts: the plain point records of every level)
   const double4* pair_pts[5];  // element blocks of the rectangles per level (n * pair_units(np) units; triangles' blocks unused)
   int pair_np[5];              // pairs per level, 0 = this level's rectangles are streamed as plain points
+  const double4* tri7_pts;     // element blocks of the triangles for the 7-point rule (n * kTri7Units units), or null
 };
 
 // per-warp bookkeeping in shared memory: the adaptive kernel's, plus the run table of each stage
 struct PairedScratch {
   WarpScratch s;
   unsigned long long n_saved;  // FP64 instructions per field point the paired form did NOT execute (against 18 per interaction)
-  uint32_t run[kStages][32];  // class (0..4: paired rectangles of that level, 5: point records) | offset << 3 | length << 11, in units
+  uint32_t run[kStages][32];  // class (0..4: paired rectangles of that level, 5: point records, 6: 7-point triangles) | offset << 3 | length << 11, in units
 };
 constexpr int kClsPoints = 5;
 
@@ -304,6 +401,12 @@ __global__ void __launch_bounds__(WARPS * 32, 1) eval_paired_kernel(const __grid
               src = pp.pair_pts[lvl] + e * estride;
               // 9 per element (D, |D|^2, S D), 9 for a centre point, 28 per pair - instead of 18 per point
               saved = 18 * realn - (9 + (realn > 2 * np ? 9 : 0) + 28 * np);
+            } else if (t == 0 && lvl == 1 && pp.tri7_pts) {  // a triangle with the 7-point rule in median form
+              cls = kClsTri7;
+              key = 16;
+              cnt = estride = kTri7Units;
+              src = pp.tri7_pts + e * kTri7Units;
+              saved = 18 * 7 - 111;
             } else {
               key = 8 + lvl;
               cnt = realn;
@@ -346,6 +449,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) eval_paired_kernel(const __grid
           case 2: consume_pairs<R, 6, false>(b, len / pair_units(6), w.px, w.py, w.pz, tot); break;
           case 3: consume_pairs<R, 8, true>(b, len / pair_units(8), w.px, w.py, w.pz, tot); break;
           case 4: consume_pairs<R, 16, true>(b, len / pair_units(16), w.px, w.py, w.pz, tot); break;
+          case kClsTri7: consume_tri7<R>(b, len / kTri7Units, w.px, w.py, w.pz, tot); break;
           default: consume_into<R, MODE>(b, len, w.px, w.py, w.pz, tot); break;
         }
       }

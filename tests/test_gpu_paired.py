@@ -110,6 +110,33 @@ def test_pairs_down_to_a_distance_ratio_of_two_and_the_fallback():
     g.close()
 
 
+@pytest.mark.parametrize("allow_upgrade", [0, 1])
+def test_triangles_only_seven_point_rule_on_the_medians(allow_upgrade):
+    """A triangle mesh (level-4 icosphere, 5120 triangles) takes the same kernel for its 7-point rule, whose
+    points are the centroid and two orbits on the medians (Q = C + kappa (V - C)); the other triangle rules
+    stay plain point records.  Field points from 0.5 to 400 sides off the surface: every band."""
+    etype, verts = synth.icosphere_elements(4, 1.0)
+    rng = np.random.default_rng(41)
+    sigma = rng.uniform(-1.0, 1.0, len(etype))
+    pts = _near_points(etype, verts, 22000, 42, 0.5, 400.0)
+    g = Gpu(etype, verts)
+    pol = g.b.bemcub_default_policy(True)
+    pol.allow_upgrade = allow_upgrade
+    phi, E = g.eval(sigma, pts, -1, policy=pol)
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_PAIRED
+    ref = oracle.evaluate(etype, verts, sigma, pts, -1, dr=oracle.default_policy(True), want_counts=True)
+    _split_parity(phi, E, ref, f"triangles upgrade={allow_upgrade}")
+    st = g.stats()
+    if not allow_upgrade:
+        assert st["point_interactions"] == int(ref["npi"].sum()) and st["analytic_pairs"] == int(ref["nana"].sum())
+    assert st["fp64_instructions"] < 18 * st["point_interactions"]          # the median form executed fewer
+    # without the 7-point level nothing is left to pair on a triangle mesh
+    pol.use_levels_mask = 0b111101
+    g.eval(sigma, pts, -1, policy=pol)
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_ADAPTIVE
+    g.close()
+
+
 def test_level_mask_and_reproducibility():
     """Rule levels switched off (7 -> 12, 17 -> 33 points) and repeated calls: same bits every time."""
     c = synth.config4(scale=0.005, ntracks=150, npts_per_track=150)
