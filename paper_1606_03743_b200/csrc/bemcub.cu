@@ -357,7 +357,9 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) 
 }
 
 // launch configuration of eval_paired_kernel (measured on config 4)
-constexpr int kPairedR = 3, kPairedWarps = 12;
+// (config 4 at full size, final loops: 5 field points per lane x 8 warps/SM 7187 ms, 6 x 8 7265, 3 x 12 7282, 4 x 8 7314; with fewer
+// field points the tiles must stay small: 3 x 12, then 1 x 12)
+constexpr int kPairedR = 5, kPairedWarps = 8, kPairedMidR = 3, kPairedMidWarps = 12;
 
 template <typename T, int R, int MODE = kModePhiE>
 int launch_fixed(bemcub_ctx* c, const FixedParams& fp, const SplitPlan& sp) {
@@ -409,7 +411,8 @@ int configure_kernels() {
       (rc = configure_adaptive<float, kModePhiE>()) || (rc = configure_adaptive<float, kModePhi>()) ||
       (rc = opt_in_smem(assemble_kernel, assemble_smem_bytes())) ||
       (rc = opt_in_smem(eval_paired_kernel<kPairedR, kPairedWarps>, paired_smem_bytes<kPairedWarps>())) ||
-      (rc = opt_in_smem(eval_paired_kernel<1, kPairedWarps>, paired_smem_bytes<kPairedWarps>())) ||
+      (rc = opt_in_smem(eval_paired_kernel<kPairedMidR, kPairedMidWarps>, paired_smem_bytes<kPairedMidWarps>())) ||
+      (rc = opt_in_smem(eval_paired_kernel<1, kPairedMidWarps>, paired_smem_bytes<kPairedMidWarps>())) ||
       (rc = opt_in_smem(inner_loop_kernel<4>, eval_smem_bytes<double>())))
     return rc;
   return BEMCUB_OK;
@@ -830,6 +833,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     }
   }
   SplitPlan sp = plan_splits(c, m, paired ? kPairedR : (grad ? 2 : 4), adaptive);  // R = 6 was measured: 2 % slower than R = 4 in the full kernel
+  if (paired && sp.R != kPairedR) sp = plan_splits(c, m, kPairedMidR, adaptive);  // 5, else 3, else 1 field points per lane
   if ((rc = ensure(c->partial, (size_t)sp.nsplit * (size_t)m * sizeof(double4)))) return rc;
   if (grad && (rc = ensure(c->partial_g, (size_t)sp.nsplit * (size_t)m * 48))) return rc;
   // a2: tiles of spatially close field points (adaptive mode; a fixed rule has nothing to choose)
@@ -913,11 +917,14 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
         pq.pair_pts[l] = (const double4*)c->pair64[l].ptr;
       }
       pq.tri7_pts = tri7 ? (const double4*)c->tri7.ptr : nullptr;
-      const int grid = (int)std::min<int64_t>(c->num_sms, (sp.nitems + kPairedWarps - 1) / kPairedWarps);
+      const int wpc = sp.R == kPairedR ? kPairedWarps : kPairedMidWarps;
+      const int grid = (int)std::min<int64_t>(c->num_sms, (sp.nitems + wpc - 1) / wpc);
       if (sp.R == kPairedR)
         eval_paired_kernel<kPairedR, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);
+      else if (sp.R == kPairedMidR)
+        eval_paired_kernel<kPairedMidR, kPairedMidWarps><<<grid, kPairedMidWarps * 32, paired_smem_bytes<kPairedMidWarps>(), c->stream>>>(pq);
       else
-        eval_paired_kernel<1, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);
+        eval_paired_kernel<1, kPairedMidWarps><<<grid, kPairedMidWarps * 32, paired_smem_bytes<kPairedMidWarps>(), c->stream>>>(pq);
       count_launch(c);
       CUDA_TRY(cudaGetLastError());
       rc = BEMCUB_OK;

@@ -1,8 +1,8 @@
 """-m gpu parity tests of eval_paired_kernel (csrc/kernels_paired.cuh): the distance-ratio evaluation with the
 rectangle rules' points taken in symmetric pairs (App. B, Eq. 3.2, Eq. 4.1).  The kernel is taken
 for FP64 Phi + E distance-ratio calls on meshes with rectangles (bemcub_last_path says which kernel ran):
-with 96-point tiles once there are field points enough - these cases are sized for that while the oracle
-still needs only seconds - and with 32-point tiles below (every adaptive case of test_gpu_eval.py on a
+with 160- or 96-point tiles once there are field points enough - these cases are sized for that while the
+oracle still needs only seconds - and with 32-point tiles below (every adaptive case of test_gpu_eval.py on a
 mixed mesh).  Same acceptance protocol as everywhere (gpu_common.py)."""
 import numpy as np
 import pytest
@@ -26,11 +26,12 @@ def _split_parity(phi, E, ref, what):
     return float(ephi.max()), float(eE.max())
 
 
-@pytest.mark.parametrize("allow_upgrade", [0, 1])
-def test_mixed_mesh_far_field(allow_upgrade):
-    """Config 4 in small (4000 rectangles + 1000 triangles, 22 500 track points, a ragged last tile): paired
-    rectangles of the 7- and 12-point rules next to plain triangle points in the same stages."""
-    c = synth.config4(scale=0.005, ntracks=150, npts_per_track=150)
+@pytest.mark.parametrize("allow_upgrade,ntracks", [(0, 150), (1, 150), (0, 191), (1, 191)])
+def test_mixed_mesh_far_field(allow_upgrade, ntracks):
+    """Config 4 in small (4000 rectangles + 1000 triangles; 22 500 track points: tiles of 96, or 36 481: tiles
+    of 160 - the launch configuration of the full-size bench - each with a ragged last tile): paired rectangles
+    of the 7- and 12-point rules next to median-form and plain triangle points in the same stages."""
+    c = synth.config4(scale=0.005, ntracks=ntracks, npts_per_track=ntracks)
     g = Gpu(c["etype"], c["verts"])
     pol = g.b.bemcub_default_policy(True)
     pol.allow_upgrade = allow_upgrade
