@@ -413,6 +413,9 @@ int configure_kernels() {
       (rc = opt_in_smem(eval_paired_kernel<kPairedR, kPairedWarps>, paired_smem_bytes<kPairedWarps>())) ||
       (rc = opt_in_smem(eval_paired_kernel<kPairedMidR, kPairedMidWarps>, paired_smem_bytes<kPairedMidWarps>())) ||
       (rc = opt_in_smem(eval_paired_kernel<1, kPairedMidWarps>, paired_smem_bytes<kPairedMidWarps>())) ||
+      (rc = opt_in_smem(eval_paired_kernel<kPairedR, kPairedWarps, kModePhi>, paired_smem_bytes<kPairedWarps>())) ||
+      (rc = opt_in_smem(eval_paired_kernel<kPairedMidR, kPairedMidWarps, kModePhi>, paired_smem_bytes<kPairedMidWarps>())) ||
+      (rc = opt_in_smem(eval_paired_kernel<1, kPairedMidWarps, kModePhi>, paired_smem_bytes<kPairedMidWarps>())) ||
       (rc = opt_in_smem(inner_loop_kernel<4>, eval_smem_bytes<double>())))
     return rc;
   return BEMCUB_OK;
@@ -801,11 +804,13 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   // density, a policy whose analytic branch covers the rectangles below a distance ratio of 2 at least (so
   // that |d| < |D| wherever a pair is evaluated), and field points enough for tiles of 32 kPairedR.
   bool paired = false, tri7 = false;
-  if (adaptive && !grad && precision == BEMCUB_F64 && out_E && !sigma_v && pol.map[5] == 5) {
+  if (adaptive && !grad && precision == BEMCUB_F64 && !sigma_v && pol.map[5] == 5) {
     if (c->has_rect && pol.dr[1][0] >= 2.0)
       for (int l = 0; l < 5; ++l) paired |= need[l] && c->pair_np[l] > 0;
     // ... and the 7-point triangle rule in median form, under the same condition on the triangles' analytic limit
-    tri7 = c->has_tri && c->tri7_ok && need[1] && pol.dr[0][0] >= 2.0;
+    // (a potential-only call on a mesh of triangles alone is typically the mat-vec of a solve: field points on the mesh
+    // itself, where the 7-point rule is never reached - the level-5 icosphere solve was 19 % slower through this kernel)
+    tri7 = c->has_tri && c->tri7_ok && need[1] && pol.dr[0][0] >= 2.0 && (out_E || paired);
     paired |= tri7;
     // (with fewer field points: one per lane, as the plain kernel does - plan_splits gives 3 or 1)
   }
@@ -919,12 +924,17 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
       pq.tri7_pts = tri7 ? (const double4*)c->tri7.ptr : nullptr;
       const int wpc = sp.R == kPairedR ? kPairedWarps : kPairedMidWarps;
       const int grid = (int)std::min<int64_t>(c->num_sms, (sp.nitems + wpc - 1) / wpc);
-      if (sp.R == kPairedR)
-        eval_paired_kernel<kPairedR, kPairedWarps><<<grid, kPairedWarps * 32, paired_smem_bytes<kPairedWarps>(), c->stream>>>(pq);
-      else if (sp.R == kPairedMidR)
-        eval_paired_kernel<kPairedMidR, kPairedMidWarps><<<grid, kPairedMidWarps * 32, paired_smem_bytes<kPairedMidWarps>(), c->stream>>>(pq);
-      else
-        eval_paired_kernel<1, kPairedMidWarps><<<grid, kPairedMidWarps * 32, paired_smem_bytes<kPairedMidWarps>(), c->stream>>>(pq);
+      const size_t sm_big = paired_smem_bytes<kPairedWarps>(), sm_mid = paired_smem_bytes<kPairedMidWarps>();
+      if (out_E) {
+        if (sp.R == kPairedR) eval_paired_kernel<kPairedR, kPairedWarps><<<grid, kPairedWarps * 32, sm_big, c->stream>>>(pq);
+        else if (sp.R == kPairedMidR) eval_paired_kernel<kPairedMidR, kPairedMidWarps><<<grid, kPairedMidWarps * 32, sm_mid, c->stream>>>(pq);
+        else eval_paired_kernel<1, kPairedMidWarps><<<grid, kPairedMidWarps * 32, sm_mid, c->stream>>>(pq);
+      } else {  // potential only (the mat-vec of bemcub_solve)
+        if (sp.R == kPairedR) eval_paired_kernel<kPairedR, kPairedWarps, kModePhi><<<grid, kPairedWarps * 32, sm_big, c->stream>>>(pq);
+        else if (sp.R == kPairedMidR)
+          eval_paired_kernel<kPairedMidR, kPairedMidWarps, kModePhi><<<grid, kPairedMidWarps * 32, sm_mid, c->stream>>>(pq);
+        else eval_paired_kernel<1, kPairedMidWarps, kModePhi><<<grid, kPairedMidWarps * 32, sm_mid, c->stream>>>(pq);
+      }
       count_launch(c);
       CUDA_TRY(cudaGetLastError());
       rc = BEMCUB_OK;

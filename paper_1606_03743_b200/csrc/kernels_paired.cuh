@@ -68,9 +68,11 @@ __global__ void expand_pairs_kernel(int64_t n, int level, int np, const uint8_t*
 }
 
 // `nelem` element blocks of NP pairs (+ centre if HC) applied to the lane's R field points.
-template <int R, int NP, bool HC>
+// MODE = kModePhi (potential only: the mat-vec of a BEM solve, any call without out_E): 18 per pair, 6 for the centre.
+template <int R, int NP, bool HC, int MODE>
 __device__ __forceinline__ void consume_pairs(const double4* __restrict__ buf, int nelem, const double (&px)[R], const double (&py)[R],
-                                              const double (&pz)[R], Accum<double, R, kModePhiE>& a) {
+                                              const double (&pz)[R], Accum<double, R, MODE>& a) {
+  constexpr bool kE = MODE != kModePhi;
   constexpr int UNITS = pair_units(NP);
   const double c375 = c_three_eighths;
 #pragma unroll 1
@@ -83,12 +85,11 @@ __device__ __forceinline__ void consume_pairs(const double4* __restrict__ buf, i
       Dx[r] = __dsub_rn(px[r], c.x); Dy[r] = __dsub_rn(py[r], c.y); Dz[r] = __dsub_rn(pz[r], c.z);
       const double yz = __fma_rn(Dy[r], Dy[r], __dmul_rn(Dz[r], Dz[r]));
       D2[r] = __fma_rn(Dx[r], Dx[r], yz);
+      S[r] = 0.0;
       if constexpr (HC) {  // the centre point: |P - Q| = |D|
         const double y = rsqrt_f64(D2[r], yz, c375);
         a.phi[r] = __fma_rn(c.w, y, a.phi[r]);
-        S[r] = __dmul_rn(c.w, __dmul_rn(y, __dmul_rn(y, y)));
-      } else {
-        S[r] = 0.0;
+        if constexpr (kE) S[r] = __dmul_rn(c.w, __dmul_rn(y, __dmul_rn(y, y)));
       }
     }
     constexpr int kUnroll = NP <= 3 ? NP : 1;  // (partial unrolling of the longer rules: no difference measured)
@@ -102,20 +103,24 @@ __device__ __forceinline__ void consume_pairs(const double4* __restrict__ buf, i
         const double rp = __fma_rn(-2.0, B, A), rm = __fma_rn(2.0, B, A);  // |P - (C + d)|^2, |P - (C - d)|^2
         const double yp = rsqrt_f64(rp, A, c375), ym = rsqrt_f64(rm, B, c375);
         a.phi[r] = __fma_rn(a0.w, __dadd_rn(yp, ym), a.phi[r]);
-        const double cp = __dmul_rn(yp, __dmul_rn(yp, yp)), cm = __dmul_rn(ym, __dmul_rn(ym, ym));
-        // E += q y+^3 (D - d) + q y-^3 (D + d) = q (y+^3 + y-^3) D + (y-^3 - y+^3) (q d)
-        S[r] = __fma_rn(a0.w, __dadd_rn(cp, cm), S[r]);
-        const double t = __dsub_rn(cm, cp);
-        a.ex[r] = __fma_rn(t, a1.y, a.ex[r]);
-        a.ey[r] = __fma_rn(t, a1.z, a.ey[r]);
-        a.ez[r] = __fma_rn(t, a1.w, a.ez[r]);
+        if constexpr (kE) {
+          const double cp = __dmul_rn(yp, __dmul_rn(yp, yp)), cm = __dmul_rn(ym, __dmul_rn(ym, ym));
+          // E += q y+^3 (D - d) + q y-^3 (D + d) = q (y+^3 + y-^3) D + (y-^3 - y+^3) (q d)
+          S[r] = __fma_rn(a0.w, __dadd_rn(cp, cm), S[r]);
+          const double t = __dsub_rn(cm, cp);
+          a.ex[r] = __fma_rn(t, a1.y, a.ex[r]);
+          a.ey[r] = __fma_rn(t, a1.z, a.ey[r]);
+          a.ez[r] = __fma_rn(t, a1.w, a.ez[r]);
+        }
       }
     }
+    if constexpr (kE) {
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      a.ex[r] = __fma_rn(S[r], Dx[r], a.ex[r]);
-      a.ey[r] = __fma_rn(S[r], Dy[r], a.ey[r]);
-      a.ez[r] = __fma_rn(S[r], Dz[r], a.ez[r]);
+      for (int r = 0; r < R; ++r) {
+        a.ex[r] = __fma_rn(S[r], Dx[r], a.ex[r]);
+        a.ey[r] = __fma_rn(S[r], Dy[r], a.ey[r]);
+        a.ez[r] = __fma_rn(S[r], Dz[r], a.ez[r]);
+      }
     }
   }
 }
@@ -164,9 +169,10 @@ __global__ void expand_tri7_kernel(int64_t n, const uint8_t* __restrict__ type, 
   }
 }
 
-template <int R>
+template <int R, int MODE>
 __device__ __forceinline__ void consume_tri7(const double4* __restrict__ buf, int nelem, const double (&px)[R], const double (&py)[R],
-                                             const double (&pz)[R], Accum<double, R, kModePhiE>& a) {
+                                             const double (&pz)[R], Accum<double, R, MODE>& a) {
+  constexpr bool kE = MODE != kModePhi;
   const double c375 = c_three_eighths;
 #pragma unroll 1
   for (int e = 0; e < nelem; ++e) {
@@ -180,7 +186,7 @@ __device__ __forceinline__ void consume_tri7(const double4* __restrict__ buf, in
       D2[r] = __fma_rn(Dx[r], Dx[r], yz);
       const double y = rsqrt_f64(D2[r], yz, c375);  // the centroid point
       a.phi[r] = __fma_rn(c.w, y, a.phi[r]);
-      S[r] = __dmul_rn(c.w, __dmul_rn(y, __dmul_rn(y, y)));
+      S[r] = kE ? __dmul_rn(c.w, __dmul_rn(y, __dmul_rn(y, y))) : 0.0;
     }
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
@@ -197,19 +203,23 @@ __device__ __forceinline__ void consume_tri7(const double4* __restrict__ buf, in
           const double r2 = __fma_rn(p0.x, B[r], A);
           const double y = rsqrt_f64(r2, A, c375);
           a.phi[r] = __fma_rn(p0.z, y, a.phi[r]);
-          const double y3 = __dmul_rn(y, __dmul_rn(y, y));
-          S[r] = __fma_rn(p0.z, y3, S[r]);
-          a.ex[r] = __fma_rn(y3, p1.x, a.ex[r]);
-          a.ey[r] = __fma_rn(y3, p1.y, a.ey[r]);
-          a.ez[r] = __fma_rn(y3, p1.z, a.ez[r]);
+          if constexpr (kE) {
+            const double y3 = __dmul_rn(y, __dmul_rn(y, y));
+            S[r] = __fma_rn(p0.z, y3, S[r]);
+            a.ex[r] = __fma_rn(y3, p1.x, a.ex[r]);
+            a.ey[r] = __fma_rn(y3, p1.y, a.ey[r]);
+            a.ez[r] = __fma_rn(y3, p1.z, a.ez[r]);
+          }
         }
       }
     }
+    if constexpr (kE) {
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      a.ex[r] = __fma_rn(S[r], Dx[r], a.ex[r]);
-      a.ey[r] = __fma_rn(S[r], Dy[r], a.ey[r]);
-      a.ez[r] = __fma_rn(S[r], Dz[r], a.ez[r]);
+      for (int r = 0; r < R; ++r) {
+        a.ex[r] = __fma_rn(S[r], Dx[r], a.ex[r]);
+        a.ey[r] = __fma_rn(S[r], Dy[r], a.ey[r]);
+        a.ez[r] = __fma_rn(S[r], Dz[r], a.ez[r]);
+      }
     }
   }
 }
@@ -234,9 +244,9 @@ constexpr size_t paired_smem_bytes() {
   return (size_t)WARPS * (kStages * kBuf * sizeof(double4) + kStages * 8 + sizeof(PairedScratch));
 }
 
-template <int R, int WARPS>
+template <int R, int WARPS, int MODE = kModePhiE>
 __global__ void __launch_bounds__(WARPS * 32, 1) eval_paired_kernel(const __grid_constant__ PairedParams pp) {
-  constexpr int MODE = kModePhiE;
+  static_assert(MODE == kModePhiE || MODE == kModePhi, "Phi + E or Phi only");
   typedef double4 P4;
   const AdaptiveParams& p = pp.ad;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -400,13 +410,15 @@ __global__ void __launch_bounds__(WARPS * 32, 1) eval_paired_kernel(const __grid
               cnt = estride = pair_units(np);
               src = pp.pair_pts[lvl] + e * estride;
               // 9 per element (D, |D|^2, S D), 9 for a centre point, 28 per pair - instead of 18 per point
-              saved = 18 * realn - (9 + (realn > 2 * np ? 9 : 0) + 28 * np);
+              // (Phi only: 6, 6 and 18 instead of 12 per point)
+              saved = MODE == kModePhi ? 12 * realn - (6 + (realn > 2 * np ? 6 : 0) + 18 * np)
+                                       : 18 * realn - (9 + (realn > 2 * np ? 9 : 0) + 28 * np);
             } else if (t == 0 && lvl == 1 && pp.tri7_pts) {  // a triangle with the 7-point rule in median form
               cls = kClsTri7;
               key = 16;
               cnt = estride = kTri7Units;
               src = pp.tri7_pts + e * kTri7Units;
-              saved = 18 * 7 - 111;
+              saved = MODE == kModePhi ? 12 * 7 - 69 : 18 * 7 - 111;
             } else {
               key = 8 + lvl;
               cnt = realn;
@@ -444,12 +456,12 @@ __global__ void __launch_bounds__(WARPS * 32, 1) eval_paired_kernel(const __grid
         const P4* b = win + stage * kBuf + ((ent >> 3) & 255u);
         const int len = (int)(ent >> 11);
         switch (ent & 7u) {
-          case 0: consume_pairs<R, 2, false>(b, len / pair_units(2), w.px, w.py, w.pz, tot); break;
-          case 1: consume_pairs<R, 3, true>(b, len / pair_units(3), w.px, w.py, w.pz, tot); break;
-          case 2: consume_pairs<R, 6, false>(b, len / pair_units(6), w.px, w.py, w.pz, tot); break;
-          case 3: consume_pairs<R, 8, true>(b, len / pair_units(8), w.px, w.py, w.pz, tot); break;
-          case 4: consume_pairs<R, 16, true>(b, len / pair_units(16), w.px, w.py, w.pz, tot); break;
-          case kClsTri7: consume_tri7<R>(b, len / kTri7Units, w.px, w.py, w.pz, tot); break;
+          case 0: consume_pairs<R, 2, false, MODE>(b, len / pair_units(2), w.px, w.py, w.pz, tot); break;
+          case 1: consume_pairs<R, 3, true, MODE>(b, len / pair_units(3), w.px, w.py, w.pz, tot); break;
+          case 2: consume_pairs<R, 6, false, MODE>(b, len / pair_units(6), w.px, w.py, w.pz, tot); break;
+          case 3: consume_pairs<R, 8, true, MODE>(b, len / pair_units(8), w.px, w.py, w.pz, tot); break;
+          case 4: consume_pairs<R, 16, true, MODE>(b, len / pair_units(16), w.px, w.py, w.pz, tot); break;
+          case kClsTri7: consume_tri7<R, MODE>(b, len / kTri7Units, w.px, w.py, w.pz, tot); break;
           default: consume_into<R, MODE>(b, len, w.px, w.py, w.pz, tot); break;
         }
       }

@@ -44,10 +44,14 @@ def test_mixed_mesh_far_field(allow_upgrade, ntracks):
         assert st["point_interactions"] >= int(ref["npi"].sum())
     else:
         assert st["point_interactions"] == int(ref["npi"].sum()) and st["analytic_pairs"] == int(ref["nana"].sum())
-    # Phi only and the field gradient are not paired: the call falls back to the plain kernel, same numbers
+    # potential only (out_E = NULL, the mat-vec of a solve): the paired / median forms without their field part
     phi2, _ = g.eval(c["sigma"], c["pts"], -1, policy=pol, want_E=False)
-    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_ADAPTIVE
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_PAIRED
     assert np.max(np.abs(phi2 - ref["phi"]) / ref["Sphi"]) <= TOL_F64
+    st2 = g.stats()
+    assert st2["fp64_instructions"] < 12 * st2["point_interactions"]
+    if not allow_upgrade:
+        assert st2["point_interactions"] == int(ref["npi"].sum())
     g.close()
 
 
