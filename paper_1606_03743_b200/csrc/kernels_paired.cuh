@@ -19,6 +19,9 @@
 // points on the medians and is taken in a similar form (consume_tri7 below); the other triangle rules, and
 // all elements in the pair-by-pair and analytic branches, go through the same code as in eval_adaptive_kernel.
 //
+// Potential-only calls (out_E = NULL: the mat-vec of a BEM solve, L34) take the same forms without their field
+// part: 18 instead of 24 FP64 instructions per pair, 6 instead of 12 for a centre point.
+//
 // Same execution model as kernels_eval.cuh (persistent CTAs, autonomous warps, atomic work queue, per-warp
 // double-buffered bulk-TMA windows).  A stage of the window holds whole elements in batch order; a small
 // run table beside it says which stretches are paired rectangles of one level (element blocks: centre
