@@ -82,7 +82,8 @@ enum {
   BEMCUB_ERR_CUDA = -5,
   BEMCUB_ERR_NOMEM = -6,
   BEMCUB_ERR_NO_ELEMENTS = -7,        /* eval/assemble before a successful set_elements    */
-  BEMCUB_ERR_NOT_CONVERGED = -8       /* bemcub_solve: mat-vec limit reached (outputs valid) */
+  BEMCUB_ERR_NOT_CONVERGED = -8,      /* bemcub_solve: mat-vec limit reached (outputs valid) */
+  BEMCUB_ERR_FIXED_SCRATCH = -9       /* bemcub_eval_few_noalloc: more than its fixed scratch holds */
 };
 
 /* Distance-ratio policy (Sec. 4).  dr[t][b], t = element type, are the UPPER distance-ratio
@@ -161,6 +162,36 @@ int bemcub_set_elements(bemcub_ctx* ctx, int64_t n, const uint8_t* type, const d
  * m = 0 is a no-op.  Asynchronous. */
 int bemcub_eval(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
                 int64_t m, const double* field_pts, double* out_phi, double* out_E, int precision);
+
+/* bemcub_eval for callers that are not allowed to allocate device memory: same arguments (FP64), same
+ * kernel, same grid and therefore the same bits as a bemcub_eval call with m <= 64, but no cudaMalloc,
+ * cudaFree or allocating library call is made - neither on this call nor on any later one.
+ *   Who needs it.  A particle tracker (L32) asks for the field at one point after the other from inside
+ *   its integration loop.  Such a loop often runs where allocating is forbidden or ruinous: in a host
+ *   application that has handed all device memory to its own pool, next to other streams that a
+ *   cudaMalloc would stall (it synchronises the whole device), or under a latency budget that one
+ *   allocation would break.  bemcub_eval may allocate whenever a call is the first of its shape
+ *   (partial sums) or brings a sigma (the ctx keeps a copy); this call never does.
+ *   How.  The partial sums of the CTAs and the counters of the kernel live in one array that is part of
+ *   the library image: 655,872 bytes (641 KB) on EVERY GPU on which this process has loaded the
+ *   library, held until the process exits, whether or not this function is ever called.
+ *   Limits.  1 <= m <= 64 field points per call (m = 0 is a no-op) on a device of at most 160 SMs;
+ *   beyond either, BEMCUB_ERR_FIXED_SCRATCH and nothing is enqueued - split the points over several calls.
+ *   sigma[n] must be passed (no NULL reuse): it is read in place, the ctx keeps nothing of this call, and
+ *   the kept sigma / expanded points of earlier bemcub_eval calls stay as they were.  out_phi is required,
+ *   out_E may be NULL.  The mesh is the one of bemcub_set_elements (which does allocate: set the mesh up
+ *   before entering the region that must not).  bemcub_get_stats counts the launch but not its
+ *   interactions; bemcub_last_path and the timing calls do not see it.
+ *   First call on a device.  It asks the runtime for the array's address on that device (with the device
+ *   made current) and remembers it for the process; make this first call during set-up, before any
+ *   stream capture begins.
+ *   Sharing.  There is ONE array per GPU for all contexts, streams and host threads of the process.  A call
+ *   clears the counters it needs (stream-ordered) and overwrites the sums of the previous call, so calls
+ *   that follow one another on one stream are safe; two calls that can be on the same GPU at the same time
+ *   (different streams, or different ctxs on different streams) corrupt each other's results - serialise
+ *   them.  Asynchronous, like bemcub_eval. */
+int bemcub_eval_few_noalloc(bemcub_ctx* ctx, const double* sigma, int rule_id, const bemcub_policy* host_policy,
+                            int64_t m, const double* field_pts, double* out_phi, double* out_E);
 
 /* The single-element integrator (the paper's innermost layer, L193-196 item a; the unit of its
  * accuracy protocol, L68 and L149, Figs. 8-10): element k seen from field point k, k < npairs, NO

@@ -59,6 +59,7 @@ def _load() -> C.CDLL:
         "bemcub_default_policy": [PP, C.c_int],
         "bemcub_set_elements": [vp, i64, vp, vp],
         "bemcub_eval": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
+        "bemcub_eval_few_noalloc": [vp, vp, C.c_int, PP, i64, vp, vp, vp],
         "bemcub_eval_gradient": [vp, vp, C.c_int, PP, i64, vp, vp, vp, vp],
         "bemcub_eval_pairs": [vp, i64, vp, vp, vp, C.c_int, PP, vp, vp, vp, C.c_int],
         "bemcub_eval_linear": [vp, vp, C.c_int, PP, i64, vp, vp, vp, C.c_int],
@@ -92,7 +93,7 @@ def _load() -> C.CDLL:
 
 
 _lib = _load()
-EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval",
+EXPORTED = ["bemcub_create", "bemcub_destroy", "bemcub_default_policy", "bemcub_set_elements", "bemcub_eval", "bemcub_eval_few_noalloc",
             "bemcub_eval_gradient", "bemcub_eval_linear", "bemcub_eval_pairs", "bemcub_solve", "bemcub_solve_storage", "bemcub_matvec",
             "bemcub_assemble", "bemcub_assemble_rows", "bemcub_set_elements_host", "bemcub_eval_host",
             "bemcub_rule_info", "bemcub_rule_points", "bemcub_expand_points", "bemcub_get_geometry",
@@ -183,6 +184,19 @@ def bemcub_set_elements(ctx, n: int, etype, verts) -> None:
 def bemcub_eval(ctx, sigma, rule_id: int, policy, m: int, field_pts, out_phi, out_E, precision: int = F64) -> None:
     _check(_lib.bemcub_eval(ctx, _dptr(sigma), rule_id, _policy_ptr(policy), m, _dptr(field_pts), _dptr(out_phi),
                             _dptr(out_E), precision), "bemcub_eval")
+
+
+ERR_FIXED_SCRATCH = -9
+NOALLOC_MAX_M = 64
+
+
+def bemcub_eval_few_noalloc(ctx, sigma, rule_id: int, policy, m: int, field_pts, out_phi, out_E) -> None:
+    """bemcub_eval for at most NOALLOC_MAX_M field points without any device allocation by the library
+    (for tracking loops that run where cudaMalloc is off limits: memory owned by the application's pool,
+    or a device-wide stall nobody can afford).  Its scratch is one fixed array per GPU shared by every
+    ctx and stream: do not let two such calls run on a GPU at the same time.  See include/bemcub.h."""
+    _check(_lib.bemcub_eval_few_noalloc(ctx, _dptr(sigma), rule_id, _policy_ptr(policy), m, _dptr(field_pts),
+                                        _dptr(out_phi), _dptr(out_E)), "bemcub_eval_few_noalloc")
 
 
 def bemcub_eval_gradient(ctx, sigma, rule_id: int, policy, m: int, field_pts, out_phi, out_E, out_G) -> None:

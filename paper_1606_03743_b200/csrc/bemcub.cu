@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include <cuda_runtime.h>
@@ -496,6 +497,8 @@ const char* bemcub_strerror(int code) {
     case BEMCUB_ERR_NOMEM: return "out of device memory";
     case BEMCUB_ERR_NO_ELEMENTS: return "no mesh: call bemcub_set_elements first";
     case BEMCUB_ERR_NOT_CONVERGED: return "iteration stopped at the mat-vec limit before reaching the tolerance";
+    case BEMCUB_ERR_FIXED_SCRATCH:
+      return "bemcub_eval_few_noalloc: beyond its fixed scratch (at most 64 field points per call, devices of at most 160 SMs)";
   }
   return "unknown error code";
 }
@@ -1322,3 +1325,111 @@ int bemcub_reset_stats(bemcub_ctx* c) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// bemcub_eval_few_noalloc (include/bemcub.h): the few-point evaluation for callers that must not
+// allocate.  eval_few_kernel needs two pieces of global scratch - the CTAs' partial sums and the
+// counters by which the last CTA of a pass knows it is the last - which bemcub_eval takes from
+// ctx-owned cudaMalloc memory.  Here they live in the array below: part of the library's image, put
+// on every GPU that loads the library and kept there until the process exits (about 641 KB each).
+//   bytes [0, 512)      counters: interaction tallies, then one "CTAs done" counter per pass; the
+//                       kernel counts up from zero, so they are cleared before every launch
+//   bytes [512, end)    partial sums [CTA][m] (double4); every CTA writes all of its entries before
+//                       the last one reads them, so what the previous call left there never matters
+// The array is shared by every ctx and every stream of the process: two calls that are on the GPU
+// at the same time would count in each other's counters and overwrite each other's sums.
+constexpr int kNoAllocMaxM = kFewMaxM;  // 64 field points per call
+constexpr int kNoAllocMaxCtas = 320;    // two CTAs per SM, as bemcub_eval launches them: devices of up to 160 SMs
+constexpr size_t kNoAllocCounterBytes = 512;
+constexpr size_t kNoAllocBytes = kNoAllocCounterBytes + (size_t)kNoAllocMaxCtas * kNoAllocMaxM * sizeof(double4);
+static_assert(kCounterSlots * sizeof(unsigned long long) <= kNoAllocCounterBytes, "counter block too small");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+namespace {
+
+// In host code `g_noalloc_scratch` is only a handle for the runtime, not somewhere a kernel can write:
+// the array's address on a given GPU comes from cudaGetSymbolAddress, asked once per device with that
+// device current, and that address is what the kernel gets.
+constexpr int kNoAllocMaxDevices = 64;
+void* g_noalloc_addr[kNoAllocMaxDevices] = {};
+std::mutex g_noalloc_mutex;
+
+int noalloc_scratch_of_current_device(int device, unsigned char** out) {
+  if (device < 0 || device >= kNoAllocMaxDevices) return BEMCUB_ERR_INVALID_ARG;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_addr[device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p) {
+      cudaGetLastError();
+      return BEMCUB_ERR_CUDA;
+    }
+    g_noalloc_addr[device] = p;
+  }
+  *out = static_cast<unsigned char*>(g_noalloc_addr[device]);
+  return BEMCUB_OK;
+}
+
+}  // namespace
+
+extern "C" int bemcub_eval_few_noalloc(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_policy* host_policy,
+                                       int64_t m, const double* field_pts, double* out_phi, double* out_E) {
+  if (!c || m < 0) return BEMCUB_ERR_INVALID_ARG;
+  if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
+  if (rule_id < -1 || rule_id > 4) return BEMCUB_ERR_BAD_RULE;
+  const bool adaptive = rule_id == BEMCUB_RULE_ADAPTIVE;
+  PolicyDev pol;
+  if (adaptive) {
+    const int rc = build_policy(host_policy, &pol);
+    if (rc) return rc;
+  }
+  if (m == 0) return BEMCUB_OK;
+  const int blocks = c->num_sms * 2;  // the grid of bemcub_eval's few-point route: same sums in the same order
+  if (m > kNoAllocMaxM || blocks > kNoAllocMaxCtas) return BEMCUB_ERR_FIXED_SCRATCH;
+  if (!field_pts || !out_phi || (c->n > 0 && !sigma)) return BEMCUB_ERR_INVALID_ARG;
+  DeviceGuard g(c->device);
+  if (!g.ok) return BEMCUB_ERR_CUDA;
+  if (c->n == 0) {  // empty mesh: zero potential and field
+    CUDA_TRY(cudaMemsetAsync(out_phi, 0, (size_t)m * 8, c->stream));
+    if (out_E) CUDA_TRY(cudaMemsetAsync(out_E, 0, (size_t)m * 24, c->stream));
+    return BEMCUB_OK;
+  }
+  unsigned char* scratch = nullptr;
+  const int rc = noalloc_scratch_of_current_device(c->device, &scratch);
+  if (rc) return rc;
+
+  FewParams fw;
+  fw.cenL = (const double4*)c->cenL.ptr;
+  fw.type = (const uint8_t*)c->type.ptr;
+  fw.verts = (const double*)c->verts.ptr;
+  fw.sigma = sigma;  // read in place: nothing of this call is kept in the ctx
+  fw.n = c->n;
+  if (adaptive) fw.pol = pol;
+  fw.rule = adaptive ? -1 : rule_id;
+  fw.field = field_pts;
+  fw.m = m;
+  fw.counters = reinterpret_cast<unsigned long long*>(scratch);
+  fw.done = reinterpret_cast<unsigned*>(fw.counters + 8);
+  fw.partial = reinterpret_cast<double4*>(scratch + kNoAllocCounterBytes);
+  fw.area = (const double*)c->area.ptr;
+  fw.sigma_v = nullptr;
+  fw.k = coulomb_k();
+  fw.out_phi = out_phi;
+  fw.out_E = out_E;
+  CUDA_TRY(cudaMemsetAsync(scratch, 0, kNoAllocCounterBytes, c->stream));
+  const int per_pass = m >= 3 ? kFewM : (int)m;
+  const dim3 grid((unsigned)blocks, (unsigned)((m + per_pass - 1) / per_pass));
+  const int threads = kFewWarps * 32;
+  if (out_E) {
+    if (per_pass == 1) eval_few_kernel<kModePhiE, 1><<<grid, threads, 0, c->stream>>>(fw);
+    else if (per_pass == 2) eval_few_kernel<kModePhiE, 2><<<grid, threads, 0, c->stream>>>(fw);
+    else eval_few_kernel<kModePhiE, kFewM><<<grid, threads, 0, c->stream>>>(fw);
+  } else {
+    if (per_pass == 1) eval_few_kernel<kModePhi, 1><<<grid, threads, 0, c->stream>>>(fw);
+    else if (per_pass == 2) eval_few_kernel<kModePhi, 2><<<grid, threads, 0, c->stream>>>(fw);
+    else eval_few_kernel<kModePhi, kFewM><<<grid, threads, 0, c->stream>>>(fw);
+  }
+  c->stats.kernel_launches += 1;
+  CUDA_TRY(cudaGetLastError());
+  return BEMCUB_OK;
+}
