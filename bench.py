@@ -43,8 +43,30 @@ FLOP_PER_INTERACTION_GRAD = 41  # + 5 DFMA + 4 DMUL + 1 DADD for the gradient su
 FP64_LANES_PER_SM = 64          # B200: one FP64 warp instruction per scheduler every 2 cycles (profiles/r2_issue_model.md)
 METRIC = "FP64 Phi+E element.point interactions/s"
 UNIT = "element.point interactions/s"
-# ncu counter of the committed capture of the bench's own launch configuration (not measured by this run)
-NCU_PIPE = {"cfg4": ("profiles/r2_cfg4_full_eval_paired_counters.csv", "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed")}
+# committed ncu capture of ONE launch of the bench's own launch configuration (hardware counters; not measured by this run)
+NCU_CAPTURE = {"cfg4": ("profiles/r2_cfg4_full_eval_paired_counters.csv", "eval_paired_kernel")}
+NCU_PIPE_METRIC = "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed"
+LINE_LIMIT = 4096               # bytes of the stdout record (the driver keeps a tail of stdout: round 2's 20 KB line did not parse)
+
+
+def ncu_capture(workload: str, kernel: str):
+    """{metric: value} of the committed counter capture of this workload's dominant kernel, or None."""
+    import csv
+    ent = NCU_CAPTURE.get(workload)
+    if not ent or not kernel.startswith(ent[1]):
+        return None
+    out = {}
+    try:
+        with open(os.path.join(ROOT, ent[0]), newline="") as f:
+            for row in csv.reader(f):
+                if len(row) >= 3 and ent[1] in " ".join(row[:-3]):
+                    try:
+                        out[row[-3]] = float(row[-1].replace(",", ""))
+                    except ValueError:
+                        pass
+    except OSError:
+        return None
+    return {"file": ent[0], "metrics": out} if out else None
 
 
 def parse_args():
@@ -67,6 +89,9 @@ def parse_args():
     ap.add_argument("--store-matrix", action="store_true",
                     help="--workload solve: let the solve keep the matrix (bemcub_solve_storage): one matrix fill, GEMV mat-vecs")
     ap.add_argument("--out", default=None, help="--workload accuracy: text file for the tables")
+    ap.add_argument("--detail-out", default=os.path.join("gpurun_out", "bench_detail.json"),
+                    help="file for the full record (peak sweep, definitions, the secondary runs with their rooflines); the "
+                         "stdout line is the compact contract record only")
     return ap.parse_args()
 
 
@@ -265,7 +290,7 @@ def run_reference(args, rank: int):
         "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
-    print(json.dumps(line), flush=True)
+    print(json.dumps(contract_line(line)), flush=True)
 
 
 # --------------------------------------------------------------------------------------------
@@ -288,34 +313,37 @@ def nominal_tflops(num_sms: int, sm_mhz: float) -> float:
     return FP64_LANES_PER_SM * num_sms * 2.0 * sm_mhz * 1e6 / 1e12
 
 
-def roofline_block(kernel: str, k_ms: float, step_ms: float, inter: float, inter_own, fpi: int, ipi: int, peak: dict,
+def roofline_block(kernel: str, k_ms: float, step_ms: float, inter: float, inter_own, fpi: int, ipi: float, peak: dict,
                    num_sms: int, kernel_mhz, smi_mhz) -> dict:
-    """FLOP fractions of the dominant kernel four ways (executed / the method's own work, against the
-    measured peak / the nominal rate at the clock the kernel ran at) and the arithmetic pipe fraction."""
-    ach = inter * fpi / (k_ms * 1e-3) / 1e12
+    """The dominant kernel against the FP64-ALU roofline.  `achieved` / `frac` count the ALGORITHMIC work (SURVEY.md
+    section 8(d)): the point-charge interactions the per-pair distance-ratio policy asks for (`inter_own`; a fixed rule:
+    all of them) x `fpi` flop each.  `frac_executed` counts the interactions the tiles really evaluated (a few per cent
+    more: upgraded tiles), `fp64_issue_frac` the FP64 instructions really executed against the measured issue rate."""
+    sec = k_ms * 1e-3
+    base = inter if inter_own is None else inter_own
+    ach = base * fpi / sec / 1e12
+    ach_exec = inter * fpi / sec / 1e12
     clock = kernel_mhz or smi_mhz or peak["sm_mhz"]
     nom = nominal_tflops(num_sms, clock)
-    r = {"bound": "alu", "achieved": ach, "peak": peak["tflops"], "unit": "TFLOP/s", "frac": ach / peak["tflops"],
-         "traffic": None,
-         "traffic_source": "not measured by this run; dram__bytes of one launch are in the ncu captures under profiles/ (ALU-bound: "
-                           "the bytes do not set the time)",
-         "kernel": kernel, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / step_ms if step_ms else None,
-         "point_interactions_per_launch": inter, "flop_per_interaction": fpi, "fp64_inst_per_interaction": ipi,
-         "frac_nominal": ach / nom, "nominal_tflops": nom,
-         "nominal_def": f"{num_sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {clock:.0f} MHz "
-                        f"({'SM clock read inside the kernel: cycle counter / global timer' if kernel_mhz else 'nvidia-smi median'})",
-         "peak_over_nominal": peak["tflops"] / nom, "peak_source": peak["source"], "peak_best_variant": peak["best"],
-         "kernel_sm_mhz": kernel_mhz,
-         "fp64_issue_frac_arith": inter * ipi / (k_ms * 1e-3) / peak["fp64_inst_per_s"],
-         "fp64_issue_frac_arith_def": "FP64 instructions of the interactions executed (interactions x instructions per interaction) "
-                                      "/ kernel time / measured issue rate: arithmetic, not a hardware counter"}
-    if inter_own is not None:
-        own = inter_own * fpi / (k_ms * 1e-3) / 1e12
-        r.update({"frac_own_work": own / peak["tflops"], "frac_own_work_nominal": own / nom,
-                  "own_work_interactions_per_launch": inter_own,
-                  "own_work_def": "point-charge interactions of the per-pair distance-ratio policy (what the method asks for; "
-                                  "device counter of one untimed call with allow_upgrade = 0); the tiles execute a few per cent more"})
-    return r
+    return {"bound": "alu", "achieved": ach, "peak": peak["tflops"], "unit": "TFLOP/s", "frac": ach / peak["tflops"],
+            "traffic": None,
+            "traffic_source": "not measured by this run; ALU-bound (the bytes do not set the time); ncu captures are under profiles/",
+            "kernel": kernel, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / step_ms if step_ms else None,
+            "work": "own" if inter_own is not None else "executed",
+            "work_def": "point-charge interactions of the per-pair distance-ratio policy (device counter of one untimed call with "
+                        "allow_upgrade = 0; fixed rule: every interaction) x flop_per_interaction: algorithm-equivalent flop, whatever "
+                        "instruction sequence the kernel used for them",
+            "interactions_per_launch": base, "interactions_executed_per_launch": inter,
+            "flop_per_interaction": fpi, "fp64_inst_per_interaction": ipi,
+            "achieved_executed": ach_exec, "frac_executed": ach_exec / peak["tflops"],
+            "frac_nominal": ach / nom, "frac_executed_nominal": ach_exec / nom, "nominal_tflops": nom,
+            "nominal_def": f"{num_sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x {clock:.0f} MHz "
+                           f"({'SM clock read inside the kernel: cycle counter / global timer' if kernel_mhz else 'nvidia-smi median'})",
+            "peak_over_nominal": peak["tflops"] / nom, "peak_source": peak["source"], "peak_best_variant": peak["best"],
+            "kernel_sm_mhz": kernel_mhz,
+            "fp64_issue_frac": inter * ipi / sec / peak["fp64_inst_per_s"],
+            "fp64_issue_frac_def": "FP64 instructions executed (interactions executed x instructions per interaction, device tally) "
+                                   "/ kernel time / measured FP64 issue rate"}
 
 
 def kernel_clock_mhz(st: dict):
@@ -389,7 +417,8 @@ def secondary_block(args, b, torch, dev_index: int, peak: dict, num_sms: int, ba
         t = r.timed(step, steps_for(probe["ms"]), 3, barrier, dev_index, period_ms=100)
         st = t["stats"]
         inter = float(st["point_interactions"])
-        entry = {"workload": c["desc"], "dtype": precision_name, "ms_per_step": t["ms"], "kernel_ms": t["kernel_ms"],
+        entry = {"name": "%s rule level %d %s" % (name, rule, precision_name),
+                 "workload": c["desc"], "dtype": precision_name, "ms_per_step": t["ms"], "kernel_ms": t["kernel_ms"],
                  "value": float(r.n) * r.m / (t["ms"] * 1e-3), "unit": UNIT, "clocks": t["clocks"],
                  "points_per_pair": inter / (float(r.n) * r.m)}
         if prec == b.F64:
@@ -421,7 +450,7 @@ def secondary_block(args, b, torch, dev_index: int, peak: dict, num_sms: int, ba
     roof = roofline_block("assemble_kernel", t["kernel_ms"], t["ms"], inter, own, FLOP_PER_INTERACTION_PHI, 12, peak, num_sms,
                           kernel_clock_mhz(st), t["clocks"].get("sm_mhz"))
     roof["store_stream_gb_s"] = float(r.n) * r.n * 8 / (t["kernel_ms"] * 1e-3) / 1e9
-    entry = {"workload": c3["desc"], "dtype": "f64", "ms_per_step": t["ms"], "kernel_ms": t["kernel_ms"],
+    entry = {"name": "cfg3 matrix fill 20480^2", "workload": c3["desc"], "dtype": "f64", "ms_per_step": t["ms"], "kernel_ms": t["kernel_ms"],
              "value": float(r.n) * r.n / (t["ms"] * 1e-3), "unit": "matrix entries/s", "steps": 300, "clocks": t["clocks"],
              "points_per_entry": inter / (float(r.n) * r.n), "points_per_entry_own_work": own / (float(r.n) * r.n),
              "analytic_entries_per_row": st["analytic_pairs"] / float(r.n), "roofline": roof}
@@ -437,6 +466,86 @@ def secondary_block(args, b, torch, dev_index: int, peak: dict, num_sms: int, ba
             out.append(fixed_rule_entry("cfg2", rule, prec))
     out.append(fixed_rule_entry("cfg5", 1, "f64"))
     return out
+
+
+# --------------------------------------------------------------------------------------------
+def _pick(d, keys):
+    return None if d is None else {k: d[k] for k in keys if k in d}
+
+
+def _clip(v, n: int):
+    return v if not isinstance(v, str) or len(v) <= n else v[:n - 3] + "..."
+
+
+def _sig(v, digits: int = 6):
+    """Floats to `digits` significant digits (the record is read by people and by a tail-limited log)."""
+    if isinstance(v, float):
+        return float(f"{v:.{digits}g}")
+    if isinstance(v, dict):
+        return {k: _sig(x, digits) for k, x in v.items()}
+    if isinstance(v, list):
+        return [_sig(x, digits) for x in v]
+    return v
+
+
+def contract_line(full: dict, detail_path=None) -> dict:
+    """The ONE stdout record of the driver contract from the full record: the contract keys, short strings, no
+    sweeps, no definitions; the secondary runs as one short row each.  Stays below LINE_LIMIT bytes."""
+    top = ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+           "vs_baseline", "dtype", "data", "pct_fp64_peak", "gpu_launches")
+    line = {k: full[k] for k in top if k in full}
+    cfg = dict(full.get("config") or {})
+    for k in cfg:
+        cfg[k] = _clip(cfg[k], 230 if k == "workload" else 90)
+    line["config"] = cfg
+    line["clocks"] = _pick(full.get("clocks"), ("sm_mhz", "sm_max_mhz", "power_w_max", "samples", "reasons"))
+    line["e2e"] = _pick(full.get("e2e"), ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step", "api", "note"))
+    if line["e2e"] and "api" in line["e2e"]:
+        line["e2e"]["api"] = _clip(line["e2e"]["api"], 80)
+    roof = _pick(full.get("roofline"), ("bound", "achieved", "peak", "unit", "frac", "traffic", "traffic_source", "kernel",
+                                         "kernel_ms", "kernel_share_of_step", "work", "flop_per_interaction",
+                                         "fp64_inst_per_interaction", "frac_executed", "frac_nominal", "fp64_issue_frac",
+                                         "fp64_pipe_pct_ncu", "store_stream_gb_s", "peak_source", "note"))
+    if roof:
+        for k, n in (("traffic_source", 150), ("peak_source", 100), ("note", 120)):
+            if k in roof:
+                roof[k] = _clip(roof[k], n)
+    line["roofline"] = roof
+    cpu = _pick(full.get("cpu_baseline"), ("value", "unit", "cores", "threads_busy", "kind", "sample", "value_single_thread"))
+    if cpu and "sample" in cpu:
+        cpu["sample"] = _clip(cpu["sample"], 120)
+    line["cpu_baseline"] = cpu
+    if full.get("solve"):
+        line["solve"] = _pick(full["solve"], ("matvecs", "rel_residual", "converged", "capacitance_over_4pi_eps0_R"))
+    if full.get("secondary"):
+        rows = []
+        for e in full["secondary"][:8]:
+            rf = e.get("roofline") or {}
+            rows.append({"name": _clip(e.get("name") or e.get("workload", ""), 40), "ms_per_step": e.get("ms_per_step"),
+                         "value": e.get("value"), "frac": rf.get("frac")})
+        line["secondary"] = rows
+        line["secondary_def"] = "other configs, device-timed: value in matrix entries/s (fill) or element.point/s; frac as roofline.frac"
+    if detail_path:
+        line["detail"] = detail_path
+    line = _sig(line)
+    if len(json.dumps(line)) >= LINE_LIMIT:      # never print a record the driver cannot keep: drop the optional parts
+        for k in ("secondary", "secondary_def", "solve"):
+            line.pop(k, None)
+    return line
+
+
+def emit(full: dict, detail_path=None):
+    """Full record -> `detail_path` (best effort), compact record -> the one stdout line."""
+    wrote = None
+    if detail_path:
+        try:
+            os.makedirs(os.path.dirname(os.path.abspath(detail_path)) or ".", exist_ok=True)
+            with open(detail_path, "w") as f:
+                json.dump(full, f, indent=1)
+            wrote = detail_path
+        except OSError:
+            wrote = None
+    print(json.dumps(contract_line(full, wrote)), flush=True)
 
 
 # --------------------------------------------------------------------------------------------
@@ -580,18 +689,25 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "source": "bemcub_inner_loop_rate: Eq. 4.1 loop (18 FP64 instr + MUFU, 8 of 18 are FMAs => at most 26/36 = 72.2% "
                       "of the FLOP peak), resident data"}
         if paired:
-            roof["paired_form"] = ("rectangle rules evaluated in +- point pairs (kernels_paired.cuh): the same point-charge "
-                                   "interactions of Eq. 4.1 (26 flop each by the plain count, which `achieved` and `frac` use) with "
-                                   "%.2f instead of 18 FP64 instructions per interaction, so the 26/36 = 72.2 %% cap of the plain "
-                                   "instruction mix does not bind; fp64_issue_frac_arith uses the executed count; "
-                                   "inner_loop_ceiling is the PLAIN loop's rate" % ipi)
+            roof["paired_form"] = ("rectangle rules evaluated in +- point pairs and the 7-point triangle rule on its medians "
+                                   "(kernels_paired.cuh): the same point-charge interactions of Eq. 4.1, %.2f instead of 18 FP64 "
+                                   "instructions each, so the 26/36 = 72.2 %% cap of the plain instruction mix does not bind `frac`; "
+                                   "fp64_issue_frac uses the executed count; inner_loop_ceiling is the PLAIN loop's rate" % ipi)
         roof["peak_sweep"] = peak["sweep"]
         if is_matrix:
             roof["store_stream_gb_s"] = float(n) * n * 8 / (k_ms * 1e-3) / 1e9
-        if args.workload in NCU_PIPE and args.scale == 1.0 and not args.gradient:
-            roof["ncu_fp64_pipe_counter"] = {"file": NCU_PIPE[args.workload][0], "metric": NCU_PIPE[args.workload][1],
-                                             "note": "hardware counter of a committed capture of this launch configuration, "
-                                                     "not of this run"}
+        cap = ncu_capture(args.workload, kernel) if (args.scale == 1.0 and not args.gradient) else None
+        if cap:
+            mt = cap["metrics"]
+            if "dram__bytes_read.sum" in mt and "dram__bytes_write.sum" in mt:
+                roof["traffic"] = mt["dram__bytes_read.sum"] + mt["dram__bytes_write.sum"]
+                roof["traffic_source"] = ("dram__bytes_read.sum + dram__bytes_write.sum of one launch, committed ncu capture "
+                                          f"{cap['file']} (same launch configuration; not this run)")
+            if NCU_PIPE_METRIC in mt:
+                roof["fp64_pipe_pct_ncu"] = mt[NCU_PIPE_METRIC]
+                roof["ncu_fp64_pipe_counter"] = {"file": cap["file"], "metric": NCU_PIPE_METRIC,
+                                                 "note": "hardware counter of a committed capture of this launch configuration, "
+                                                         "not of this run"}
 
     # end to end through the host-buffer C-ABI calls: H2D of the inputs, compute, D2H of Phi/E
     e2e = None
@@ -644,7 +760,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         r = None
         del phi, E
         torch.cuda.empty_cache()
-        secondary = secondary_block(args, b, torch, local_rank, peak, num_sms, barrier)
+        try:
+            secondary = secondary_block(args, b, torch, local_rank, peak, num_sms, barrier)
+        except Exception as exc:     # the contract record does not depend on the side runs
+            secondary = [{"workload": "secondary block failed", "error": repr(exc)[:200]}]
 
     if rank == 0:
         line = {
@@ -673,7 +792,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                                         "solve.matvec_roofline (HBM-bound); value counts every mat-vec as n^2 element.point pairs"
                                         if args.store_matrix else
                                         "kernel_ms / interactions are those of the LAST mat-vec of the solve")
-        print(json.dumps(line), flush=True)
+        emit(line, args.detail_out)
     if r is not None:
         r.close()
 
