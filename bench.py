@@ -960,6 +960,10 @@ def run_accuracy(args, b, torch, dev_index: int, barrier):
 
 def main():
     args = parse_args()
+    from paper_1606_03743_b200 import build as _libbuild
+    if args.impl == "ours" and _libbuild.override_refused():
+        raise SystemExit("bench.py: BEMCUB_LIB is set (%s): the bench times the library built from csrc/; unset it, or set "
+                         "BEMCUB_LIB_ALLOW=1 to time that binary on purpose" % os.environ["BEMCUB_LIB"])
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

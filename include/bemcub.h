@@ -83,7 +83,8 @@ enum {
   BEMCUB_ERR_NOMEM = -6,
   BEMCUB_ERR_NO_ELEMENTS = -7,        /* eval/assemble before a successful set_elements    */
   BEMCUB_ERR_NOT_CONVERGED = -8,      /* bemcub_solve: mat-vec limit reached (outputs valid) */
-  BEMCUB_ERR_FIXED_SCRATCH = -9       /* bemcub_eval_few_noalloc: more than its fixed scratch holds */
+  BEMCUB_ERR_FIXED_SCRATCH = -9,      /* bemcub_eval_few_noalloc: more than its fixed scratch holds */
+  BEMCUB_ERR_TOO_MANY_ELEMENTS = -10  /* bemcub_assemble*: mesh of more than 2^25 elements         */
 };
 
 /* Distance-ratio policy (Sec. 4).  dr[t][b], t = element type, are the UPPER distance-ratio
@@ -237,7 +238,10 @@ int bemcub_eval_linear(bemcub_ctx* ctx, const double* sigma_vertex, int rule_id,
  * the self term has D = 0 and is analytic).  Units V m^2 / C.  ld >= n.  The policy's
  * allow_upgrade is honoured per 32-row group of a 128-row tile.  Asynchronous.
  * bemcub_assemble_rows fills rows [row0, row0+nrows) only, into out_rows[(i-row0)*ld + j]
- * (row sharding across GPUs; sampling). */
+ * (row sharding across GPUs; sampling).
+ * Limit: the mesh may have at most 2^25 = 33,554,432 elements (the fill kernel's queue of near pairs keeps
+ * the column index in 25 bits) - also for a window of a few rows of a larger mesh; beyond it both calls
+ * return BEMCUB_ERR_TOO_MANY_ELEMENTS and write nothing (the evaluation calls have no such limit). */
 int bemcub_assemble(bemcub_ctx* ctx, const bemcub_policy* host_policy, double* out_matrix, int64_t ld);
 int bemcub_assemble_rows(bemcub_ctx* ctx, const bemcub_policy* host_policy, int64_t row0, int64_t nrows,
                          double* out_rows, int64_t ld);

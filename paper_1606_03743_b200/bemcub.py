@@ -50,6 +50,10 @@ def _load() -> C.CDLL:
         except Exception as exc:  # no nvcc on this box and no prebuilt library
             if not Path(path).exists():
                 raise ImportError(f"libbemcub.so is missing and could not be built: {exc}") from exc
+    if _build.override_active():
+        import sys
+        print(f"bemcub: BEMCUB_LIB is set - loading {path}, which is NOT rebuilt from csrc/ and may not match it",
+              file=sys.stderr, flush=True)
     lib = C.CDLL(str(path))
     vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
     PP = C.POINTER(bemcub_policy)
@@ -187,6 +191,7 @@ def bemcub_eval(ctx, sigma, rule_id: int, policy, m: int, field_pts, out_phi, ou
 
 
 ERR_FIXED_SCRATCH = -9
+ERR_TOO_MANY_ELEMENTS = -10
 NOALLOC_MAX_M = 64
 
 

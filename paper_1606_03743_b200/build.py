@@ -14,7 +14,9 @@ from pathlib import Path
 
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
-# BEMCUB_LIB: load another build of the same library (A/B timing of kernel variants); never rebuilt
+# BEMCUB_LIB: load another build of the same library (A/B timing of kernel variants); never rebuilt, so it
+# may not match csrc/ - the binding says so on stderr when it loads it, and the tests and bench.py refuse it
+# unless BEMCUB_LIB_ALLOW=1 is set as well (override_active / override_refused below)
 LIB = Path(os.environ["BEMCUB_LIB"]) if os.environ.get("BEMCUB_LIB") else PKG / "libbemcub.so"
 SOURCES = [CSRC / "bemcub.cu"]
 DEPS = sorted(CSRC.glob("*.cu*")) + sorted(CSRC.glob("*.h")) + sorted(CSRC.glob("*.inl")) + [PKG.parent / "include" / "bemcub.h"]
@@ -23,6 +25,15 @@ NVCC_FLAGS = [
     "-shared", "-Xcompiler", "-fPIC", "-O3", "-std=c++17",
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
 ]
+
+
+def override_active() -> bool:
+    return bool(os.environ.get("BEMCUB_LIB"))
+
+
+def override_refused() -> bool:
+    """True where results must describe the sources in this tree (tests, bench.py) and BEMCUB_LIB points elsewhere."""
+    return override_active() and os.environ.get("BEMCUB_LIB_ALLOW") != "1"
 
 
 def nvcc_path() -> str:

@@ -213,6 +213,15 @@ int upload_pair_tables(int np_out[5]) {
     }
     np[l] = ok ? k : 0;
     if (!ok) cw[l] = 0.0;
+    // eval_paired_kernel's consume_stage is instantiated per level for exactly these pair counts, with / without
+    // a centre point (kernels_paired.cuh); a table that pairs differently is left to the plain point records
+    static const int kPairsOfLevel[5] = {2, 3, 6, 8, 16};
+    static const bool kCentreOfLevel[5] = {false, true, false, true, true};
+    if (np[l] != 0 && (np[l] != kPairsOfLevel[l] || (cw[l] != 0.0) != kCentreOfLevel[l])) {
+      np[l] = 0;
+      cw[l] = 0.0;
+      for (int k2 = 0; k2 < 16 * 4; ++k2) tab[4 * 16 * l + k2] = 0.0;
+    }
   }
   CUDA_TRY(cudaMemcpyToSymbol(c_pair_tab, tab, sizeof(tab)));
   CUDA_TRY(cudaMemcpyToSymbol(c_pair_center_w, cw, sizeof(cw)));
@@ -497,6 +506,8 @@ const char* bemcub_strerror(int code) {
     case BEMCUB_ERR_NOMEM: return "out of device memory";
     case BEMCUB_ERR_NO_ELEMENTS: return "no mesh: call bemcub_set_elements first";
     case BEMCUB_ERR_NOT_CONVERGED: return "iteration stopped at the mat-vec limit before reaching the tolerance";
+    case BEMCUB_ERR_TOO_MANY_ELEMENTS:
+      return "matrix fill: the mesh has more than 2^25 = 33,554,432 elements (columns), even for a window of a few rows";
     case BEMCUB_ERR_FIXED_SCRATCH:
       return "bemcub_eval_few_noalloc: beyond its fixed scratch (at most 64 field points per call, devices of at most 160 SMs)";
   }
@@ -1033,7 +1044,8 @@ int bemcub_assemble_rows(bemcub_ctx* c, const bemcub_policy* host_policy, int64_
                          int64_t ld) {
   if (!c) return BEMCUB_ERR_INVALID_ARG;
   if (!c->has_mesh) return BEMCUB_ERR_NO_ELEMENTS;
-  if (row0 < 0 || nrows < 0 || row0 + nrows > c->n || ld < c->n || c->n > kAsmMaxN) return BEMCUB_ERR_INVALID_ARG;
+  if (row0 < 0 || nrows < 0 || row0 + nrows > c->n || ld < c->n) return BEMCUB_ERR_INVALID_ARG;
+  if (c->n > kAsmMaxN) return BEMCUB_ERR_TOO_MANY_ELEMENTS;  // the kernel's near-pair queue packs the column into 25 bits
   PolicyDev pol;
   int rc = build_policy(host_policy, &pol);
   if (rc) return rc;

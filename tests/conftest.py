@@ -12,6 +12,11 @@ GOLDEN = os.path.join(ROOT, "tests", "golden")
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on a B200)")
+    # a leftover BEMCUB_LIB would make every parity result describe some other binary than csrc/ at HEAD
+    from paper_1606_03743_b200 import build
+    if build.override_refused():
+        raise pytest.UsageError("BEMCUB_LIB is set (%s): the tests check the library built from csrc/; unset it, or set "
+                                "BEMCUB_LIB_ALLOW=1 to test that binary on purpose" % os.environ["BEMCUB_LIB"])
 
 
 def read_golden(name):

@@ -86,3 +86,15 @@ def test_rule_info_errors():
     p = bemcub.bemcub_default_policy(False)
     assert [p.dr[0][i] for i in range(5)] == [3, 8, 20, 80, 1500]
     assert p.allow_upgrade == 1 and p.use_levels_mask == 63
+
+
+def test_limit_errors_say_what_the_limit_is():
+    """A refused size names its limit (bemcub.h documents both next to the calls they belong to)."""
+    from paper_1606_03743_b200 import bemcub
+    assert "2^25" in bemcub.bemcub_strerror(bemcub.ERR_TOO_MANY_ELEMENTS)
+    assert "64 field points" in bemcub.bemcub_strerror(bemcub.ERR_FIXED_SCRATCH)
+    hdr = open(os.path.join(ROOT, "include", "bemcub.h")).read()
+    assert "BEMCUB_ERR_TOO_MANY_ELEMENTS" in hdr and "2^25" in hdr
+    codes = dict(re.findall(r"(BEMCUB_ERR_[A-Z_]+) = (-\d+)", hdr))
+    for name, val in codes.items():
+        assert bemcub.bemcub_strerror(int(val)) != "unknown error code", name
