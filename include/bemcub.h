@@ -121,6 +121,10 @@ typedef struct {
                                /* last eval/assemble executed: 18 (Phi+E), 12 (Phi), 28     */
                                /* (+gradient) per interaction; fewer where rules ran in      */
                                /* paired / median form (BEMCUB_PATH_PAIRED); 0 for FP32     */
+  int64_t field_points_per_lane; /* R of the last bemcub_eval* call's kernel: the template      */
+                               /* instantiation it ran (1, 2, 4; paired 1, 3, 5); tiles hold   */
+                               /* 32 R field points; 0 for calls with m <= 64 (the tests use   */
+                               /* it to know which instantiation a parity case reached)        */
 } bemcub_stats;
 
 /* device: CUDA device ordinal.  cuda_stream: a cudaStream_t cast to void* (NULL = default).    */

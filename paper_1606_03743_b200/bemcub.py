@@ -33,7 +33,8 @@ class bemcub_policy(C.Structure):
 class bemcub_stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_int64), ("point_interactions", C.c_int64),
                 ("analytic_pairs", C.c_int64), ("last_eval_launches", C.c_int64),
-                ("kernel_cycles", C.c_int64), ("kernel_ns", C.c_int64), ("fp64_instructions", C.c_int64)]
+                ("kernel_cycles", C.c_int64), ("kernel_ns", C.c_int64), ("fp64_instructions", C.c_int64),
+                ("field_points_per_lane", C.c_int64)]
 
 
 class BemcubError(RuntimeError):

@@ -798,6 +798,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
     mark(c, 2);
     mark(c, 3);  // a6 (sum over the CTAs, k) happens in the last CTA of every pass
     c->last_path = BEMCUB_PATH_FEW;
+    c->stats.field_points_per_lane = 0;
     c->last_ipi = out_E ? 18 : 12;
     c->timing_valid = c->timing;
     c->counters_pending = true;
@@ -967,6 +968,7 @@ int eval_common(bemcub_ctx* c, const double* sigma, int rule_id, const bemcub_po
   }
 
   c->last_path = !adaptive ? BEMCUB_PATH_FIXED : paired ? BEMCUB_PATH_PAIRED : BEMCUB_PATH_ADAPTIVE;
+  c->stats.field_points_per_lane = sp.R;
   c->last_ipi = precision != BEMCUB_F64 ? 0 : grad ? 28 : out_E ? 18 : 12;
   mark(c, 2);
   // a6: cross-split reduction and the 1/(4 pi eps0) prefactor

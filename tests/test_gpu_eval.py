@@ -85,8 +85,8 @@ def test_cfg1_icosphere_n7_f64():
 @pytest.mark.parametrize("level", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("precision", [0, 1])
 def test_cfg2_cube_all_rules(level, precision):
-    m = 10000 if level <= 1 else 3000
-    c = synth.config2(m=m)
+    c = synth.config2()                        # the configuration's full 10^4 field points at every rule
+    assert len(c["pts"]) == 10000
     g = Gpu(c["etype"], c["verts"])
     phi, E = g.eval(c["sigma"], c["pts"], level, precision=precision)
     ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], level)
@@ -257,6 +257,8 @@ def test_cfg4_full_size_sampled():
     g = Gpu(c["etype"], c["verts"])
     pol = _policy(g.b, True, 1)
     phi, E = g.eval(c["sigma"], c["pts"], -1, policy=pol)
+    assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_PAIRED       # the kernel bench.py times ...
+    assert g.stats()["field_points_per_lane"] == 5                     # ... in the instantiation it times: <5, 8>
     assert np.all(np.isfinite(phi)) and np.all(np.isfinite(E))
     ppp_upgrade = g.stats()["point_interactions"] / (float(n) * m)
     # Morton order of the field points, recomputed here (30-bit keys on the bounding box, as DESIGN.md

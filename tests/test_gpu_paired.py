@@ -110,8 +110,15 @@ def test_pairs_down_to_a_distance_ratio_of_two_and_the_fallback():
     dr_low[1, 0] = 1.9
     phi, E = g.eval(sigma, pts, -1, policy=g.b.make_policy(dr_low, 0))
     assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_ADAPTIVE
+    assert g.stats()["field_points_per_lane"] == 2                    # eval_adaptive_kernel<double, 2>: 22000 points
+    ref_low = oracle.evaluate(etype, verts, sigma, pts, -1, dr=dr_low, want_counts=True)
+    _split_parity(phi, E, ref_low, "fallback: rectangle analytic limit 1.9")
+    assert g.stats()["point_interactions"] == int(ref_low["npi"].sum())
     phi, E = g.eval(sigma, pts, -1, policy=g.b.make_policy(dr, 0, 0b011111))
     assert g.b.bemcub_last_path(g.ctx.handle) == g.b.PATH_ADAPTIVE
+    ref_cub = oracle.evaluate(etype, verts, sigma, pts, -1, dr=dr, levels_mask=0b011111, want_counts=True)
+    _split_parity(phi, E, ref_cub, "fallback: no analytic branch")
+    assert g.stats()["point_interactions"] == int(ref_cub["npi"].sum())
     g.close()
 
 
