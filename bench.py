@@ -44,7 +44,7 @@ FP64_LANES_PER_SM = 64          # B200: one FP64 warp instruction per scheduler 
 METRIC = "FP64 Phi+E element.point interactions/s"
 UNIT = "element.point interactions/s"
 # committed ncu capture of ONE launch of the bench's own launch configuration (hardware counters; not measured by this run)
-NCU_CAPTURE = {"cfg4": ("profiles/r2_cfg4_full_eval_paired_counters.csv", "eval_paired_kernel")}
+NCU_CAPTURE = {"cfg4": ("profiles/r3_cfg4_full_eval_paired_counters.csv", "eval_paired_kernel")}
 NCU_PIPE_METRIC = "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed"
 LINE_LIMIT = 4096               # bytes of the stdout record (the driver keeps a tail of stdout: round 2's 20 KB line did not parse)
 
