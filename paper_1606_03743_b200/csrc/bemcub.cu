@@ -336,7 +336,12 @@ struct SplitPlan {
 SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) {
   SplitPlan s;
   const int64_t warps = (int64_t)c->num_sms * kWarpsPerCta;
-  const int64_t max_by_len = std::max<int64_t>(1, c->n / 64);
+  // shortest split: 64 elements where the rule is chosen per batch of 32 (adaptive), 32 elements for a fixed rule.
+  // Round 3, fixed rule with 32 instead of 64: config 2 (6144 squares x 1e4 points) gets R = 2 and 30144 items,
+  // kernel 0.504 -> 0.495 ms (N = 7), 2.311 -> 2.265 ms (N = 33); config 1 (1280 x 1000) 1280 instead of 640 items for
+  // 1776 warps, kernel 38.8 -> 24.5 us; 1.5e6 x 1e4 unchanged (116.2 ms).  Asking for 8 instead of 16 items per warp,
+  // or one CTA per item for grids below the SM count, changed nothing measurable.
+  const int64_t max_by_len = std::max<int64_t>(1, c->n / (adaptive ? 64 : 32));
   s.R = 1;
   // Largest R that still leaves enough items per warp.  A fixed rule only gains from a larger R
   // (more chains per lane), so it may use many splits; in adaptive mode a larger tile of FEW field

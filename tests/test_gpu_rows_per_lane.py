@@ -40,10 +40,11 @@ def _split_parity(phi, E, ref, tol, what):
 
 
 # ------------------------------------------------------------------ eval_fixed_kernel<T, R, Phi+E | Phi>
-@pytest.mark.parametrize("scale,level,want_R", [(0.04, 1, 4), (0.02, 3, 2)])
+@pytest.mark.parametrize("scale,level,want_R", [(0.04, 1, 4), (0.01, 3, 2)])
 def test_fixed_rule_R4_and_R2(scale, level, want_R):
-    """40000 (R = 4) / 19909 (R = 2) mixed elements x 10010 track points: 79 tiles of 128 (the last holds 26)
-    or 157 tiles of 64 (the last 26); FP64 and FP32, Phi + E and Phi only."""
+    """40000 (R = 4) / 10000 (R = 2) mixed elements x 10010 track points: 79 tiles of 128 (the last holds 26)
+    or 157 tiles of 64 (the last 26); FP64 and FP32, Phi + E and Phi only.  (plan_splits: tiles x min(n / 32,
+    512) splits must reach 16 items for each of the 1776 warps: 79 x 512 does, 79 x 312 does not, 157 x 312 does.)"""
     c = synth.config4(scale=scale, ntracks=10, npts_per_track=1001)
     m = len(c["pts"])
     assert m % (32 * want_R) != 0
