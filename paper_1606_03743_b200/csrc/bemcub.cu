@@ -348,7 +348,10 @@ SplitPlan plan_splits(const bemcub_ctx* c, int64_t m, int max_r, bool adaptive) 
   // points is also a looser tile (more upgraded elements), so R grows only when tiles are plentiful
   // (measured on 1.5e6 elements x 1e4 points: fixed rule +4 % with R = 4, adaptive -5 %; round 2, forcing
   // R = 4: that shape -6 %, the mat-vec of the level-5 icosphere solve -6 %).
-  const int64_t split_cap = adaptive ? 64 : 512, per_warp = adaptive ? 8 : 16;
+  // (a fixed rule on a mesh of at most 64 elements - config 5's single element x 1e6 points: the items are so short
+  // that their fixed cost counts, not their balance, so 4 items per warp are enough for a larger R: kernel 35.1 -> 22.5 us
+  // at N = 7, 61.4 -> 55.3 us at N = 33)
+  const int64_t split_cap = adaptive ? 64 : 512, per_warp = adaptive ? 8 : (c->n <= 64 ? 4 : 16);
   for (int R = max_r; R > 1; R >>= 1) {
     const int64_t nt = (m + 32 * R - 1) / (32 * R);
     if (nt * std::min<int64_t>(max_by_len, split_cap) >= per_warp * warps) {

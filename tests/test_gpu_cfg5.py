@@ -46,6 +46,7 @@ def cfg5(request):
 def test_parity_and_accuracy(cfg5, level, precision):
     c, g, phi_x, E_x = cfg5
     phi, E = g.eval(c["sigma"], c["pts"], level, precision=precision)
+    assert g.stats()["field_points_per_lane"] == 4      # eval_fixed_kernel<T, 4>: 7813 tiles of 128, the last of 64
     ref = oracle.evaluate(c["etype"], c["verts"], c["sigma"], c["pts"], level)
     err = parity_errors(phi, E, ref)
     tol = TOL_F32 if precision else TOL_F64
